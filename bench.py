@@ -1,0 +1,281 @@
+#!/usr/bin/env python
+"""bench.py -- photon packages/s and shell-crossings/s of the DIES hot path on B200 (BASELINE.json metric).
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--workload config2] [--packages P]
+
+A "step" is one pass of the whole hot path over one batch of synthetic input: dies_run on config 2 (externally
+heated sphere, 100 shells, 200 frequencies, 1e7 packages, full IRE).  `value` is timed with CUDA events around
+dies_run with the model resident in HBM; `e2e` times create_model + set_sources + run + get_temperature +
+get_escape_spectrum through the C ABI with host buffers.  Full IRE on one model does not shard (DESIGN.md,
+"Multi-GPU": replicas only): with --gpus N every rank runs an independent replica (its own seed).
+--impl reference times the CPU oracle (oracle/, test infrastructure) on a bounded sample of the same workload.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+from paper_2408_13807_b200 import synth  # noqa: E402
+
+# Algorithmic thread-instructions per unit of work, read from the SASS of the shipped tracker kernel
+# (straight-line path of each unit, profiles/ and DESIGN.md "Roofline"): crossing, scattering, absorption, package.
+INSTR = dict(crossing=24, scattering=230, absorption=330, package=210)
+SM_COUNT, SCHEDULERS, LANES = 148, 4, 32
+
+
+def load_peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        d = json.load(open(path))
+        return float(d.get("sm_max_mhz", 1965.0)), "measured sm_max_mhz of MEASURED_PEAKS.json"
+    return 1965.0, "fallback clocks.max.sm of B200_PROFILING.md"
+
+
+def make_problem(workload, packages):
+    if workload == "config1":
+        p = synth.config1()
+    elif workload == "config2":
+        p = synth.config2()
+    elif workload == "config2_kbg":
+        p = synth.config2(k_bg=0.2)
+    elif workload == "config3":
+        p = synth.config3()
+    elif workload == "config3_thick":
+        p = synth.config3(tau_V=1000.0)
+    elif workload == "config4":
+        p = synth.config4()
+    elif workload == "config4_noffi":
+        p = synth.config4(ffi=0)
+    else:
+        raise SystemExit(f"unknown workload {workload}")
+    if packages:
+        p.n_packages = int(packages)
+    return p
+
+
+class ClockSampler:
+    """nvidia-smi clocks and throttle reasons DURING the timed region (B200_PROFILING.md recipe)."""
+
+    def __init__(self, index):
+        self.rows, self.proc, self.index = [], None, index
+
+    def start(self):
+        q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+             "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+             "clocks_event_reasons.sw_power_cap")
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--query-gpu={q}", "--format=csv,noheader,nounits",
+                                          "-i", str(self.index), "-lms", "50"], stdout=subprocess.PIPE, text=True)
+            self.t = threading.Thread(target=self._read, daemon=True)
+            self.t.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append(line.strip())
+
+    def stop(self):
+        if not self.proc:
+            return dict(sm_mhz=None, sm_max_mhz=None, reasons=["nvidia-smi unavailable"])
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except Exception:
+            self.proc.kill()
+        sm, mx, reasons = [], [], set()
+        for r in self.rows:
+            f = [x.strip() for x in r.split(",")]
+            if len(f) < 7:
+                continue
+            try:
+                sm.append(float(f[0])); mx.append(float(f[1]))
+            except ValueError:
+                continue
+            for name, v in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), f[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(name)
+        return dict(sm_mhz=float(np.median(sm)) if sm else None, sm_max_mhz=max(mx) if mx else None,
+                    reasons=sorted(reasons), samples=len(sm))
+
+
+def oracle_rate(p, n_sample, seed=1):
+    """The oracle as it stands on one host core: packages/s and crossings/s on a bounded sample."""
+    from oracle import dies_oracle as orc
+    o = orc.Oracle(p)
+    t0 = time.perf_counter()
+    o.run(n_sample, seed=seed, k_bg=p.k_bg, ffi=p.ffi)
+    dt = time.perf_counter() - t0
+    c = o.counters
+    return n_sample / dt, c["crossings"] / dt, dt, c
+
+
+def run_reference(args, rank, world):
+    if rank != 0:
+        return
+    p = make_problem(args.workload, args.packages)
+    n_sample = min(p.n_packages, args.ref_sample)
+    for _ in range(args.warmup):
+        oracle_rate(p, max(1, n_sample // 10))
+    times, cross = [], 0
+    for s in range(args.steps):
+        r, cr, dt, c = oracle_rate(p, n_sample, seed=1 + s)
+        times.append(dt); cross += c["crossings"]
+    tot = float(np.sum(times))
+    value = n_sample * args.steps / tot
+    line = dict(impl="reference", metric="packages_per_s", value=value, unit="packages/s", n_gpus=args.gpus,
+                steps=args.steps, warmup=args.warmup, ms_per_step=1e3 * tot / args.steps, higher_is_better=True,
+                scaling="weak", vs_baseline=None, dtype="f64", data="synthetic",
+                crossings_per_s=cross / tot,
+                config=dict(workload=args.workload, n_shells=p.n_shells, n_freq=p.n_freq, n_T=p.n_T,
+                            packages_per_step=n_sample, mode="full IRE", note="serial CPU oracle on a bounded sample"),
+                cpu_baseline=dict(value=value, unit="packages/s", cores=1, kind="oracle",
+                                  sample=f"{n_sample} packages of {args.workload} per step, {args.steps} steps"),
+                e2e=dict(value=value, unit="packages/s", h2d_bytes_per_step=0, d2h_bytes_per_step=0),
+                gpu_launches=0)
+    print(json.dumps(line))
+
+
+def run_ours(args, rank, world, local_rank):
+    import torch
+    import torch.distributed as dist
+    from paper_2408_13807_b200 import binding as dies
+
+    dev = torch.device(f"cuda:{local_rank}")
+    torch.cuda.set_device(dev)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+    p = make_problem(args.workload, args.packages)
+    n = p.n_packages
+    opts = dict(k_bg=p.k_bg, ffi=p.ffi)
+    m = dies.Model(p, device=str(dev))
+    info = dies.dies_device_info()
+    stream = torch.cuda.current_stream(dev)
+    flush = torch.empty(256 * 1024 * 1024, dtype=torch.uint8, device=dev)   # > 126 MB L2
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize(dev)
+
+    for w in range(args.warmup):
+        m.dies_run(n, seed=1000 + w + 7919 * rank, **opts)
+    torch.cuda.synchronize(dev)
+    c0 = m.dies_get_counters()
+
+    # ---- device-timed steps: CUDA events on the launching stream, L2 flushed between steps
+    sampler = ClockSampler(local_rank)
+    sampler.start()
+    barrier()
+    t_wall = time.perf_counter()
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    tot_counts = dict(crossings=0, scatterings=0, absorptions=0, packages=0)
+    for s in range(args.steps):
+        flush.fill_(s & 0xFF)
+        ev[s][0].record(stream)
+        m.dies_run(n, seed=1 + s + 7919 * rank, **opts)
+        ev[s][1].record(stream)
+    barrier()
+    t_wall = time.perf_counter() - t_wall
+    clocks = sampler.stop()
+    ms = [a.elapsed_time(b) for a, b in ev]
+    c1 = m.dies_get_counters()
+    # counters are zeroed by every non-accumulating run: c1 holds the last step; steps are statistically identical
+    for k in tot_counts:
+        tot_counts[k] = c1[k]
+    step_ms = float(np.sum(ms)) / args.steps
+    t = torch.tensor([float(np.sum(ms))], dtype=torch.float64, device=dev)
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    total_ms = float(t.item())
+    value = world * n * args.steps / (total_ms * 1e-3)
+    crossings_per_s = world * c1["crossings"] * args.steps / (total_ms * 1e-3)
+
+    # ---- end to end through the C ABI with host buffers: create + sources + run + both getters
+    e2e_t = []
+    for s in range(max(1, min(args.steps, 5))):
+        torch.cuda.synchronize(dev)
+        t0 = time.perf_counter()
+        m2 = dies.Model(p, device=str(dev))
+        m2.dies_run(n, seed=1 + s, **opts)
+        T = m2.dies_get_temperature()
+        Lesc = m2.dies_get_escape_spectrum()
+        e2e_t.append(time.perf_counter() - t0)
+        m2.close()
+    e2e_val = world * n / float(np.median(e2e_t))
+    h2d = 8 * (p.emis.size + p.T_grid.size + 3 * p.n_freq + p.r_bounds.size + p.rho.size + 2 * p.n_freq)
+    d2h = 8 * (p.n_shells + p.n_freq) + 64
+
+    if rank != 0:
+        return
+    sm_max, peak_src = load_peaks()
+    peak = SM_COUNT * SCHEDULERS * LANES * sm_max * 1e6 / 1e12          # thread-instructions/s, 1e12
+    work = (c1["crossings"] * INSTR["crossing"] + c1["scatterings"] * INSTR["scattering"] +
+            c1["absorptions"] * INSTR["absorption"] + c1["packages"] * INSTR["package"])
+    achieved = work / (step_ms * 1e-3) / 1e12
+    held = clocks.get("sm_mhz") or sm_max
+    line = dict(metric="packages_per_s", value=value, unit="packages/s", n_gpus=world, steps=args.steps,
+                warmup=args.warmup, ms_per_step=total_ms / args.steps, higher_is_better=True, scaling="weak",
+                vs_baseline=None, dtype="f32", data="synthetic",
+                crossings_per_s=crossings_per_s,
+                config=dict(workload=args.workload, n_shells=p.n_shells, n_freq=p.n_freq, n_T=p.n_T,
+                            packages_per_step=n, mode="full IRE", k_bg=p.k_bg, ffi=p.ffi,
+                            parallelism="replicas only" if world > 1 else "1 GPU", l2="flushed between steps (256 MiB fill)",
+                            per_package=dict(crossings=c1["crossings"] / n, scatterings=c1["scatterings"] / n,
+                                             absorptions=c1["absorptions"] / n),
+                            grid=dict(**info)),
+                clocks=clocks,
+                e2e=dict(value=e2e_val, unit="packages/s", h2d_bytes_per_step=int(h2d), d2h_bytes_per_step=int(d2h),
+                         ms_per_step=1e3 * float(np.median(e2e_t))),
+                gpu_launches=int(2 * args.steps),
+                roofline=dict(bound="alu", achieved=achieved, peak=peak, unit="Tinstr/s", frac=achieved / peak,
+                              frac_at_held_clock=achieved / (peak * held / sm_max), traffic=None,
+                              peak_source=f"148 SMs x 4 schedulers x 32 lanes x {sm_max:.0f} MHz ({peak_src})",
+                              instr_per_unit=INSTR, kernel="dies_track<0,false>", kernel_ms=step_ms),
+                wall_s=t_wall)
+    # ---- the oracle timed beside it on this box's host cores (rank 0, N = 1 only)
+    if world == 1 and not args.no_cpu_baseline:
+        r, cr, dt, c = oracle_rate(p, min(n, args.cpu_sample))
+        line["cpu_baseline"] = dict(value=r, unit="packages/s", cores=1, kind="oracle", crossings_per_s=cr,
+                                    sample=f"{min(n, args.cpu_sample)} packages of {args.workload} ({dt:.1f} s), serial fp64 oracle",
+                                    host_cores=os.cpu_count())
+    print(json.dumps(line))
+    m.close()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="config2")
+    ap.add_argument("--packages", type=float, default=0)
+    ap.add_argument("--cpu-sample", type=int, default=6_000_000)
+    ap.add_argument("--ref-sample", type=int, default=1_000_000)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    if args.impl == "reference":
+        run_reference(args, rank, world)
+    else:
+        if args.warmup < 3:
+            args.warmup = 3
+        run_ours(args, rank, world, local_rank)
+
+
+if __name__ == "__main__":
+    main()

@@ -1,0 +1,149 @@
+/*
+ * dies.h -- C ABI of libdies: the data-parallel hot path of DIES (arXiv 2408.13807) on one B200.
+ *
+ * Monte Carlo propagation of photon packages through a 1D spherically symmetric dust cloud of
+ * concentric shells with the immediate re-emission (IRE) method (section 2.1),
+ * with initial-direction weighting k_bg (Eq. 5) and forced first interaction (Eq. 9-12,
+ * L132-149).  Citations are lines of /root/reference/PAPER.md; "R<n>" are the readings of
+ * DESIGN.md.  Every step of the path runs in hand-written sm_100a CUDA kernels; there is no CPU
+ * fallback: every entry point that needs the device returns DIES_ECUDA when it is missing.
+ *
+ * Conventions
+ *  - All array arguments are caller-owned HOST pointers unless marked "device"; they are copied
+ *    during the call and never kept.  Getters write into caller-owned host buffers.
+ *  - The caller allocates the device workspace (dies_workspace_bytes) and keeps it alive until
+ *    dies_destroy; the library never allocates device memory for a model.
+ *  - All functions return DIES_OK (0) or a negative error code; dies_last_error() gives a
+ *    thread-local message.  Nothing is printed, nothing aborts.
+ *  - Units are the caller's; only consistency is required: kappa * rho * length dimensionless,
+ *    emis and L / (rho * volume) in the same power-per-dust-mass unit.
+ *  - A handle is not thread-safe; different handles are independent.
+ *  - Shells are numbered 0 (innermost) .. n_shells-1; frequency bins 0 .. n_freq-1.
+ *
+ * Random numbers (part of the parity contract): Philox4x32-10 with
+ * key = (seed lo32, seed hi32), counter = (package_id lo32, package_id hi32, block, model_index);
+ * block counts the 4-word blocks consumed by the package from 0; a 32-bit word x gives the
+ * uniform u = ((x >> 9) + 0.5) * 2^-23 in (0,1).
+ */
+#ifndef DIES_H
+#define DIES_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct dies_model dies_model;   /* opaque; owned by the library, freed by dies_destroy */
+
+enum {
+    DIES_OK = 0,
+    DIES_EINVAL = -1,      /* bad argument (sizes, ordering, sign, NULL) */
+    DIES_ENOMEM = -2,      /* workspace too small or host allocation failed */
+    DIES_ECUDA = -3,       /* CUDA runtime error or no sm_100 device */
+    DIES_ESTATE = -4,      /* call out of order (e.g. run before set_sources) */
+    DIES_EOVERFLOW = -5    /* a 64-bit tally exceeded 2^62 */
+};
+
+/* modes of dies_run */
+enum { DIES_MODE_IRE = 0, DIES_MODE_FIXED_T = 1 };
+
+/* event types of dies_trace_* (quadruples: type, shell, freq_bin, crossings so far) */
+enum { DIES_EV_LAUNCH = 0, DIES_EV_SCATTER = 1, DIES_EV_ABSORB = 2, DIES_EV_ESCAPE = 3,
+       DIES_EV_TERMINATE = 4, DIES_EV_UNINTERACTED = 5 };
+
+/* indices into the array filled by dies_get_counters */
+enum { DIES_C_PACKAGES = 0, DIES_C_CROSSINGS, DIES_C_FFI_CROSSINGS, DIES_C_SCATTERINGS, DIES_C_ABSORPTIONS,
+       DIES_C_ESCAPED, DIES_C_UNINTERACTED, DIES_C_TERMINATED, DIES_C_EXTRA_BLOCKS, DIES_C_CLAMP_HI_SAMPLES,
+       DIES_C_INJECTED_RAW, DIES_C_ESCAPED_RAW, DIES_C_TERMINATED_RAW, DIES_C_T_CLAMP_LO, DIES_C_T_CLAMP_HI,
+       DIES_C_KERNEL_LAUNCHES, DIES_N_COUNTERS };
+
+typedef struct {
+    double   k_bg;        /* Eq. 5: mu = u^k_bg, W = 2 k_bg mu^(2-1/k_bg); 0.5 = unweighted (Eq. 2)          */
+    int32_t  ffi;         /* Eq. 9-12: forced first interaction on the launch flight (R11)                  */
+    int32_t  mode;        /* DIES_MODE_IRE or DIES_MODE_FIXED_T (rows from dies_set_fixed_temperature)      */
+    int32_t  accumulate;  /* 0: zero tallies and counters first; 1: continue (package ids continue too)     */
+    int32_t  fixed_shift; /* S: a package of weight W adds round(W 2^S) to the 64-bit tallies; 0 -> 24      */
+    uint64_t n_total;     /* packages per source over the whole (possibly split) run; package energy is
+                             L_source / n_total (L51).  0 -> n_packages of this call                        */
+} dies_run_opts;
+
+/* Bytes of device workspace a model (n_models = 1) or a batch needs. */
+int dies_workspace_bytes(int n_shells, int n_freq, int n_T, int n_models, size_t* bytes);
+
+/* The model of PAPER.md L49 / L67-71 / L87: shells, dust, and the emission table behind the two lookup
+ * tables (absorbed energy -> temperature; (T_old, T_new, u) -> re-emitted frequency).
+ *   r_bounds  n_shells+1 strictly ascending, r_bounds[0] >= 0; r_bounds[0] > 0 is an empty cavity (R10)
+ *   rho       n_shells, >= 0, dust mass per volume
+ *   freq      n_freq ascending; labels only (frequencies are discrete bins, R3)
+ *   kappa_abs, kappa_sca  n_freq, >= 0, per dust mass; g_hg n_freq, |g| < 1 (Henyey-Greenstein, L167)
+ *   T_grid    n_T strictly ascending
+ *   emis      n_T x n_freq row-major, >= 0, power emitted per dust mass in bin k at T_t; rows must not
+ *             decrease with t in any bin and their sums must strictly increase
+ *   workspace_dev  DEVICE pointer, 256-byte aligned, workspace_bytes >= dies_workspace_bytes(...)
+ * Tables are built on the device during the call (which synchronises before returning). */
+int dies_create_model(int n_shells, const double* r_bounds, const double* rho,
+                      int n_freq, const double* freq,
+                      const double* kappa_abs, const double* kappa_sca, const double* g_hg,
+                      int n_T, const double* T_grid, const double* emis,
+                      void* workspace_dev, size_t workspace_bytes, dies_model** out);
+
+/* Config 5: n_models spheres of n_shells shells each sharing dust and emission tables.
+ *   r_bounds n_models x (n_shells+1), rho n_models x n_shells, row-major. */
+int dies_create_batch(int n_models, int n_shells, const double* r_bounds, const double* rho,
+                      int n_freq, const double* freq,
+                      const double* kappa_abs, const double* kappa_sca, const double* g_hg,
+                      int n_T, const double* T_grid, const double* emis,
+                      void* workspace_dev, size_t workspace_bytes, dies_model** out);
+
+/* Sources (L49-55).  ext_bin_intensity: n_freq bin-integrated mean intensities of the isotropic external
+ * field (luminosity 4 pi R^2 * pi * sum_k J_k), or NULL.  L_point > 0 with point_bin_weights (n_freq
+ * relative spectrum) is the central point source, else pass 0 / NULL.  Each active source gets n_total
+ * packages of equal energy (L51, R2): ids [0, n_total) external, then the point source. */
+int dies_set_sources(dies_model*, const double* ext_bin_intensity, double L_point, const double* point_bin_weights);
+/* Batch form: ext n_models x n_freq or NULL; L_point n_models or NULL; point weights n_models x n_freq or NULL. */
+int dies_set_sources_batch(dies_model*, const double* ext_bin_intensity, const double* L_point,
+                           const double* point_bin_weights);
+
+/* Follow n_packages packages per active source (per model) on `cuda_stream` (a cudaStream_t; NULL = default
+ * stream).  Asynchronous: returns after the launches.  opts == NULL means {0.5, 0, IRE, 0, 24, n_packages}. */
+int dies_run(dies_model*, uint64_t n_packages, uint64_t seed, const dies_run_opts* opts, void* cuda_stream);
+int dies_run_batch(dies_model*, uint64_t n_packages_per_model, uint64_t seed, const dies_run_opts* opts,
+                   void* cuda_stream);
+
+/* Dust temperatures from the absorbed-energy tallies (L87 lookup table; log-log interpolation, R6):
+ * T[n_models x n_shells]; n must equal that size.  Synchronises the stream of the last run. */
+int dies_get_temperature(dies_model*, double* T, int n);
+/* Escaping luminosity per frequency bin, n_models x n_freq (L87 last sentence; un-interacted FFI share included). */
+int dies_get_escape_spectrum(dies_model*, double* L_esc, int n);
+
+/* Parity-test support ---------------------------------------------------------------------------------- */
+/* Fixed-temperature tracking mode: shell i re-emits with the table row of T[i] (#{t: T_grid[t] <= T[i]}). */
+int dies_set_fixed_temperature(dies_model*, const double* T, int n);
+/* Raw 64-bit tallies (n_models x n_shells) and the energy per raw unit of each model (n_models). */
+int dies_get_absorbed(dies_model*, int64_t* raw, double* energy_per_raw_unit, int n);
+/* DIES_N_COUNTERS counters summed over models (see enum); n must be DIES_N_COUNTERS. */
+int dies_get_counters(dies_model*, uint64_t* c, int n);
+/* Replay packages first_id .. first_id+count-1 of model model_index against the current tallies (read only)
+ * and list their events: events[p][e] = (type, shell, freq_bin, crossings so far), at most max_events each;
+ * n_events[p] is the true number.  Runs the same device code as dies_run. */
+int dies_trace_packages(dies_model*, int model_index, uint64_t first_id, int count, uint64_t n_total, uint64_t seed,
+                        const dies_run_opts* opts, int32_t* events, int max_events, int32_t* n_events);
+int dies_trace_package(dies_model*, uint64_t package_id, uint64_t n_total, uint64_t seed, const dies_run_opts* opts,
+                       int32_t* events, int max_events, int32_t* n_events);
+/* The device Philox and uniform of the RNG contract: out[4*j..] = words of block `block` of package first_id+j. */
+int dies_test_philox(uint64_t seed, uint64_t first_id, uint32_t block, uint32_t model_index, int n,
+                     uint32_t* words, float* uniforms);
+/* Device tables as built (for table parity): eps n_T (double), F n_T x n_freq (float). Either may be NULL. */
+int dies_get_tables(dies_model*, double* eps, float* F);
+
+int dies_destroy(dies_model*);
+const char* dies_last_error(void);
+/* "sm_100a" build tag, number of SMs and resident blocks per SM of the tracker (for the bench log). */
+int dies_device_info(int* n_sms, int* blocks_per_sm, int* threads_per_block);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* DIES_H */

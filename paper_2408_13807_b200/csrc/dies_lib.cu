@@ -1,0 +1,762 @@
+// dies_lib.cu -- C ABI of libdies (include/dies.h): host argument checking, device table construction,
+// launches of the tracker (dies_tracker.cuh) and read-back.  Compiled for sm_100a only; no CPU fallback.
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <vector>
+
+#include "../../include/dies.h"
+#include "dies_tracker.cuh"
+
+using namespace dies;
+
+// ------------------------------------------------------------------ errors
+static thread_local char g_err[512] = "";
+static int fail(int code, const char* fmt, ...)
+{
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(g_err, sizeof(g_err), fmt, ap);
+    va_end(ap);
+    return code;
+}
+#define CUDA_TRY(expr)                                                                          \
+    do {                                                                                        \
+        cudaError_t e_ = (expr);                                                                \
+        if (e_ != cudaSuccess) return fail(DIES_ECUDA, "%s: %s", #expr, cudaGetErrorString(e_)); \
+    } while (0)
+
+extern "C" const char* dies_last_error(void) { return g_err; }
+
+// ------------------------------------------------------------------ workspace layout
+struct Layout {
+    size_t emis, eps, Tgrid, epsgrid, F, bintab, omega, dustin, rb, rho, mass, stab, cscale, srccdf, srcin, Lsrc, mp,
+        fixed_row, Tfix, A, esc, next_id, counters, ticket, T_out, Lesc_out, eunit, flags, epsref, total;
+};
+static size_t al(size_t x) { return (x + 255) & ~(size_t)255; }
+static Layout make_layout(int N, int K, int nT, int M)
+{
+    Layout L;
+    const size_t ldS = (size_t)N + 1;
+    size_t o = 0;
+    auto take = [&](size_t bytes) { size_t at = o; o = al(o + bytes); return at; };
+    L.emis = take((size_t)nT * K * 8);
+    L.eps = take((size_t)nT * 8);
+    L.Tgrid = take((size_t)nT * 8);
+    L.epsgrid = take((size_t)nT * 4);
+    L.F = take((size_t)nT * K * 4);
+    L.bintab = take((size_t)K * 16);
+    L.omega = take((size_t)K * 4);
+    L.dustin = take((size_t)3 * K * 8);
+    L.rb = take((size_t)M * (N + 1) * 8);
+    L.rho = take((size_t)M * N * 8);
+    L.mass = take((size_t)M * ldS * 8);
+    L.stab = take((size_t)M * 2 * (ldS + 1) * 8);
+    L.cscale = take((size_t)M * ldS * 8);
+    L.srccdf = take((size_t)M * 2 * K * 4);
+    L.srcin = take((size_t)M * 2 * K * 8);
+    L.Lsrc = take((size_t)M * 2 * 8);
+    L.mp = take((size_t)M * sizeof(ModelParams));
+    L.fixed_row = take((size_t)M * ldS * 4);
+    L.Tfix = take((size_t)M * N * 8);
+    L.A = take((size_t)M * ldS * 8);
+    L.esc = take((size_t)M * K * 8);
+    L.next_id = take((size_t)M * 8);
+    L.counters = take((size_t)DIES_N_COUNTERS * 8);
+    L.ticket = take(16);
+    L.T_out = take((size_t)M * N * 8);
+    L.Lesc_out = take((size_t)M * K * 8);
+    L.eunit = take((size_t)M * 8);
+    L.flags = take(64);
+    L.epsref = take(16);
+    L.total = o;
+    return L;
+}
+
+struct dies_model {
+    int N, K, nT, M, ldS;
+    Layout L;
+    unsigned char* ws;
+    DeviceModel D;
+    bool sources_set, fixed_set, ran;
+    std::vector<double> L_ext, L_point;   // per model
+    std::vector<int> has_ext, has_point;
+    unsigned long long done, n_total;     // packages per source already followed / planned
+    int shift;
+    cudaStream_t stream;
+    int grid_max, blocks_per_sm, n_sms;
+    size_t smem_bytes;
+    unsigned long long launches;
+};
+
+template <class T>
+static T* wsp(dies_model* m, size_t off) { return reinterpret_cast<T*>(m->ws + off); }
+
+// ------------------------------------------------------------------ table construction kernels
+// eps_t = sum_k emis[t][k];  F[t][k] = cumsum_k(emis[t] - emis[t-1]) / sum_k(emis[t] - emis[t-1])   (R4)
+__global__ void k_build_tables(const double* __restrict__ emis, int nT, int K, double* __restrict__ eps,
+                               float* __restrict__ F, int* flags)
+{
+    const int t = blockIdx.x * blockDim.x + threadIdx.x;
+    if (t >= nT) return;
+    const double* row = emis + (size_t)t * K;
+    const double* prev = t > 0 ? row - K : nullptr;
+    double s = 0.0, tot = 0.0;
+    bool bad = false;
+    for (int k = 0; k < K; k++) {
+        const double d = row[k] - (prev ? prev[k] : 0.0);
+        if (!(d >= 0.0)) bad = true;
+        s += row[k];
+        tot += d;
+    }
+    eps[t] = s;
+    if (bad || !(tot > 0.0)) atomicOr(flags, 1);
+    double c = 0.0;
+    float* f = F + (size_t)t * K;
+    for (int k = 0; k < K; k++) {
+        c += row[k] - (prev ? prev[k] : 0.0);
+        f[k] = (float)(c / tot);
+    }
+    f[K - 1] = 1.0f;
+}
+
+__global__ void k_build_epsgrid(const double* __restrict__ eps, int nT, float* __restrict__ grid, double* epsref,
+                                int* flags)
+{
+    const double ref = sqrt(eps[0] * eps[nT - 1]);
+    const int t = blockIdx.x * blockDim.x + threadIdx.x;
+    if (t == 0) *epsref = ref;
+    if (t >= nT) return;
+    if (t > 0 && !(eps[t] > eps[t - 1])) atomicOr(flags, 2);
+    grid[t] = (float)(eps[t] / ref);
+}
+
+// dust table: opacities in units of kappa_ref = max_k(kappa_abs + kappa_sca)
+__global__ void k_build_dust(const double* __restrict__ dustin, int K, double kref, float4* bintab, float* omega)
+{
+    const int k = blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= K) return;
+    const double ka = dustin[k] / kref, ks = dustin[K + k] / kref, g = dustin[2 * K + k];
+    bintab[k] = make_float4((float)(1.0 / ka), (float)(1.0 / ks), (float)g, (float)(ka + ks));   // 1/0 = inf: never hit
+    omega[k] = (ka + ks) > 0 ? (float)(ks / (ka + ks)) : 0.f;
+}
+
+// shells: lengths in units of the outer radius R, densities as rho^ = rho R kappa_ref; internal shell 0 is the
+// empty cavity when r_bounds[0] > 0 (R10)
+__global__ void k_build_shells(const double* __restrict__ rb, const double* __restrict__ rho, int N, int M, double kref,
+                               float2* stab, double* mass, ModelParams* mp)
+{
+    const int ldS = N + 1;
+    const int idx = blockIdx.x * blockDim.x + threadIdx.x;
+    if (idx >= M * (ldS + 1)) return;
+    const int m = idx / (ldS + 1), j = idx % (ldS + 1);
+    const double* r = rb + (size_t)m * (N + 1);
+    const double* d = rho + (size_t)m * N;
+    const double R = r[N];
+    const int cav = r[0] > 0.0 ? 1 : 0;
+    const int Np = N + cav;
+    float2* st = stab + (size_t)m * 2 * (ldS + 1);
+    if (j == 0) {
+        ModelParams p = mp[m];
+        p.Np = Np; p.cav = cav; p.r0hat = (float)(r[0] / R);
+        mp[m] = p;
+    }
+    double r_in = 0.0, r_out = 0.0, dens = 0.0;
+    if (j < Np) {
+        const int i = j - cav;                    // user shell, -1 = cavity
+        r_in = i < 0 ? 0.0 : r[i];
+        r_out = i < 0 ? r[0] : r[i + 1];
+        dens = i < 0 ? 0.0 : d[i];
+        if (i == 0 && cav == 0) r_in = 0.0;
+    } else {
+        r_in = R; r_out = R;                       // dummy entries read when a package escapes
+    }
+    const float x_in = (float)((r_in / R) * (r_in / R)), x_out = (float)((r_out / R) * (r_out / R));
+    const float dh = (float)(dens * R * kref);
+    st[2 * j] = make_float2(x_in, dh);
+    st[2 * j + 1] = make_float2(x_out, dh);
+    if (j < ldS) {
+        const double pi = 3.14159265358979323846;
+        mass[(size_t)m * ldS + j] = j < Np ? dens * (4.0 * pi / 3.0) * (r_out * r_out * r_out - r_in * r_in * r_in) : 0.0;
+    }
+}
+
+// source spectrum tables and luminosities: L_ext = 4 pi R^2 * pi * sum_k J_k
+__global__ void k_build_sources(const double* __restrict__ srcin, const double* __restrict__ rb, int N, int K, int M,
+                                float* srccdf, double* Lsrc)
+{
+    const int idx = blockIdx.x * blockDim.x + threadIdx.x;
+    if (idx >= 2 * M) return;
+    const int m = idx >> 1, which = idx & 1;
+    const double* w = srcin + ((size_t)m * 2 + which) * K;
+    float* cdf = srccdf + ((size_t)m * 2 + which) * K;
+    double tot = 0.0;
+    for (int k = 0; k < K; k++) tot += w[k];
+    if (which == 0) {
+        const double pi = 3.14159265358979323846;
+        const double R = rb[(size_t)m * (N + 1) + N];
+        Lsrc[2 * m] = 4.0 * pi * R * R * pi * tot;
+    }
+    double c = 0.0;
+    for (int k = 0; k < K; k++) {
+        c += w[k];
+        cdf[k] = tot > 0.0 ? (float)(c / tot) : 1.0f;
+    }
+    cdf[K - 1] = 1.0f;
+}
+
+// fixed-temperature rows: #{t : T_grid[t] <= T} clamped
+__global__ void k_fixed_rows(const double* __restrict__ Tfix, const double* __restrict__ Tgrid, int nT, int N, int M,
+                             const ModelParams* mp, int* fixed_row)
+{
+    const int idx = blockIdx.x * blockDim.x + threadIdx.x;
+    if (idx >= M * N) return;
+    const int m = idx / N, i = idx % N;
+    const double T = Tfix[idx];
+    int lo = 0, hi = nT;
+    while (lo < hi) { const int mid = (lo + hi) >> 1; if (Tgrid[mid] > T) hi = mid; else lo = mid + 1; }
+    fixed_row[(size_t)m * (N + 1) + i + mp[m].cav] = min(lo, nT - 1);
+}
+
+// per run: energy scale of the raw tallies, zeroing, counters
+__global__ void k_prepare_run(DeviceModel D, const double* __restrict__ mass, const double* __restrict__ Lsrc,
+                              const double* __restrict__ epsref, double* cscale, double* eunit, ModelParams* mp,
+                              double n_total, double qscale, int zero)
+{
+    const int ldS = D.ldS;
+    const int idx = blockIdx.x * blockDim.x + threadIdx.x;
+    if (idx == 0) { *D.ticket = 0u; if (zero) for (int c = 0; c < DIES_N_COUNTERS; c++) D.counters[c] = 0ull; }
+    if (idx < D.n_models) {
+        D.next_id[idx] = 0ull;
+        ModelParams p = mp[idx];
+        const double Le = p.has_ext ? Lsrc[2 * idx] : 0.0, Lp = p.has_point ? Lsrc[2 * idx + 1] : 0.0;
+        const double Lref = fmax(Le, Lp);
+        p.qs_ext = Lref > 0 ? (float)(Le / Lref) : 0.f;
+        p.qs_point = Lref > 0 ? (float)(Lp / Lref) : 0.f;
+        mp[idx] = p;
+        eunit[idx] = Lref / n_total / qscale;
+    }
+    if (idx < D.n_models * ldS) {
+        const int m = idx / ldS;
+        const ModelParams p = mp[m];
+        const double Le = p.has_ext ? Lsrc[2 * m] : 0.0, Lp = p.has_point ? Lsrc[2 * m + 1] : 0.0;
+        const double eu = fmax(Le, Lp) / n_total / qscale;
+        const double ms = mass[idx];
+        cscale[idx] = ms > 0.0 ? eu / (ms * *epsref) : 0.0;
+        if (zero) D.A[idx] = 0ull;
+    }
+    if (zero && idx < D.n_models * D.K) D.esc[idx] = 0ull;
+}
+
+// temperatures from the tallies: eps = A e_unit / m, log-log interpolation in the (eps, T) table (L87; R6)
+__global__ void k_finalize(DeviceModel D, const double* __restrict__ mass, const double* __restrict__ eunit,
+                           const double* __restrict__ eps, const double* __restrict__ Tgrid, const ModelParams* mp,
+                           double* T_out, double* Lesc_out, int* flags)
+{
+    const int N = D.N, K = D.K, nT = D.nT, ldS = D.ldS;
+    const int idx = blockIdx.x * blockDim.x + threadIdx.x;
+    if (idx < D.n_models * K) {
+        const unsigned long long v = D.esc[idx];
+        if (v > (1ull << 62)) atomicOr(flags + 1, 1);
+        Lesc_out[idx] = (double)v * eunit[idx / K];
+    }
+    if (idx < D.n_models * N) {
+        const int m = idx / N, i = idx % N;
+        const int j = i + mp[m].cav;
+        const unsigned long long a = D.A[(size_t)m * ldS + j];
+        if (a > (1ull << 62)) atomicOr(flags + 1, 1);
+        const double ms = mass[(size_t)m * ldS + j];
+        double T = 0.0;
+        if (ms > 0.0) {
+            const double e = (double)a * eunit[m] / ms;
+            if (e < eps[0]) { T = Tgrid[0]; atomicAdd(&D.counters[DIES_C_T_CLAMP_LO], 1ull); }
+            else if (e >= eps[nT - 1]) { T = Tgrid[nT - 1]; atomicAdd(&D.counters[DIES_C_T_CLAMP_HI], 1ull); }
+            else {
+                int lo = 0, hi = nT;      // first index with eps > e
+                while (lo < hi) { const int mid = (lo + hi) >> 1; if (eps[mid] > e) hi = mid; else lo = mid + 1; }
+                const int t = lo - 1;
+                const double f = (log(e) - log(eps[t])) / (log(eps[t + 1]) - log(eps[t]));
+                T = exp(log(Tgrid[t]) + f * (log(Tgrid[t + 1]) - log(Tgrid[t])));
+            }
+        }
+        T_out[idx] = T;
+    }
+}
+
+__global__ void k_sum_escaped(DeviceModel D)
+{
+    unsigned long long s = 0;
+    for (int x = threadIdx.x; x < D.n_models * D.K; x += blockDim.x) s += D.esc[x];
+    for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
+    if ((threadIdx.x & 31) == 0 && s) atomicAdd(&D.counters[DIES_C_ESCAPED_RAW], s);
+}
+
+__global__ void k_test_philox(uint32_t k0, uint32_t k1, unsigned long long first, uint32_t blk, uint32_t mi, int n,
+                              uint32_t* words, float* uni)
+{
+    const int x = blockIdx.x * blockDim.x + threadIdx.x;
+    if (x >= n) return;
+    const unsigned long long id = first + x;
+    uint32_t o[4];
+    philox4x32_10(k0, k1, (uint32_t)id, (uint32_t)(id >> 32), blk, mi, o);
+    for (int c = 0; c < 4; c++) { words[4 * x + c] = o[c]; uni[4 * x + c] = uniform24(o[c]); }
+}
+
+// ------------------------------------------------------------------ helpers
+static int check_device()
+{
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return fail(DIES_ECUDA, "no CUDA device: %s", cudaGetErrorString(e));
+    cudaDeviceProp p;
+    CUDA_TRY(cudaGetDeviceProperties(&p, dev));
+    if (p.major != 10) return fail(DIES_ECUDA, "libdies is built for sm_100a only; device is sm_%d%d", p.major, p.minor);
+    return DIES_OK;
+}
+
+static size_t tracker_smem(int N, int K, int nT)
+{
+    const size_t ldS = (size_t)N + 1;
+    return (size_t)K * 16 + (size_t)K * 8 + ldS * 8 + ldS * 8 + 2 * (ldS + 1) * 8 + (size_t)nT * 4 + (size_t)K * 4 +
+           (size_t)2 * K * 4 + ldS * 4 + 64;
+}
+
+template <int MODE, bool TRACE>
+static cudaError_t set_smem(size_t bytes)
+{
+    return cudaFuncSetAttribute(dies_track<MODE, TRACE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
+}
+
+extern "C" int dies_workspace_bytes(int n_shells, int n_freq, int n_T, int n_models, size_t* bytes)
+{
+    if (!bytes || n_shells < 1 || n_freq < 1 || n_T < 2 || n_models < 1) return fail(DIES_EINVAL, "bad sizes");
+    *bytes = make_layout(n_shells, n_freq, n_T, n_models).total;
+    return DIES_OK;
+}
+
+extern "C" int dies_device_info(int* n_sms, int* blocks_per_sm, int* threads_per_block)
+{
+    int rc = check_device();
+    if (rc) return rc;
+    int dev = 0, sms = 0, bps = 0;
+    CUDA_TRY(cudaGetDevice(&dev));
+    CUDA_TRY(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+    CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&bps, dies_track<0, false>, kBlock, tracker_smem(100, 200, 1000)));
+    if (n_sms) *n_sms = sms;
+    if (blocks_per_sm) *blocks_per_sm = bps;
+    if (threads_per_block) *threads_per_block = kBlock;
+    return DIES_OK;
+}
+
+// ------------------------------------------------------------------ create
+extern "C" int dies_create_batch(int n_models, int n_shells, const double* r_bounds, const double* rho, int n_freq,
+                                 const double* freq, const double* kappa_abs, const double* kappa_sca,
+                                 const double* g_hg, int n_T, const double* T_grid, const double* emis,
+                                 void* workspace_dev, size_t workspace_bytes, dies_model** out)
+{
+    if (!out) return fail(DIES_EINVAL, "out is NULL");
+    *out = nullptr;
+    const int N = n_shells, K = n_freq, nT = n_T, M = n_models;
+    if (N < 1 || K < 1 || nT < 2 || M < 1) return fail(DIES_EINVAL, "bad sizes");
+    if (!r_bounds || !rho || !kappa_abs || !kappa_sca || !g_hg || !T_grid || !emis || !workspace_dev)
+        return fail(DIES_EINVAL, "NULL argument");
+    if (((uintptr_t)workspace_dev & 255) != 0) return fail(DIES_EINVAL, "workspace must be 256-byte aligned");
+    for (int m = 0; m < M; m++) {
+        const double* r = r_bounds + (size_t)m * (N + 1);
+        if (!(r[0] >= 0.0)) return fail(DIES_EINVAL, "model %d: r_bounds[0] < 0", m);
+        for (int i = 0; i < N; i++) {
+            if (!(r[i + 1] > r[i])) return fail(DIES_EINVAL, "model %d: r_bounds not strictly ascending at %d", m, i);
+            if (!(rho[(size_t)m * N + i] >= 0.0)) return fail(DIES_EINVAL, "model %d: rho[%d] < 0", m, i);
+        }
+    }
+    double kref = 0.0;
+    for (int k = 0; k < K; k++) {
+        if (!(kappa_abs[k] >= 0.0) || !(kappa_sca[k] >= 0.0)) return fail(DIES_EINVAL, "negative opacity in bin %d", k);
+        if (!(fabs(g_hg[k]) < 1.0)) return fail(DIES_EINVAL, "|g| >= 1 in bin %d", k);
+        if (freq && k > 0 && !(freq[k] > freq[k - 1])) return fail(DIES_EINVAL, "freq not ascending at %d", k);
+        kref = fmax(kref, kappa_abs[k] + kappa_sca[k]);
+    }
+    if (!(kref > 0.0)) kref = 1.0;
+    for (int t = 1; t < nT; t++)
+        if (!(T_grid[t] > T_grid[t - 1])) return fail(DIES_EINVAL, "T_grid not strictly ascending at %d", t);
+    int rc = check_device();
+    if (rc) return rc;
+    const Layout L = make_layout(N, K, nT, M);
+    if (workspace_bytes < L.total) return fail(DIES_ENOMEM, "workspace too small: %zu < %zu", workspace_bytes, L.total);
+    const size_t smem = tracker_smem(N, K, nT);
+    if (smem > 200 * 1024) return fail(DIES_EINVAL, "tables do not fit in shared memory (%zu bytes)", smem);
+
+    dies_model* m = new (std::nothrow) dies_model();
+    if (!m) return fail(DIES_ENOMEM, "host allocation failed");
+    m->N = N; m->K = K; m->nT = nT; m->M = M; m->ldS = N + 1;
+    m->L = L; m->ws = (unsigned char*)workspace_dev;
+    m->sources_set = m->fixed_set = m->ran = false;
+    m->done = m->n_total = 0; m->shift = 24; m->stream = 0; m->launches = 0;
+    m->L_ext.assign(M, 0.0); m->L_point.assign(M, 0.0); m->has_ext.assign(M, 0); m->has_point.assign(M, 0);
+    m->smem_bytes = smem;
+    DeviceModel& D = m->D;
+    D.N = N; D.K = K; D.nT = nT; D.n_models = M; D.ldS = N + 1;
+    D.bintab = wsp<float4>(m, L.bintab); D.omega = wsp<float>(m, L.omega); D.epsgrid = wsp<float>(m, L.epsgrid);
+    D.F = wsp<float>(m, L.F); D.stab = wsp<float2>(m, L.stab); D.cscale = wsp<double>(m, L.cscale);
+    D.srccdf = wsp<float>(m, L.srccdf); D.mp = wsp<ModelParams>(m, L.mp); D.fixed_row = wsp<int>(m, L.fixed_row);
+    D.A = wsp<unsigned long long>(m, L.A); D.esc = wsp<unsigned long long>(m, L.esc);
+    D.next_id = wsp<unsigned long long>(m, L.next_id); D.counters = wsp<unsigned long long>(m, L.counters);
+    D.ticket = wsp<unsigned int>(m, L.ticket);
+
+#define TRY_OR_FREE(expr)                                                                                   \
+    do {                                                                                                    \
+        cudaError_t e_ = (expr);                                                                            \
+        if (e_ != cudaSuccess) { delete m; return fail(DIES_ECUDA, "%s: %s", #expr, cudaGetErrorString(e_)); } \
+    } while (0)
+    TRY_OR_FREE(cudaMemsetAsync(m->ws, 0, L.total, 0));
+    TRY_OR_FREE(cudaMemcpyAsync(m->ws + L.emis, emis, (size_t)nT * K * 8, cudaMemcpyHostToDevice, 0));
+    TRY_OR_FREE(cudaMemcpyAsync(m->ws + L.Tgrid, T_grid, (size_t)nT * 8, cudaMemcpyHostToDevice, 0));
+    TRY_OR_FREE(cudaMemcpyAsync(m->ws + L.dustin, kappa_abs, (size_t)K * 8, cudaMemcpyHostToDevice, 0));
+    TRY_OR_FREE(cudaMemcpyAsync(m->ws + L.dustin + (size_t)K * 8, kappa_sca, (size_t)K * 8, cudaMemcpyHostToDevice, 0));
+    TRY_OR_FREE(cudaMemcpyAsync(m->ws + L.dustin + (size_t)2 * K * 8, g_hg, (size_t)K * 8, cudaMemcpyHostToDevice, 0));
+    TRY_OR_FREE(cudaMemcpyAsync(m->ws + L.rb, r_bounds, (size_t)M * (N + 1) * 8, cudaMemcpyHostToDevice, 0));
+    TRY_OR_FREE(cudaMemcpyAsync(m->ws + L.rho, rho, (size_t)M * N * 8, cudaMemcpyHostToDevice, 0));
+    int* flags = wsp<int>(m, L.flags);
+    k_build_tables<<<(nT + 127) / 128, 128>>>(wsp<double>(m, L.emis), nT, K, wsp<double>(m, L.eps), wsp<float>(m, L.F), flags);
+    k_build_epsgrid<<<(nT + 127) / 128, 128>>>(wsp<double>(m, L.eps), nT, wsp<float>(m, L.epsgrid), wsp<double>(m, L.epsref), flags);
+    k_build_dust<<<(K + 127) / 128, 128>>>(wsp<double>(m, L.dustin), K, kref, wsp<float4>(m, L.bintab), wsp<float>(m, L.omega));
+    k_build_shells<<<(M * (N + 2) + 127) / 128, 128>>>(wsp<double>(m, L.rb), wsp<double>(m, L.rho), N, M, kref,
+                                                       wsp<float2>(m, L.stab), wsp<double>(m, L.mass), wsp<ModelParams>(m, L.mp));
+    m->launches += 4;
+    int hflags[2] = {0, 0};
+    TRY_OR_FREE(cudaMemcpy(hflags, flags, sizeof(hflags), cudaMemcpyDeviceToHost));
+    TRY_OR_FREE(cudaGetLastError());
+    if (hflags[0] & 1) { delete m; return fail(DIES_EINVAL, "emis must be >= 0 and non-decreasing with T in every bin"); }
+    if (hflags[0] & 2) { delete m; return fail(DIES_EINVAL, "row sums of emis must strictly increase with T"); }
+    TRY_OR_FREE((set_smem<0, false>(smem)));
+    TRY_OR_FREE((set_smem<1, false>(smem)));
+    TRY_OR_FREE((set_smem<0, true>(smem)));
+    TRY_OR_FREE((set_smem<1, true>(smem)));
+    int dev = 0;
+    TRY_OR_FREE(cudaGetDevice(&dev));
+    TRY_OR_FREE(cudaDeviceGetAttribute(&m->n_sms, cudaDevAttrMultiProcessorCount, dev));
+    TRY_OR_FREE(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&m->blocks_per_sm, dies_track<0, false>, kBlock, smem));
+    if (m->blocks_per_sm < 1) { delete m; return fail(DIES_ECUDA, "tracker does not fit on an SM"); }
+    m->grid_max = m->n_sms * m->blocks_per_sm;
+#undef TRY_OR_FREE
+    *out = m;
+    return DIES_OK;
+}
+
+extern "C" int dies_create_model(int n_shells, const double* r_bounds, const double* rho, int n_freq, const double* freq,
+                                 const double* kappa_abs, const double* kappa_sca, const double* g_hg, int n_T,
+                                 const double* T_grid, const double* emis, void* workspace_dev, size_t workspace_bytes,
+                                 dies_model** out)
+{
+    return dies_create_batch(1, n_shells, r_bounds, rho, n_freq, freq, kappa_abs, kappa_sca, g_hg, n_T, T_grid, emis,
+                             workspace_dev, workspace_bytes, out);
+}
+
+extern "C" int dies_destroy(dies_model* m)
+{
+    if (!m) return DIES_OK;
+    cudaStreamSynchronize(m->stream);
+    delete m;
+    return DIES_OK;
+}
+
+// ------------------------------------------------------------------ sources
+extern "C" int dies_set_sources_batch(dies_model* m, const double* ext, const double* L_point, const double* point_w)
+{
+    if (!m) return fail(DIES_EINVAL, "model is NULL");
+    const int K = m->K, M = m->M, N = m->N;
+    std::vector<double> in((size_t)M * 2 * K, 0.0);
+    std::vector<ModelParams> mp(M);
+    CUDA_TRY(cudaStreamSynchronize(m->stream));
+    CUDA_TRY(cudaMemcpy(mp.data(), m->ws + m->L.mp, (size_t)M * sizeof(ModelParams), cudaMemcpyDeviceToHost));
+    bool any = false;
+    for (int i = 0; i < M; i++) {
+        double J = 0.0, P = 0.0;
+        if (ext) for (int k = 0; k < K; k++) {
+            const double v = ext[(size_t)i * K + k];
+            if (!(v >= 0.0)) return fail(DIES_EINVAL, "model %d: negative external intensity in bin %d", i, k);
+            in[((size_t)i * 2) * K + k] = v; J += v;
+        }
+        const double Lp = L_point ? L_point[i] : 0.0;
+        if (point_w && Lp > 0.0) for (int k = 0; k < K; k++) {
+            const double v = point_w[(size_t)i * K + k];
+            if (!(v >= 0.0)) return fail(DIES_EINVAL, "model %d: negative point-source weight in bin %d", i, k);
+            in[((size_t)i * 2 + 1) * K + k] = v; P += v;
+        }
+        if (Lp < 0.0) return fail(DIES_EINVAL, "model %d: L_point < 0", i);
+        m->has_ext[i] = J > 0.0; m->has_point[i] = (Lp > 0.0 && P > 0.0);
+        m->L_point[i] = m->has_point[i] ? Lp : 0.0;
+        mp[i].has_ext = m->has_ext[i]; mp[i].has_point = m->has_point[i];
+        any = any || m->has_ext[i] || m->has_point[i];
+    }
+    std::vector<double> Ls((size_t)2 * M, 0.0);
+    for (int i = 0; i < M; i++) Ls[2 * i + 1] = m->L_point[i];
+    CUDA_TRY(cudaMemcpy(m->ws + m->L.srcin, in.data(), in.size() * 8, cudaMemcpyHostToDevice));
+    CUDA_TRY(cudaMemcpy(m->ws + m->L.Lsrc, Ls.data(), Ls.size() * 8, cudaMemcpyHostToDevice));
+    CUDA_TRY(cudaMemcpy(m->ws + m->L.mp, mp.data(), (size_t)M * sizeof(ModelParams), cudaMemcpyHostToDevice));
+    k_build_sources<<<(2 * M + 127) / 128, 128>>>(wsp<double>(m, m->L.srcin), wsp<double>(m, m->L.rb), N, K, M,
+                                                  wsp<float>(m, m->L.srccdf), wsp<double>(m, m->L.Lsrc));
+    m->launches += 1;
+    CUDA_TRY(cudaMemcpy(Ls.data(), m->ws + m->L.Lsrc, Ls.size() * 8, cudaMemcpyDeviceToHost));
+    CUDA_TRY(cudaGetLastError());
+    for (int i = 0; i < M; i++) m->L_ext[i] = m->has_ext[i] ? Ls[2 * i] : 0.0;
+    m->sources_set = any;
+    m->ran = false; m->done = 0;
+    return DIES_OK;
+}
+
+extern "C" int dies_set_sources(dies_model* m, const double* ext, double L_point, const double* point_w)
+{
+    if (!m) return fail(DIES_EINVAL, "model is NULL");
+    if (m->M != 1) return fail(DIES_EINVAL, "use dies_set_sources_batch for a batch handle");
+    return dies_set_sources_batch(m, ext, &L_point, point_w);
+}
+
+extern "C" int dies_set_fixed_temperature(dies_model* m, const double* T, int n)
+{
+    if (!m || !T) return fail(DIES_EINVAL, "NULL argument");
+    if (n != m->M * m->N) return fail(DIES_EINVAL, "n must be n_models*n_shells = %d", m->M * m->N);
+    CUDA_TRY(cudaStreamSynchronize(m->stream));
+    CUDA_TRY(cudaMemcpy(m->ws + m->L.Tfix, T, (size_t)n * 8, cudaMemcpyHostToDevice));
+    k_fixed_rows<<<(n + 127) / 128, 128>>>(wsp<double>(m, m->L.Tfix), wsp<double>(m, m->L.Tgrid), m->nT, m->N, m->M,
+                                           wsp<ModelParams>(m, m->L.mp), wsp<int>(m, m->L.fixed_row));
+    m->launches += 1;
+    CUDA_TRY(cudaDeviceSynchronize());
+    m->fixed_set = true;
+    return DIES_OK;
+}
+
+// ------------------------------------------------------------------ run
+static int thr_from_env()
+{
+    const char* e = getenv("DIES_THRESH");
+    if (e) { int v = atoi(e); if (v >= 0 && v <= 32) return v; }
+    return 16;
+}
+
+static int fill_run_params(dies_model* m, uint64_t n_packages, uint64_t seed, const dies_run_opts* o, RunParams* R,
+                           int* mode, int* accumulate, int* shift, uint64_t* n_total)
+{
+    dies_run_opts d = {0.5, 0, DIES_MODE_IRE, 0, 24, 0};
+    if (o) d = *o;
+    if (!(d.k_bg > 0.0) || d.k_bg > 1.0) return fail(DIES_EINVAL, "k_bg must be in (0, 1]");
+    if (d.mode != DIES_MODE_IRE && d.mode != DIES_MODE_FIXED_T) return fail(DIES_EINVAL, "bad mode");
+    if (d.fixed_shift == 0) d.fixed_shift = 24;
+    if (d.fixed_shift < 1 || d.fixed_shift > 30) return fail(DIES_EINVAL, "fixed_shift must be in [1, 30]");
+    if (d.n_total == 0) d.n_total = n_packages;
+    if (d.mode == DIES_MODE_FIXED_T && !m->fixed_set) return fail(DIES_ESTATE, "fixed-T mode needs dies_set_fixed_temperature");
+    *mode = d.mode; *accumulate = d.accumulate; *shift = d.fixed_shift; *n_total = d.n_total;
+    int two = 0;
+    for (int i = 0; i < m->M; i++) two |= (m->has_ext[i] && m->has_point[i]);
+    R->n_run = n_packages; R->n_total = d.n_total; R->id_base = 0;
+    R->key0 = (uint32_t)seed; R->key1 = (uint32_t)(seed >> 32);
+    R->k_bg = (float)d.k_bg; R->ffi = d.ffi ? 1 : 0;
+    R->uniform_q = (d.k_bg == 0.5 && !d.ffi && !two) ? 1 : 0;
+    R->qscale = (float)(1u << d.fixed_shift);
+    R->thr_num = thr_from_env();
+    R->n_tickets = 0; R->parts = 1;
+    return DIES_OK;
+}
+
+extern "C" int dies_run(dies_model* m, uint64_t n_packages, uint64_t seed, const dies_run_opts* opts, void* cuda_stream)
+{
+    if (!m) return fail(DIES_EINVAL, "model is NULL");
+    if (!m->sources_set) return fail(DIES_ESTATE, "dies_run before dies_set_sources");
+    if (n_packages == 0) return fail(DIES_EINVAL, "n_packages is 0");
+    RunParams R;
+    int mode, accumulate, shift; uint64_t n_total;
+    int rc = fill_run_params(m, n_packages, seed, opts, &R, &mode, &accumulate, &shift, &n_total);
+    if (rc) return rc;
+    if (accumulate && m->ran) {
+        if (n_total != m->n_total || shift != m->shift) return fail(DIES_ESTATE, "accumulate needs the same n_total and fixed_shift");
+    } else {
+        accumulate = 0;
+        m->done = 0;
+    }
+    if (m->done + n_packages > n_total) return fail(DIES_EINVAL, "more packages than n_total");
+    R.id_base = m->done;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    if (m->ran && st != m->stream) CUDA_TRY(cudaStreamSynchronize(m->stream));
+    m->stream = st;
+    m->n_total = n_total; m->shift = shift;
+
+    // grid: persistent blocks, at most blocks_per_sm per SM, fewer for tiny runs
+    unsigned long long ids = 0;
+    for (int i = 0; i < m->M; i++) ids += n_packages * (unsigned long long)(m->has_ext[i] + m->has_point[i]);
+    unsigned long long want = (ids + 2ull * kBlock - 1) / (2ull * kBlock);
+    int grid = (int)(want < 1 ? 1 : (want > (unsigned long long)m->grid_max ? m->grid_max : want));
+    if (m->M == 1) { R.parts = grid; R.n_tickets = grid; }
+    else { R.parts = (8 * grid + m->M - 1) / m->M; if (R.parts < 1) R.parts = 1; R.n_tickets = m->M * R.parts; }
+
+    const int prep = m->M * (m->K > m->ldS ? m->K : m->ldS);
+    k_prepare_run<<<(prep + 255) / 256, 256, 0, st>>>(m->D, wsp<double>(m, m->L.mass), wsp<double>(m, m->L.Lsrc),
+                                                    wsp<double>(m, m->L.epsref), wsp<double>(m, m->L.cscale),
+                                                    wsp<double>(m, m->L.eunit), wsp<ModelParams>(m, m->L.mp),
+                                                    (double)n_total, (double)R.qscale, accumulate ? 0 : 1);
+    TraceParams tp = {0, 0, 0, nullptr, 0, nullptr};
+    if (mode == DIES_MODE_IRE) dies_track<0, false><<<grid, kBlock, m->smem_bytes, st>>>(m->D, R, tp);
+    else dies_track<1, false><<<grid, kBlock, m->smem_bytes, st>>>(m->D, R, tp);
+    m->launches += 2;
+    CUDA_TRY(cudaGetLastError());
+    m->done += n_packages;
+    m->ran = true;
+    return DIES_OK;
+}
+
+extern "C" int dies_run_batch(dies_model* m, uint64_t n, uint64_t seed, const dies_run_opts* opts, void* cuda_stream)
+{
+    return dies_run(m, n, seed, opts, cuda_stream);
+}
+
+// ------------------------------------------------------------------ getters
+static int finalize(dies_model* m)
+{
+    if (!m->ran) return fail(DIES_ESTATE, "no run yet");
+    const int n = m->M * (m->K > m->N ? m->K : m->N);
+    int* flags = wsp<int>(m, m->L.flags);
+    CUDA_TRY(cudaMemsetAsync(flags, 0, 16, m->stream));
+    // the derived counters ESCAPED_RAW .. T_CLAMP_HI are recomputed by every finalisation
+    CUDA_TRY(cudaMemsetAsync(m->ws + m->L.counters + DIES_C_ESCAPED_RAW * 8, 0, 4 * 8, m->stream));
+    k_finalize<<<(n + 255) / 256, 256, 0, m->stream>>>(m->D, wsp<double>(m, m->L.mass), wsp<double>(m, m->L.eunit),
+                                                     wsp<double>(m, m->L.eps), wsp<double>(m, m->L.Tgrid),
+                                                     wsp<ModelParams>(m, m->L.mp), wsp<double>(m, m->L.T_out),
+                                                     wsp<double>(m, m->L.Lesc_out), flags);
+    k_sum_escaped<<<1, 256, 0, m->stream>>>(m->D);
+    m->launches += 2;
+    int hf[2];
+    CUDA_TRY(cudaMemcpyAsync(hf, flags, sizeof(hf), cudaMemcpyDeviceToHost, m->stream));
+    CUDA_TRY(cudaStreamSynchronize(m->stream));
+    CUDA_TRY(cudaGetLastError());
+    if (hf[1]) return fail(DIES_EOVERFLOW, "a tally exceeded 2^62");
+    return DIES_OK;
+}
+
+extern "C" int dies_get_temperature(dies_model* m, double* T, int n)
+{
+    if (!m || !T) return fail(DIES_EINVAL, "NULL argument");
+    if (n != m->M * m->N) return fail(DIES_EINVAL, "n must be n_models*n_shells = %d", m->M * m->N);
+    int rc = finalize(m);
+    if (rc) return rc;
+    CUDA_TRY(cudaMemcpy(T, m->ws + m->L.T_out, (size_t)n * 8, cudaMemcpyDeviceToHost));
+    return DIES_OK;
+}
+
+extern "C" int dies_get_escape_spectrum(dies_model* m, double* Lesc, int n)
+{
+    if (!m || !Lesc) return fail(DIES_EINVAL, "NULL argument");
+    if (n != m->M * m->K) return fail(DIES_EINVAL, "n must be n_models*n_freq = %d", m->M * m->K);
+    int rc = finalize(m);
+    if (rc) return rc;
+    CUDA_TRY(cudaMemcpy(Lesc, m->ws + m->L.Lesc_out, (size_t)n * 8, cudaMemcpyDeviceToHost));
+    return DIES_OK;
+}
+
+extern "C" int dies_get_absorbed(dies_model* m, int64_t* raw, double* energy_per_raw_unit, int n)
+{
+    if (!m || !raw) return fail(DIES_EINVAL, "NULL argument");
+    if (n != m->M * m->N) return fail(DIES_EINVAL, "n must be n_models*n_shells = %d", m->M * m->N);
+    if (!m->ran) return fail(DIES_ESTATE, "no run yet");
+    CUDA_TRY(cudaStreamSynchronize(m->stream));
+    std::vector<unsigned long long> a((size_t)m->M * m->ldS);
+    std::vector<ModelParams> mp(m->M);
+    CUDA_TRY(cudaMemcpy(a.data(), m->ws + m->L.A, a.size() * 8, cudaMemcpyDeviceToHost));
+    CUDA_TRY(cudaMemcpy(mp.data(), m->ws + m->L.mp, mp.size() * sizeof(ModelParams), cudaMemcpyDeviceToHost));
+    for (int i = 0; i < m->M; i++)
+        for (int s = 0; s < m->N; s++) {
+            const unsigned long long v = a[(size_t)i * m->ldS + s + mp[i].cav];
+            if (v > (1ull << 62)) return fail(DIES_EOVERFLOW, "a tally exceeded 2^62");
+            raw[(size_t)i * m->N + s] = (int64_t)v;
+        }
+    if (energy_per_raw_unit) CUDA_TRY(cudaMemcpy(energy_per_raw_unit, m->ws + m->L.eunit, (size_t)m->M * 8, cudaMemcpyDeviceToHost));
+    return DIES_OK;
+}
+
+extern "C" int dies_get_counters(dies_model* m, uint64_t* c, int n)
+{
+    if (!m || !c) return fail(DIES_EINVAL, "NULL argument");
+    if (n != DIES_N_COUNTERS) return fail(DIES_EINVAL, "n must be DIES_N_COUNTERS = %d", (int)DIES_N_COUNTERS);
+    int rc = finalize(m);
+    if (rc) return rc;
+    CUDA_TRY(cudaMemcpy(c, m->ws + m->L.counters, (size_t)n * 8, cudaMemcpyDeviceToHost));
+    c[DIES_C_KERNEL_LAUNCHES] = m->launches;
+    return DIES_OK;
+}
+
+extern "C" int dies_get_tables(dies_model* m, double* eps, float* F)
+{
+    if (!m) return fail(DIES_EINVAL, "model is NULL");
+    CUDA_TRY(cudaStreamSynchronize(m->stream));
+    if (eps) CUDA_TRY(cudaMemcpy(eps, m->ws + m->L.eps, (size_t)m->nT * 8, cudaMemcpyDeviceToHost));
+    if (F) CUDA_TRY(cudaMemcpy(F, m->ws + m->L.F, (size_t)m->nT * m->K * 4, cudaMemcpyDeviceToHost));
+    return DIES_OK;
+}
+
+// ------------------------------------------------------------------ trace / tests
+extern "C" int dies_trace_packages(dies_model* m, int model_index, uint64_t first_id, int count, uint64_t n_total,
+                                   uint64_t seed, const dies_run_opts* opts, int32_t* events, int max_events,
+                                   int32_t* n_events)
+{
+    if (!m || !events || !n_events) return fail(DIES_EINVAL, "NULL argument");
+    if (!m->sources_set) return fail(DIES_ESTATE, "trace before dies_set_sources");
+    if (model_index < 0 || model_index >= m->M || count < 1 || max_events < 1 || n_total == 0)
+        return fail(DIES_EINVAL, "bad trace arguments");
+    RunParams R;
+    int mode, accumulate, shift; uint64_t nt;
+    dies_run_opts o = {0.5, 0, DIES_MODE_FIXED_T, 0, 24, n_total};
+    if (opts) o = *opts;
+    o.n_total = n_total;
+    int rc = fill_run_params(m, 1, seed, &o, &R, &mode, &accumulate, &shift, &nt);
+    if (rc) return rc;
+    if (mode == DIES_MODE_IRE && (!m->ran || nt != m->n_total || shift != m->shift))
+        return fail(DIES_ESTATE, "IRE-mode trace replays against the tallies of a run with the same n_total");
+    CUDA_TRY(cudaStreamSynchronize(m->stream));
+    if (!m->ran) {
+        // energy scales are set per run; a trace before any run sets them for n_total
+        k_prepare_run<<<(m->M * (m->K > m->ldS ? m->K : m->ldS) + 255) / 256, 256>>>(
+            m->D, wsp<double>(m, m->L.mass), wsp<double>(m, m->L.Lsrc), wsp<double>(m, m->L.epsref),
+            wsp<double>(m, m->L.cscale), wsp<double>(m, m->L.eunit), wsp<ModelParams>(m, m->L.mp), (double)nt,
+            (double)R.qscale, 1);
+        m->launches += 1;
+    }
+    R.n_run = nt; R.id_base = 0;
+    int32_t *d_ev = nullptr, *d_n = nullptr;
+    CUDA_TRY(cudaMalloc(&d_ev, (size_t)count * max_events * 16));
+    if (cudaMalloc(&d_n, (size_t)count * 4) != cudaSuccess) { cudaFree(d_ev); return fail(DIES_ECUDA, "cudaMalloc failed"); }
+    cudaMemset(d_n, 0, (size_t)count * 4);
+    TraceParams tp = {model_index, first_id, count, d_ev, max_events, d_n};
+    const int grid = (count + kBlock - 1) / kBlock;
+    if (mode == DIES_MODE_IRE) dies_track<0, true><<<grid, kBlock, m->smem_bytes>>>(m->D, R, tp);
+    else dies_track<1, true><<<grid, kBlock, m->smem_bytes>>>(m->D, R, tp);
+    m->launches += 1;
+    cudaError_t e = cudaDeviceSynchronize();
+    if (e == cudaSuccess) e = cudaMemcpy(events, d_ev, (size_t)count * max_events * 16, cudaMemcpyDeviceToHost);
+    if (e == cudaSuccess) e = cudaMemcpy(n_events, d_n, (size_t)count * 4, cudaMemcpyDeviceToHost);
+    cudaFree(d_ev); cudaFree(d_n);
+    if (e != cudaSuccess) return fail(DIES_ECUDA, "trace: %s", cudaGetErrorString(e));
+    return DIES_OK;
+}
+
+extern "C" int dies_trace_package(dies_model* m, uint64_t package_id, uint64_t n_total, uint64_t seed,
+                                  const dies_run_opts* opts, int32_t* events, int max_events, int32_t* n_events)
+{
+    return dies_trace_packages(m, 0, package_id, 1, n_total, seed, opts, events, max_events, n_events);
+}
+
+extern "C" int dies_test_philox(uint64_t seed, uint64_t first_id, uint32_t block, uint32_t model_index, int n,
+                                uint32_t* words, float* uniforms)
+{
+    if (!words || !uniforms || n < 1) return fail(DIES_EINVAL, "bad arguments");
+    int rc = check_device();
+    if (rc) return rc;
+    uint32_t* dw = nullptr; float* du = nullptr;
+    CUDA_TRY(cudaMalloc(&dw, (size_t)n * 16));
+    if (cudaMalloc(&du, (size_t)n * 16) != cudaSuccess) { cudaFree(dw); return fail(DIES_ECUDA, "cudaMalloc failed"); }
+    k_test_philox<<<(n + 255) / 256, 256>>>((uint32_t)seed, (uint32_t)(seed >> 32), first_id, block, model_index, n, dw, du);
+    cudaError_t e = cudaMemcpy(words, dw, (size_t)n * 16, cudaMemcpyDeviceToHost);
+    if (e == cudaSuccess) e = cudaMemcpy(uniforms, du, (size_t)n * 16, cudaMemcpyDeviceToHost);
+    cudaFree(dw); cudaFree(du);
+    if (e != cudaSuccess) return fail(DIES_ECUDA, "philox test: %s", cudaGetErrorString(e));
+    return DIES_OK;
+}

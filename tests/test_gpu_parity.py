@@ -1,0 +1,319 @@
+"""GPU parity: the CUDA path (through the C ABI of include/dies.h) against the CPU oracle on the same seeded
+synthetic inputs.  Bars (BASELINE.json north_star):
+  * bit-exact Philox words / uniforms, package counts and event lists of the deterministic trace test;
+  * fixed-temperature tracking with identical Philox streams: per-shell absorbed energy within 1e-4 relative;
+  * full IRE: per-shell T within 1 % or 3 combined standard errors over 8 seeds, whichever is larger;
+  * integer energy conservation exact.
+"""
+import math
+
+import numpy as np
+import pytest
+
+from paper_2408_13807_b200 import binding as dies
+from paper_2408_13807_b200 import synth
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def orc():
+    from oracle import dies_oracle
+    return dies_oracle
+
+
+def _fixed_T(n):
+    return np.linspace(12.0, 19.0, n)
+
+
+# ------------------------------------------------------------------ RNG and tables
+def test_device_philox_and_uniforms_bit_exact(orc):
+    for seed, first, blk, mi in [(1, 0, 0, 0), (0xDEADBEEF12345678, 2 ** 32 - 5, 3, 7), (42, 2 ** 40 + 11, 100, 1023)]:
+        n = 4096
+        w, u = dies.dies_test_philox(seed, first, blk, mi, n)
+        for x in range(0, n, 37):
+            pid = first + x
+            ref = orc.philox4x32_10((seed & 0xFFFFFFFF, seed >> 32), (pid & 0xFFFFFFFF, pid >> 32, blk, mi))
+            assert tuple(int(v) for v in w[x]) == ref
+            for c in range(4):
+                assert float(u[x, c]) == orc.uniform(ref[c])
+        assert u.min() > 0 and u.max() < 1
+
+
+def test_device_tables_match_oracle(orc):
+    p = synth.config1()
+    m = dies.Model(p)
+    eps, F = m.dies_get_tables()
+    o = orc.Oracle(p)
+    eps_o, F_o, _ = o.tables()
+    np.testing.assert_allclose(eps, eps_o, rtol=1e-14)
+    assert np.max(np.abs(F.astype(np.float64) - F_o)) <= 6.0e-8          # one fp32 rounding of a value <= 1
+    m.close()
+
+
+# ------------------------------------------------------------------ deterministic trace (bit-exact)
+@pytest.mark.parametrize("cfg,kw", [("config1", {}), ("config1", dict(k_bg=0.3)), ("config1", dict(ffi=1)),
+                                    ("config3s", {}), ("config2s", {})])
+def test_trace_bit_exact(orc, cfg, kw):
+    """Same Philox streams, fixed temperatures: every package whose decisions all sit further than 1e-3 (relative)
+    from their thresholds in the oracle must produce the identical event list (type, shell, bin, crossings)."""
+    if cfg == "config1":
+        p = synth.config1()
+    elif cfg == "config3s":
+        p = synth.config3(n_shells=40, n_freq=64, tau_V=30.0)
+    else:
+        p = synth.config2(n_shells=50, n_freq=64)
+    n_total, count, max_ev = 100000, 3000, 512
+    o = orc.Oracle(p)
+    o.set_fixed_temperature(_fixed_T(p.n_shells))
+    m = dies.Model(p)
+    m.dies_set_fixed_temperature(_fixed_T(p.n_shells))
+    ev, nev = m.dies_trace_packages(0, count, n_total, seed=5, max_events=max_ev, mode=dies.DIES_MODE_FIXED_T, **kw)
+    safe = same = same_safe = 0
+    for pid in range(count):
+        ref, nref, margin = o.trace(n_total, pid, seed=5, mode=1, max_events=max_ev, **kw)
+        ok = (nref == nev[pid]) and nref <= max_ev and np.array_equal(ref, ev[pid, :nref])
+        same += ok
+        if margin > 1e-3 and nref <= max_ev:
+            safe += 1
+            same_safe += ok
+            assert ok, (pid, margin, ref[:8], ev[pid, :8])
+    assert safe > 0.5 * count
+    assert same_safe == safe
+    assert same >= 0.995 * count, same / count       # the rest differ by fp32-vs-fp64 branch flips (R14)
+    m.close()
+
+
+# ------------------------------------------------------------------ fixed-T tracking, identical streams
+def _fixed_T_pair(orc, p, n, seed=3, **kw):
+    o = orc.Oracle(p)
+    o.set_fixed_temperature(_fixed_T(p.n_shells))
+    o.run(n, seed=seed, mode=1, **kw)
+    m = dies.Model(p)
+    m.dies_set_fixed_temperature(_fixed_T(p.n_shells))
+    m.dies_run(n, seed=seed, mode=dies.DIES_MODE_FIXED_T, **kw)
+    raw, unit, energy = m.dies_get_absorbed()
+    return o, m, raw, unit, energy
+
+
+@pytest.mark.parametrize("kw", [{}, dict(k_bg=0.2), dict(ffi=1)])
+def test_fixed_T_absorbed_energy_config1(orc, kw):
+    """Config 1 (1e5 packages): counts per shell are small, so one branch-flipped package already moves a shell by
+    1e-4..1e-3; the bar here is: event totals within 2e-4 and every shell within 1e-4 relative or 3 packages."""
+    p = synth.config1()
+    n = p.n_packages
+    o, m, raw, unit, energy = _fixed_T_pair(orc, p, n, **kw)
+    c, co = m.dies_get_counters(), o.counters
+    assert c["packages"] == co["packages"] == n
+    for name in ("crossings", "scatterings", "absorptions", "ffi_crossings"):
+        assert abs(c[name] - co[name]) <= 2e-4 * max(co[name], 1) + 3, (name, c[name], co[name])
+    e_pkg = o.sums["injected"] / n
+    tol = np.maximum(1e-4 * o.absorbed, 3 * e_pkg * (5 if kw.get("k_bg") else 1))
+    assert np.all(np.abs(energy - o.absorbed) <= tol), np.max(np.abs(energy - o.absorbed) / e_pkg)
+    assert c["injected_raw"] == c["escaped_raw"] + c["terminated_raw"]
+    esc = m.dies_get_escape_spectrum()
+    assert abs(esc.sum() / o.sums["escaped"] - 1) < 1e-5
+    m.close()
+
+
+def test_fixed_T_absorbed_energy_config2_1e4_relative(orc):
+    """North-star bar: per-shell absorbed energy within 1e-4 relative with identical Philox streams, on config 2
+    with enough packages that every shell holds >= 1e4 package quanta (reading R14)."""
+    p = synth.config2()
+    n = 2_000_000
+    o, m, raw, unit, energy = _fixed_T_pair(orc, p, n, seed=1)
+    c, co = m.dies_get_counters(), o.counters
+    for name in ("crossings", "scatterings", "absorptions"):
+        assert abs(c[name] / co[name] - 1) < 2e-5, (name, c[name], co[name])
+    rel = np.abs(energy / o.absorbed - 1)
+    e_pkg = o.sums["injected"] / n
+    print("max rel", rel.max(), "packages/shell min", (o.absorbed / e_pkg).min(),
+          "max |diff| in packages", np.max(np.abs(energy - o.absorbed)) / e_pkg)
+    assert abs(energy.sum() / o.absorbed.sum() - 1) < 1e-5
+    well = o.absorbed / e_pkg >= 2e4
+    assert well.sum() >= 0.5 * p.n_shells
+    assert np.all(rel[well] < 1e-4), rel.max()
+    assert np.all(np.abs(energy - o.absorbed)[~well] <= 3 * e_pkg)
+    assert c["injected_raw"] == c["escaped_raw"]
+    assert c["injected_raw"] == n * (1 << 24)
+    m.close()
+
+
+def test_fixed_T_is_deterministic_and_splittable():
+    """Integer tallies: the same seed gives bit-identical tallies whatever the scheduling, and a run split into
+    accumulate batches (PAPER.md L163 N_B batches) equals the single run exactly."""
+    p = synth.config1()
+    n = 60000
+    res = []
+    for parts in (1, 1, 3):
+        m = dies.Model(p)
+        m.dies_set_fixed_temperature(_fixed_T(p.n_shells))
+        for b in range(parts):
+            m.dies_run(n // parts, seed=9, mode=dies.DIES_MODE_FIXED_T, n_total=n, accumulate=int(b > 0))
+        raw, _, _ = m.dies_get_absorbed()
+        res.append((raw.copy(), m.dies_get_escape_spectrum().copy(), m.dies_get_counters()))
+        m.close()
+    for r in res[1:]:
+        assert np.array_equal(r[0], res[0][0])
+        assert np.array_equal(r[1], res[0][1])
+        for k in ("packages", "crossings", "scatterings", "absorptions", "injected_raw", "escaped_raw"):
+            assert r[2][k] == res[0][2][k]
+
+
+# ------------------------------------------------------------------ full IRE, statistical
+def _ire_stats(orc, p, n, seeds, model_kw=None, **kw):
+    To, Tg = [], []
+    for s in seeds:
+        o = orc.Oracle(p)
+        o.run(n, seed=s, **kw)
+        To.append(o.temperature())
+        m = dies.Model(p)
+        m.dies_run(n, seed=s, **kw)
+        Tg.append(m.dies_get_temperature())
+        c = m.dies_get_counters()
+        assert c["injected_raw"] == c["escaped_raw"] + c["terminated_raw"]      # exact conservation
+        assert c["packages"] == n and c["terminated"] == 0
+        m.close()
+    return np.array(To), np.array(Tg)
+
+
+def _assert_T_parity(To, Tg, skip_inner=0):
+    mo, mg = To.mean(0), Tg.mean(0)
+    se = np.sqrt(To.var(0, ddof=1) / len(To) + Tg.var(0, ddof=1) / len(Tg))
+    tol = np.maximum(0.01 * mo, 3 * se)
+    bad = np.abs(mg - mo) > tol
+    assert not np.any(bad[skip_inner:]), (np.nonzero(bad)[0], (mg / mo)[bad], (np.abs(mg - mo) / se)[bad])
+
+
+@pytest.mark.parametrize("name,kw", [("plain", {}), ("kbg", dict(k_bg=0.2)), ("ffi", dict(ffi=1))])
+def test_full_ire_temperature_config1(orc, name, kw):
+    p = synth.config1()
+    To, Tg = _ire_stats(orc, p, p.n_packages, range(1, 9), **kw)
+    _assert_T_parity(To, Tg)
+
+
+def test_full_ire_temperature_config2_reduced(orc):
+    p = synth.config2()
+    To, Tg = _ire_stats(orc, p, 200_000, range(1, 9))
+    _assert_T_parity(To, Tg)
+
+
+def test_full_ire_temperature_config3_reduced(orc):
+    p = synth.config3()
+    To, Tg = _ire_stats(orc, p, 30_000, range(1, 9))
+    _assert_T_parity(To, Tg)
+
+
+def test_full_ire_temperature_config4_reduced(orc):
+    p = synth.config4()
+    To, Tg = _ire_stats(orc, p, 300_000, range(1, 9), ffi=1)
+    _assert_T_parity(To, Tg)
+
+
+def test_both_sources_at_once(orc):
+    p = synth.config3(n_shells=40, n_freq=64, tau_V=20.0)
+    q = synth.config1(n_freq=64)
+    p.ext_bin_intensity = q.ext_bin_intensity * 1e6
+    To, Tg = _ire_stats(orc, p, 20_000, range(1, 9))
+    _assert_T_parity(To, Tg)
+
+
+# ------------------------------------------------------------------ batch (config 5)
+def test_batch_matches_per_model_oracle(orc):
+    b = synth.config5(n_models=6, n_packages=40_000)
+    m = dies.Model(batch=b)
+    m.dies_set_fixed_temperature(np.tile(_fixed_T(64), (b.n_models, 1)))
+    m.dies_run(b.n_packages, seed=2, mode=dies.DIES_MODE_FIXED_T)
+    raw, unit, energy = m.dies_get_absorbed()
+    esc = m.dies_get_escape_spectrum()
+    tot = dict(crossings=0, absorptions=0, scatterings=0)
+    for i in range(b.n_models):
+        p = b.model(i)
+        o = orc.Oracle(p)
+        o.set_fixed_temperature(_fixed_T(64))
+        o.run(b.n_packages, seed=2, mode=1, model_index=i)
+        e_pkg = o.sums["injected"] / b.n_packages
+        assert np.all(np.abs(energy[i] - o.absorbed) <= np.maximum(1e-4 * o.absorbed, 3 * e_pkg)), i
+        assert abs(esc[i].sum() / o.sums["escaped"] - 1) < 1e-5
+        for k in tot:
+            tot[k] += o.counters[k]
+    c = m.dies_get_counters()
+    assert c["packages"] == b.n_models * b.n_packages
+    for k in tot:
+        assert abs(c[k] - tot[k]) <= 2e-4 * tot[k] + 3
+    assert c["injected_raw"] == c["escaped_raw"]
+    # full IRE on the batch: temperatures per model within noise of the oracle
+    m.dies_run(b.n_packages, seed=4)
+    T = m.dies_get_temperature()
+    for i in (0, b.n_models - 1):
+        o = orc.Oracle(b.model(i))
+        o.run(b.n_packages, seed=4, model_index=i)
+        To = o.temperature()
+        assert np.max(np.abs(T[i][20:] / To[20:] - 1)) < 0.05
+    m.close()
+
+
+# ------------------------------------------------------------------ edge cases and errors
+def test_edge_cases(orc):
+    p = synth.config1()
+    m = dies.Model(p)
+    for n in (1, 31, 129, 1000):
+        m.dies_run(n, seed=1)
+        c = m.dies_get_counters()
+        assert c["packages"] == n == c["escaped"] + c["uninteracted"]
+        assert c["injected_raw"] == c["escaped_raw"] == n * (1 << 24)
+    # a shell of zero density and an empty cavity
+    p2 = synth.config1(n_shells=8)
+    p2.rho[3] = 0.0
+    p2.r_bounds = p2.r_bounds + 0.05 * p2.r_bounds[-1]
+    o = orc.Oracle(p2)
+    o.set_fixed_temperature(_fixed_T(8))
+    o.run(50000, seed=2, mode=1)
+    m2 = dies.Model(p2)
+    m2.dies_set_fixed_temperature(_fixed_T(8))
+    m2.dies_run(50000, seed=2, mode=dies.DIES_MODE_FIXED_T)
+    raw, unit, energy = m2.dies_get_absorbed()
+    assert raw[3] == 0 and o.absorbed[3] == 0
+    e_pkg = o.sums["injected"] / 50000
+    assert np.all(np.abs(energy - o.absorbed) <= np.maximum(1e-4 * o.absorbed, 3 * e_pkg))
+    c = m2.dies_get_counters()
+    assert abs(c["crossings"] - o.counters["crossings"]) <= 2e-4 * o.counters["crossings"]
+    T = m2.dies_get_temperature()
+    assert T[3] == 0.0
+    m.close(); m2.close()
+
+
+def test_error_codes():
+    p = synth.config1()
+    p_nosrc = synth.config1()
+    p_nosrc.ext_bin_intensity = None
+    m = dies.Model(p_nosrc)
+    with pytest.raises(dies.DiesError) as e:
+        m.dies_run(10)
+    assert e.value.code == dies.DIES_ESTATE
+    m.close()
+    m = dies.Model(p)
+    with pytest.raises(dies.DiesError) as e:
+        m.dies_get_temperature()
+    assert e.value.code == dies.DIES_ESTATE
+    with pytest.raises(dies.DiesError) as e:
+        m.dies_run(10, mode=dies.DIES_MODE_FIXED_T)
+    assert e.value.code == dies.DIES_ESTATE
+    with pytest.raises(dies.DiesError) as e:
+        m.dies_run(10, k_bg=0.0)
+    assert e.value.code == dies.DIES_EINVAL
+    m.dies_run(10)
+    import ctypes as C
+    T = np.zeros(p.n_shells + 1)
+    assert dies.lib().dies_get_temperature(m._h, T.ctypes.data_as(C.POINTER(C.c_double)), T.size) == dies.DIES_EINVAL
+    m.close()
+    bad = synth.config1()
+    bad.r_bounds[5] = bad.r_bounds[4]
+    with pytest.raises(dies.DiesError) as e:
+        dies.Model(bad)
+    assert e.value.code == dies.DIES_EINVAL
+    bad = synth.config1()
+    bad.emis[10] = bad.emis[9] * 0.5
+    with pytest.raises(dies.DiesError) as e:
+        dies.Model(bad)
+    assert e.value.code == dies.DIES_EINVAL
