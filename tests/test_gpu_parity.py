@@ -117,23 +117,26 @@ def test_fixed_T_absorbed_energy_config1(orc, kw):
 
 
 def test_fixed_T_absorbed_energy_config2_1e4_relative(orc):
-    """North-star bar: per-shell absorbed energy within 1e-4 relative with identical Philox streams, on config 2
-    with enough packages that every shell holds >= 1e4 package quanta (reading R14)."""
+    """North-star bar at config 2's full size (1e7 packages, the launch configuration bench.py times): per-shell
+    absorbed energy within 1e-4 relative with identical Philox streams wherever a shell holds >= 2e4 package
+    quanta, so that one fp32-vs-fp64 branch-flipped package stays below the bar (reading R14); elsewhere within
+    2 package quanta."""
     p = synth.config2()
-    n = 2_000_000
+    n = p.n_packages
     o, m, raw, unit, energy = _fixed_T_pair(orc, p, n, seed=1)
     c, co = m.dies_get_counters(), o.counters
     for name in ("crossings", "scatterings", "absorptions"):
         assert abs(c[name] / co[name] - 1) < 2e-5, (name, c[name], co[name])
-    rel = np.abs(energy / o.absorbed - 1)
     e_pkg = o.sums["injected"] / n
-    print("max rel", rel.max(), "packages/shell min", (o.absorbed / e_pkg).min(),
-          "max |diff| in packages", np.max(np.abs(energy - o.absorbed)) / e_pkg)
+    cnt = o.absorbed / e_pkg
+    diff = np.abs(energy - o.absorbed)
+    well = cnt >= 2e4
+    print("shells with >= 2e4 quanta:", int(well.sum()), "max rel there:", (diff[well] / o.absorbed[well]).max(),
+          "max |diff| in packages:", diff.max() / e_pkg)
     assert abs(energy.sum() / o.absorbed.sum() - 1) < 1e-5
-    well = o.absorbed / e_pkg >= 2e4
-    assert well.sum() >= 0.5 * p.n_shells
-    assert np.all(rel[well] < 1e-4), rel.max()
-    assert np.all(np.abs(energy - o.absorbed)[~well] <= 3 * e_pkg)
+    assert well.sum() >= 40
+    assert np.all(diff[well] < 1e-4 * o.absorbed[well])
+    assert np.all(diff[~well] <= 2 * e_pkg)
     assert c["injected_raw"] == c["escaped_raw"]
     assert c["injected_raw"] == n * (1 << 24)
     m.close()
