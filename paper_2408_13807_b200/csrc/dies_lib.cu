@@ -144,42 +144,53 @@ __global__ void k_build_dust(const double* __restrict__ dustin, int K, double kr
 }
 
 // shells: lengths in units of the outer radius R, densities as rho^ = rho R kappa_ref; internal shell 0 is the
-// empty cavity when r_bounds[0] > 0 (R10)
+// empty cavity when r_bounds[0] > 0 (R10).  The table is unfolded along a chord (see DeviceModel in
+// dies_tracker.cuh): entry c in [-ldS, ldS+1] = {(r_|c|/R)^2, rho^ of the shell entered, sign bit = inward}.
 __global__ void k_build_shells(const double* __restrict__ rb, const double* __restrict__ rho, int N, int M, double kref,
                                float2* stab, double* mass, ModelParams* mp)
 {
-    const int ldS = N + 1;
+    const int ldS = N + 1, ldT = 2 * ldS + 2;
     const int idx = blockIdx.x * blockDim.x + threadIdx.x;
-    if (idx >= M * (ldS + 1)) return;
-    const int m = idx / (ldS + 1), j = idx % (ldS + 1);
+    if (idx >= M * ldT) return;
+    const int m = idx / ldT, x = idx % ldT;
     const double* r = rb + (size_t)m * (N + 1);
     const double* d = rho + (size_t)m * N;
     const double R = r[N];
     const int cav = r[0] > 0.0 ? 1 : 0;
     const int Np = N + cav;
-    float2* st = stab + (size_t)m * 2 * (ldS + 1);
-    if (j == 0) {
+    if (x == 0) {
         ModelParams p = mp[m];
         p.Np = Np; p.cav = cav; p.r0hat = (float)(r[0] / R);
         mp[m] = p;
     }
-    double r_in = 0.0, r_out = 0.0, dens = 0.0;
-    if (j < Np) {
-        const int i = j - cav;                    // user shell, -1 = cavity
-        r_in = i < 0 ? 0.0 : r[i];
-        r_out = i < 0 ? r[0] : r[i + 1];
-        dens = i < 0 ? 0.0 : d[i];
-        if (i == 0 && cav == 0) r_in = 0.0;
-    } else {
-        r_in = R; r_out = R;                       // dummy entries read when a package escapes
+    // internal boundary b in [0, Np]: radius 0 at the centre, then the user's boundaries
+    auto radius = [&](int b) { return b == 0 ? 0.0 : r[b - cav]; };
+    // internal shell j in [0, Np): the cavity (if any) has no dust
+    auto dens = [&](int j) { const int i = j - cav; return i < 0 ? 0.0 : d[i]; };
+    const int c = x - ldS, a = c < 0 ? -c : c;
+    float2 e = make_float2(4.0f, 0.0f);                                  // beyond the model (entry Np+1 is read)
+    if (c <= 0 && a <= Np) {
+        const double rr = radius(a) / R;
+        const float dh = a >= 1 ? (float)(dens(a - 1) * R * kref) : 0.0f;
+        e = make_float2((float)(rr * rr), __int_as_float(__float_as_int(dh) | 0x80000000));
+    } else if (c > 0 && c < Np) {
+        const double rr = radius(c) / R;
+        e = make_float2((float)(rr * rr), (float)(dens(c) * R * kref));
+    } else if (c == Np) {
+        e = make_float2(1.0f, __int_as_float(0x7f800000));               // outer surface: "rho^ = +inf" stalls the package
+    } else if (c < 0) {
+        e = make_float2(0.0f, __int_as_float(0x80000000));
     }
-    const float x_in = (float)((r_in / R) * (r_in / R)), x_out = (float)((r_out / R) * (r_out / R));
-    const float dh = (float)(dens * R * kref);
-    st[2 * j] = make_float2(x_in, dh);
-    st[2 * j + 1] = make_float2(x_out, dh);
-    if (j < ldS) {
+    stab[(size_t)m * ldT + x] = e;
+    if (x < ldS) {
+        const int j = x;
         const double pi = 3.14159265358979323846;
-        mass[(size_t)m * ldS + j] = j < Np ? dens * (4.0 * pi / 3.0) * (r_out * r_out * r_out - r_in * r_in * r_in) : 0.0;
+        double ms = 0.0;
+        if (j < Np) {
+            const double r_in = radius(j), r_out = radius(j + 1);
+            ms = dens(j) * (4.0 * pi / 3.0) * (r_out * r_out * r_out - r_in * r_in * r_in);
+        }
+        mass[(size_t)m * ldS + j] = ms;
     }
 }
 
@@ -318,9 +329,9 @@ static int check_device()
 
 static size_t tracker_smem(int N, int K, int nT)
 {
-    const size_t ldS = (size_t)N + 1;
-    return (size_t)K * 16 + (size_t)K * 8 + ldS * 8 + ldS * 8 + 2 * (ldS + 1) * 8 + (size_t)nT * 4 + (size_t)K * 4 +
-           (size_t)2 * K * 4 + ldS * 4 + 64;
+    const size_t ldS = (size_t)N + 1, ldT = 2 * ldS + 2;
+    return (size_t)K * 16 + ldS * 8 + ldT * 8 + (size_t)nT * 4 + (size_t)K * 4 + ldS * 4 + (size_t)2 * K * 4 +
+           2 * ldS * 4 + 64;
 }
 
 template <int MODE, bool TRACE>
@@ -397,7 +408,7 @@ extern "C" int dies_create_batch(int n_models, int n_shells, const double* r_bou
     m->L_ext.assign(M, 0.0); m->L_point.assign(M, 0.0); m->has_ext.assign(M, 0); m->has_point.assign(M, 0);
     m->smem_bytes = smem;
     DeviceModel& D = m->D;
-    D.N = N; D.K = K; D.nT = nT; D.n_models = M; D.ldS = N + 1;
+    D.N = N; D.K = K; D.nT = nT; D.n_models = M; D.ldS = N + 1; D.ldT = 2 * (N + 1) + 2;
     D.bintab = wsp<float4>(m, L.bintab); D.omega = wsp<float>(m, L.omega); D.epsgrid = wsp<float>(m, L.epsgrid);
     D.F = wsp<float>(m, L.F); D.stab = wsp<float2>(m, L.stab); D.cscale = wsp<double>(m, L.cscale);
     D.srccdf = wsp<float>(m, L.srccdf); D.mp = wsp<ModelParams>(m, L.mp); D.fixed_row = wsp<int>(m, L.fixed_row);
@@ -422,7 +433,7 @@ extern "C" int dies_create_batch(int n_models, int n_shells, const double* r_bou
     k_build_tables<<<(nT + 127) / 128, 128>>>(wsp<double>(m, L.emis), nT, K, wsp<double>(m, L.eps), wsp<float>(m, L.F), flags);
     k_build_epsgrid<<<(nT + 127) / 128, 128>>>(wsp<double>(m, L.eps), nT, wsp<float>(m, L.epsgrid), wsp<double>(m, L.epsref), flags);
     k_build_dust<<<(K + 127) / 128, 128>>>(wsp<double>(m, L.dustin), K, kref, wsp<float4>(m, L.bintab), wsp<float>(m, L.omega));
-    k_build_shells<<<(M * (N + 2) + 127) / 128, 128>>>(wsp<double>(m, L.rb), wsp<double>(m, L.rho), N, M, kref,
+    k_build_shells<<<(M * (2 * N + 4) + 127) / 128, 128>>>(wsp<double>(m, L.rb), wsp<double>(m, L.rho), N, M, kref,
                                                        wsp<float2>(m, L.stab), wsp<double>(m, L.mass), wsp<ModelParams>(m, L.mp));
     m->launches += 4;
     int hflags[2] = {0, 0};

@@ -1,10 +1,11 @@
 // dies_tracker.cuh -- the persistent-thread IRE package tracker for sm_100a (hot path of include/dies.h).
 //
 // One photon package per lane.  A warp alternates between
-//   (1) an EVENT phase: escapes are tallied, free lanes are refilled from the model's global package
-//       counter, absorptions update the 64-bit fixed-point shell tallies (one returning atomic per
-//       distinct shell in the warp), then every lane that launches / scatters / re-emits draws ONE
-//       Philox4x32-10 block and two new free paths (Eq. 1);
+//   (1) an EVENT phase (all 32 lanes converged): escapes are tallied, free lanes are refilled from the model's
+//       global package counter, absorptions update the 64-bit fixed-point shell tallies (one returning atomic
+//       per distinct shell in the warp), then every lane that launches / scatters / re-emits runs ONE shared
+//       code path: a Philox4x32-10 block, two new free paths (Eq. 1), a table search for the new
+//       frequency (launch and re-emission share it), the new direction, and the set-up of the next flight;
 //   (2) a CROSSING phase: the shell-crossing loop (Eq. 4) with no random numbers and no
 //       global memory, run until fewer than a set fraction of the warp's packages are still flying.
 // Differences from the paper's OpenCL design are listed in DESIGN.md ("What differs from the paper").
@@ -15,10 +16,10 @@
 namespace dies {
 
 constexpr int kBlock = 256;          // threads per block
+constexpr int kMinBlocks = 3;        // resident blocks per SM asked from the compiler
 constexpr unsigned kFull = 0xffffffffu;
 constexpr unsigned kChunk = 128;     // package ids a warp takes from the global counter at a time
-
-enum { ST_NEED = 0, ST_LAUNCH = 1, ST_FLY = 2, ST_SCATTER = 3, ST_ABSORB = 4, ST_ESCAPED = 5 };
+constexpr int kUnroll = 4;           // crossings per vote in the crossing loop
 
 // event counters (same order as DIES_C_* in include/dies.h): the frequent ones are kept warp-uniform in
 // registers (updated from ballots), the rare ones go through shared-memory atomics
@@ -34,14 +35,20 @@ struct ModelParams {
     float pad;
 };
 
+// The shell table of one model is "unfolded" along a chord: entry c in [-ldS, ldS+1] (stored at c + ldS)
+// describes the surface passage a package makes when it reaches boundary |c| moving inward (c <= 0) or outward
+// (c > 0):  .x = (r_|c| / R)^2,  .y = rho^ of the shell entered, with the SIGN BIT SET for inward entries.
+// Entry Np (the outer surface) carries rho^ = +inf and entry Np+1 a radius beyond the model, so a package that
+// leaves the model stalls on entry Np+1 without any test in the loop.  rho^(j) = |entry(-(j+1)).y|.
 struct DeviceModel {
     int N, K, nT, n_models;
     int ldS;                         // leading dimension of the per-model shell arrays (N + 1)
+    int ldT;                         // entries of the unfolded shell table per model (2 ldS + 2)
     const float4* bintab;            // K: {1/kappa_abs^, 1/kappa_sca^, g, kappa_ext^}  (kappa^ = kappa / kappa_ref)
     const float* omega;              // K: albedo
     const float* epsgrid;            // nT: eps_t / eps_ref
     const float* F;                  // nT x K row CDFs of the re-emission spectra
-    const float2* stab;              // n_models x 2(ldS+1): [2j] = {r2_inner(j), rho^(j)}, [2j+1] = {r2_outer(j), rho^(j)}
+    const float2* stab;              // n_models x ldT unfolded shell table
     const double* cscale;            // n_models x ldS: eps^ per raw tally unit
     const float* srccdf;             // n_models x 2 x K: external, point
     const ModelParams* mp;           // n_models
@@ -95,35 +102,40 @@ __device__ __forceinline__ void philox4x32_10(uint32_t k0, uint32_t k1, uint32_t
 
 __device__ __forceinline__ float uniform24(uint32_t x) { return (__uint2float_rn(x >> 9) + 0.5f) * 1.1920928955078125e-07f; }
 
-__device__ __forceinline__ float fast_sqrt(float x)
+__device__ __forceinline__ float sqrt_ftz(float x)
 {
     float y;
-    asm("sqrt.approx.f32 %0, %1;" : "=f"(y) : "f"(x));
+    asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
     return y;
 }
 
-// smallest k in [0, n) with cdf[k] > u   (cdf[n-1] >= 1 > u)
-template <bool GLOBAL>
-__device__ __forceinline__ int sample_cdf(const float* __restrict__ cdf, int n, float u)
+// smallest k in [0, n) with cdf[k] > u (= #{i < n-1 : cdf[i] <= u} for a non-decreasing cdf with cdf[n-1] > u):
+// binary lifting with a warp-uniform trip count (top = largest power of two <= n-1, 0 if n == 1)
+__device__ __forceinline__ int sample_cdf(const float* __restrict__ cdf, int n, int top, float u)
 {
-    int lo = 0, hi = n - 1;
-    while (lo < hi) {
-        const int mid = (lo + hi) >> 1;
-        const float c = GLOBAL ? __ldg(cdf + mid) : cdf[mid];
-        if (c > u) hi = mid; else lo = mid + 1;
+    int k = 0;
+    for (int step = top; step > 0; step >>= 1) {
+        const int t = k + step;
+        if (t < n && __ldg(cdf + t - 1) <= u) k = t;
     }
-    return lo;
+    return k;
 }
 
-// t(eps) = #{j : grid[j] <= eps} clamped to n-1: the table row of a cell emitting eps (R4)
-__device__ __forceinline__ int row_of_eps(const float* grid, int n, float eps)
+// t(eps) = #{j : grid[j] <= eps} clamped to n-1, given a lower bound t0 <= t(eps): the table row of a cell
+// emitting eps (R4).  Rows only move up during a run, so the scan from the block's last known row is short.
+__device__ __forceinline__ int row_from(const float* grid, int n, int t0, float eps)
 {
-    int lo = 0, hi = n;
-    while (lo < hi) {
-        const int mid = (lo + hi) >> 1;
-        if (grid[mid] > eps) hi = mid; else lo = mid + 1;
+    int t = t0;
+    if (grid[min(t + 8, n - 1)] <= eps) {          // far away (first touch of a shell): bisect (t+8, n]
+        int lo = min(t + 8, n - 1) + 1, hi = n;
+        while (lo < hi) {
+            const int mid = (lo + hi) >> 1;
+            if (grid[mid] > eps) hi = mid; else lo = mid + 1;
+        }
+        return min(lo, n - 1);
     }
-    return min(lo, n - 1);
+    while (t < n - 1 && grid[t] <= eps) t++;
+    return t;
 }
 
 // Henyey-Greenstein deflection cosine (Eq. 6), inverse CDF; |g| < 1e-3 is isotropic
@@ -132,6 +144,15 @@ __device__ __forceinline__ float hg_cos(float g, float u)
     if (fabsf(g) < 1e-3f) return 2.f * u - 1.f;
     const float t = (1.f - g * g) / (1.f - g + 2.f * g * u);
     return (1.f + g * g - t * t) / (2.f * g);
+}
+
+// 64-bit shared-memory tally as two 32-bit words (native ATOMS.ADD instead of a 64-bit CAS loop)
+__device__ __forceinline__ void smem_add64(unsigned* lo, unsigned* hi, unsigned long long v)
+{
+    const unsigned vlo = (unsigned)v, vhi = (unsigned)(v >> 32);
+    const unsigned old = atomicAdd(lo, vlo);
+    const unsigned up = vhi + ((old + vlo < old) ? 1u : 0u);
+    if (up) atomicAdd(hi, up);
 }
 
 template <bool TRACE>
@@ -151,25 +172,26 @@ __device__ __forceinline__ void record(const TraceParams& tp, int pkg, int& n_ev
 // MODE 1: fixed temperature (row from fixed_row; tallies privatised in shared memory)
 // TRACE : replay tp.count packages of one model, one per lane, tallies read-only, events recorded
 template <int MODE, bool TRACE>
-__global__ void __launch_bounds__(kBlock, 3) dies_track(DeviceModel D, RunParams R, TraceParams tp)
+__global__ void __launch_bounds__(kBlock, kMinBlocks) dies_track(DeviceModel D, RunParams R, TraceParams tp)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    const int K = D.K, nT = D.nT, ldS = D.ldS;
-    // shared-memory layout (all offsets multiples of 16 bytes)
+    const int K = D.K, nT = D.nT, ldS = D.ldS, ldT = D.ldT;
+    // shared-memory layout
     float4* s_bin = reinterpret_cast<float4*>(smem_raw);                          // K
-    unsigned long long* s_esc = reinterpret_cast<unsigned long long*>(s_bin + K);  // K
-    unsigned long long* s_A = s_esc + K;                                           // ldS
-    double* s_cs = reinterpret_cast<double*>(s_A + ldS);                           // ldS
-    float2* s_stab = reinterpret_cast<float2*>(s_cs + ldS);                        // 2(ldS+1)
-    float* s_eps = reinterpret_cast<float*>(s_stab + 2 * (ldS + 1));               // nT
-    float* s_omega = s_eps + nT;                                                   // K
-    float* s_src = s_omega + K;                                                    // 2K
-    int* s_frow = reinterpret_cast<int*>(s_src + 2 * K);                           // ldS
+    double* s_cs = reinterpret_cast<double*>(s_bin + K);                          // ldS
+    float2* s_tab = reinterpret_cast<float2*>(s_cs + ldS);                        // ldT unfolded shell table
+    float* s_eps = reinterpret_cast<float*>(s_tab + ldT);                         // nT
+    float* s_omega = s_eps + nT;                                                  // K
+    int* s_row = reinterpret_cast<int*>(s_omega + K);                             // ldS: fixed rows / row hints
+    unsigned* s_esc = reinterpret_cast<unsigned*>(s_row + ldS);                   // 2K: low words, high words
+    unsigned* s_A = s_esc + 2 * K;                                                // 2 ldS (MODE 1)
     __shared__ unsigned int s_ticket;
     __shared__ unsigned long long s_cnt[LC_N];      // rare counters, flushed at kernel end
 
     const int tid = threadIdx.x, lane = tid & 31;
     const unsigned lt_mask = (1u << lane) - 1u;
+    int top = 0;                                     // largest power of two <= K-1 (trip count of sample_cdf)
+    for (int t = 1; t <= K - 1; t <<= 1) top = t;
 
     for (int x = tid; x < K; x += kBlock) { s_bin[x] = D.bintab[x]; s_omega[x] = D.omega[x]; }
     for (int x = tid; x < nT; x += kBlock) s_eps[x] = D.epsgrid[x];
@@ -193,61 +215,63 @@ __global__ void __launch_bounds__(kBlock, 3) dies_track(DeviceModel D, RunParams
         }
         const ModelParams mp = D.mp[m];
         const int Np = mp.Np;
-        for (int x = tid; x < 2 * (ldS + 1); x += kBlock) s_stab[x] = D.stab[(size_t)m * 2 * (ldS + 1) + x];
+        for (int x = tid; x < ldT; x += kBlock) s_tab[x] = D.stab[(size_t)m * ldT + x];
         for (int x = tid; x < ldS; x += kBlock) {
             s_cs[x] = D.cscale[(size_t)m * ldS + x];
-            s_frow[x] = D.fixed_row[(size_t)m * ldS + x];
-            s_A[x] = 0ull;
+            s_row[x] = (MODE == 1) ? D.fixed_row[(size_t)m * ldS + x] : 0;
+            s_A[x] = 0u; s_A[ldS + x] = 0u;
         }
-        for (int x = tid; x < 2 * K; x += kBlock) s_src[x] = D.srccdf[(size_t)m * 2 * K + x];
-        for (int x = tid; x < K; x += kBlock) s_esc[x] = 0ull;
+        for (int x = tid; x < 2 * K; x += kBlock) s_esc[x] = 0u;
         __syncthreads();
 
         unsigned long long* const gA = D.A + (size_t)m * ldS;
         unsigned long long* const g_next = D.next_id + m;
+        const float* const g_src = D.srccdf + (size_t)m * 2 * K;
         const unsigned long long n_ids = R.n_run * (unsigned long long)(mp.has_ext + mp.has_point);
+        const int pi_out = ldS + Np + 1;             // table index on which an escaped package stalls
 
         // ---------------- per-lane package state
-        int st = ST_NEED;
-        float b2 = 0.f, s = 0.f, col = 0.f, r2in = 0.f, r2out = 1.f, rho = 0.f;
-        int j = 0, k = 0, ev_absorb = 0;
+        // flight: along-ray coordinate s, impact parameter^2 b2 (units of R), remaining column col (units of
+        // 1/kappa_ref) to the next event, rho^ of the current shell, candidate surface passage pi (+ its entry E)
+        bool has = false;                            // the lane holds a package
+        float s = 0.f, b2 = 0.f, col = -1.f, rho = 0.f, cn = -1.f;
+        float2 E = make_float2(1.f, 0.f);
+        int pi = ldS + 1, pi0 = ldS + 1, adj = 0;    // candidate now / at the start of the flight; turn correction
+        int k = 0, ev_absorb = 0;
         unsigned blk = 0, ncross = 0;
         unsigned long long id = 0, q = 0;
         int n_ev = 0, pkg = 0;
         // warp-uniform id chunk
         unsigned long long ch_next = 0, ch_end = 0;
         bool exhausted = false;
+        bool launch = false;
         if (TRACE) {
             pkg = blockIdx.x * kBlock + tid;
             exhausted = true;
-            if (pkg < tp.count) { st = ST_LAUNCH; id = tp.first_id + (unsigned long long)pkg; }
+            if (pkg < tp.count) { launch = true; id = tp.first_id + (unsigned long long)pkg; }
         }
 
         for (;;) {
             // ======== uniform point: all 32 lanes converged ========
-            // (1) escapes: warp-first reduction of the escape tally (PAPER.md L87 last sentence)
-            const bool esc = (st == ST_ESCAPED);
+            // a lane whose last crossing attempt failed (cn < 0) has an event pending
+            const bool stuck = has && !(cn >= 0.f);
+            if (stuck) ncross += (unsigned)((pi - pi0) + adj);
+            // (1) escapes: the package stalled beyond the outer surface (PAPER.md L87 last sentence)
+            const bool esc = stuck && (pi == pi_out);
             const unsigned escmask = __ballot_sync(kFull, esc);
             if (escmask) {
-                if (!TRACE) {
-                    if (R.uniform_q) {
-                        const unsigned peers = __match_any_sync(kFull, esc ? k : -1 - lane);
-                        if (esc && lane == __ffs(peers) - 1) atomicAdd(&s_esc[k], q * (unsigned long long)__popc(peers));
-                    } else if (esc) {
-                        atomicAdd(&s_esc[k], q);
-                    }
-                }
                 if (esc) {
+                    if (!TRACE) smem_add64(&s_esc[k], &s_esc[K + k], q);
                     record<TRACE>(tp, pkg, n_ev, 3 /*ESCAPE*/, D.N - 1, k, ncross);
                     if (TRACE) tp.n_events[pkg] = n_ev;
-                    st = ST_NEED;
+                    has = false;
                 }
                 wc_esc += __popc(escmask);
                 wc_cross += __reduce_add_sync(kFull, esc ? ncross : 0u);
             }
             // (2) refill free lanes from the global package counter
             if (!exhausted) {
-                const bool need = (st == ST_NEED);
+                const bool need = !has;
                 const unsigned needmask = __ballot_sync(kFull, need);
                 if (needmask) {
                     const unsigned cnt = __popc(needmask);
@@ -276,26 +300,27 @@ __global__ void __launch_bounds__(kBlock, 3) dies_track(DeviceModel D, RunParams
                         // run-local index -> source and global package id (R2)
                         const bool second = jdx >= R.n_run;
                         id = (second ? R.n_total + (jdx - R.n_run) : jdx) + R.id_base;
-                        st = ST_LAUNCH;
+                        launch = true;
                         blk = 0;
                     }
                 }
             }
-            const unsigned live = __ballot_sync(kFull, st != ST_NEED);
-            if (!live) break;
+            if (!__ballot_sync(kFull, has || launch)) break;
 
             // (3) absorptions: add the package's quantum to the shell tally, keep the old value (L87)
-            const bool isabs = (st == ST_ABSORB);
+            const bool isabs = stuck && !esc && ev_absorb;
+            const bool issca = stuck && !esc && !ev_absorb;
+            int j = (__float_as_int(E.y) < 0) ? (ldS - pi) : (pi - ldS - 1);    // current internal shell
             const unsigned absmask = __ballot_sync(kFull, isabs);
             wc_abs += __popc(absmask);
-            wc_sca += __popc(__ballot_sync(kFull, st == ST_SCATTER));
-            wc_pkg += __popc(__ballot_sync(kFull, st == ST_LAUNCH));
+            wc_sca += __popc(__ballot_sync(kFull, issca));
+            wc_pkg += __popc(__ballot_sync(kFull, launch));
             unsigned long long old = 0;
             if (absmask) {
                 if (TRACE) {
                     if (isabs && MODE == 0) old = gA[j];
                 } else if (MODE == 1) {
-                    if (isabs) atomicAdd(&s_A[j], q);
+                    if (isabs) smem_add64(&s_A[j], &s_A[ldS + j], q);
                 } else if (R.uniform_q) {
                     const unsigned peers = __match_any_sync(kFull, isabs ? j : -1 - lane);
                     const int leader = __ffs(peers) - 1;
@@ -307,39 +332,46 @@ __global__ void __launch_bounds__(kBlock, 3) dies_track(DeviceModel D, RunParams
             }
 
             // (4) events: launch / scatter / absorb+re-emit; one Philox block each (DESIGN.md RNG contract)
-            if (st == ST_LAUNCH || st == ST_SCATTER || isabs) {
+            if (launch || isabs || issca) {
                 uint32_t xw[4];
-                int row = 0;
+                const float* cdf = nullptr;          // table the new frequency bin is drawn from (launch, re-emission)
+                bool point = false;
                 if (isabs) {
+                    int row;
                     if (MODE == 1) {
-                        row = s_frow[j];
+                        row = s_row[j];
                     } else {
                         // emitted power per mass before and after this absorption; rows of the table (R4)
                         const double cs = s_cs[j];
                         const float eps_old = (float)((double)old * cs);
                         const float eps_new = (float)((double)(old + q) * cs);
-                        row = row_of_eps(s_eps, nT, eps_old);
+                        const int hint = s_row[j];
+                        row = row_from(s_eps, nT, hint, eps_old);
+                        if (row > hint) atomicMax(&s_row[j], row);
                         const bool same = (row == nT - 1) || (eps_new < s_eps[row]);
                         if (eps_new >= s_eps[nT - 1]) atomicAdd(&s_cnt[LC_CLAMP_HI], 1ull);
                         if (!same) {
                             philox4x32_10(R.key0, R.key1, (uint32_t)id, (uint32_t)(id >> 32), blk++, (uint32_t)m, xw);
                             const float es = eps_old + uniform24(xw[0]) * (eps_new - eps_old);
-                            row = row_of_eps(s_eps, nT, es);
+                            row = row_from(s_eps, nT, row, es);
                             atomicAdd(&s_cnt[LC_EXTRA_BLOCKS], 1ull);
                         }
                     }
+                    cdf = D.F + (size_t)row * K;
+                } else if (launch) {
+                    point = mp.has_ext ? ((id - R.id_base) >= R.n_total) : true;
+                    cdf = g_src + (point ? K : 0);                              // L55 source spectrum table
                 }
                 philox4x32_10(R.key0, R.key1, (uint32_t)id, (uint32_t)(id >> 32), blk++, (uint32_t)m, xw);
                 const float u0 = uniform24(xw[0]), u1 = uniform24(xw[1]);
                 float tauS = -logf(uniform24(xw[2]));       // Eq. 1
                 float tauA = -logf(uniform24(xw[3]));
+                if (cdf) k = sample_cdf(cdf, K, top, u0);   // new frequency bin (launch: L55; re-emission: L87, R4)
                 bool forced = false;
 
-                if (st == ST_LAUNCH) {
+                if (launch) {
                     // ---- launch
-                    ncross = 0; n_ev = 0;
-                    const bool point = mp.has_ext ? ((id - R.id_base) >= R.n_total) : true;
-                    k = sample_cdf<false>(s_src + (point ? K : 0), K, u0);      // L55 source spectrum table
+                    ncross = 0; n_ev = 0; has = true; launch = false;
                     float w = 1.f;
                     if (!point) {
                         float mu_in;
@@ -347,8 +379,9 @@ __global__ void __launch_bounds__(kBlock, 3) dies_track(DeviceModel D, RunParams
                             mu_in = sqrtf(u1);                                 // Eq. 2
                             b2 = 1.f - u1;
                         } else {
-                            mu_in = powf(u1, R.k_bg);                          // Eq. 5
-                            w = 2.f * R.k_bg * powf(u1, 2.f * R.k_bg - 1.f);
+                            const float l2 = log2f(u1);                        // Eq. 5: mu = u^k_bg,
+                            mu_in = exp2f(R.k_bg * l2);                        //        W = 2 k_bg mu^(2-1/k_bg)
+                            w = 2.f * R.k_bg * exp2f((2.f * R.k_bg - 1.f) * l2);
                             b2 = (1.f - mu_in) * (1.f + mu_in);
                         }
                         s = -mu_in;
@@ -356,40 +389,41 @@ __global__ void __launch_bounds__(kBlock, 3) dies_track(DeviceModel D, RunParams
                     } else {
                         b2 = 0.f; s = mp.r0hat; j = mp.cav;                    // L65, R9: radial
                     }
-                    const float2 pi = s_stab[2 * j], po = s_stab[2 * j + 1];
-                    r2in = pi.x; r2out = po.x; rho = pi.y;
                     q = (unsigned long long)__float2ll_rn(w * (point ? mp.qs_point : mp.qs_ext) * R.qscale);
                     inj_raw += q;
                     record<TRACE>(tp, pkg, n_ev, 0 /*LAUNCH*/, j - mp.cav, k, 0);
                     if (R.ffi) {
                         // ---- forced first interaction (Eq. 9-12, R11): optical depth of the whole chord
-                        float ws = s, wri = r2in, wro = r2out, wrho = rho, colsum = 0.f;
-                        int wj = j;
+                        float ws = s, wrho = fabsf(s_tab[ldS - (j + 1)].y), colsum = 0.f;
+                        int wi = ldS + ((s < 0.f) ? -j : j + 1);
                         unsigned wc = 0;
                         for (;;) {
-                            const bool inward = (ws < 0.f) && (b2 < wri);
-                            const float root = fast_sqrt(fmaxf((inward ? wri : wro) - b2, 0.f));
-                            const float sn = inward ? -root : root;
+                            float2 We = s_tab[wi];
+                            float d = We.x - b2;
+                            if (d <= 0.f) {
+                                if (__float_as_int(We.y) < 0) { wi = 2 * ldS + 1 - wi; We = s_tab[wi]; d = We.x - b2; }
+                                d = fmaxf(d, 0.f);
+                            }
+                            const float root = sqrt_ftz(d);
+                            const float sn = (__float_as_int(We.y) < 0) ? -root : root;
                             colsum += wrho * (sn - ws);
                             ws = sn; wc++;
-                            wj += inward ? -1 : 1;
-                            if (wj == Np) break;
-                            const float2 p = s_stab[2 * wj + (inward ? 0 : 1)];
-                            if (inward) { wro = wri; wri = p.x; } else { wri = wro; wro = p.x; }
-                            wrho = p.y;
+                            wrho = fabsf(We.y);
+                            wi++;
+                            if (wi == pi_out) break;
                         }
                         atomicAdd(&s_cnt[LC_FFI_CROSSINGS], (unsigned long long)wc);
                         const float kext = s_bin[k].w;
                         const float tau0 = kext * colsum;
                         const float P = -expm1f(-tau0);                        // Eq. 12
                         const unsigned long long q_un = min(q, (unsigned long long)__float2ll_rn((float)q * expf(-tau0)));
-                        if (!TRACE && q_un) atomicAdd(&s_esc[k], q_un);        // un-interacted share escapes in bin k
+                        if (!TRACE && q_un) smem_add64(&s_esc[k], &s_esc[K + k], q_un);   // un-interacted share escapes in bin k
                         q -= q_un;
                         if (!(tau0 > 0.f)) {
                             atomicAdd(&s_cnt[LC_UNINTERACTED], 1ull);
                             record<TRACE>(tp, pkg, n_ev, 5 /*UNINTERACTED*/, j - mp.cav, k, 0);
                             if (TRACE) tp.n_events[pkg] = n_ev;
-                            st = ST_NEED;
+                            has = false;
                         } else {
                             const float tauE = -log1pf(-uniform24(xw[2]) * P);  // Eq. 10
                             ev_absorb = !(uniform24(xw[3]) < s_omega[k]);
@@ -399,11 +433,11 @@ __global__ void __launch_bounds__(kBlock, 3) dies_track(DeviceModel D, RunParams
                     }
                 } else {
                     // ---- truncate the step at the event position (L85 / L87)
-                    const float se = s + col / rho;
+                    const float se = s + col / fabsf(rho);
                     const float re2 = fmaf(se, se, b2);
                     const float re = sqrtf(re2);
-                    float mu;
-                    if (st == ST_SCATTER) {
+                    float mu = 2.f * u1 - 1.f;       // re-emission: isotropic (L87)
+                    if (issca) {
                         // ---- scattering with the HG phase function (L85, L167)
                         float mu0 = re > 0.f ? se / re : 1.f;
                         mu0 = fminf(1.f, fmaxf(-1.f, mu0));
@@ -412,18 +446,12 @@ __global__ void __launch_bounds__(kBlock, 3) dies_track(DeviceModel D, RunParams
                         const float sth = sqrtf(fmaxf(1.f - ct * ct, 0.f));
                         mu = mu0 * ct + sm * sth * cospif(2.f * u1);
                         mu = fminf(1.f, fmaxf(-1.f, mu));
-                        record<TRACE>(tp, pkg, n_ev, 1 /*SCATTER*/, j - mp.cav, k, ncross);
-                    } else {
-                        // ---- absorption + immediate re-emission (L87): new frequency from the row CDF,
-                        //      isotropic direction, same position, same energy
-                        k = sample_cdf<true>(D.F + (size_t)row * K, K, u0);
-                        mu = 2.f * u1 - 1.f;
-                        record<TRACE>(tp, pkg, n_ev, 2 /*ABSORB*/, j - mp.cav, k, ncross);
                     }
+                    record<TRACE>(tp, pkg, n_ev, issca ? 1 /*SCATTER*/ : 2 /*ABSORB*/, j - mp.cav, k, ncross);
                     s = re * mu;
                     b2 = re2 * (1.f - mu) * (1.f + mu);
                 }
-                if (st != ST_NEED) {
+                if (has) {
                     if (!forced) {
                         // column (in units of 1/kappa_ref) to the next event and its type (L85/L87; R7 tie -> absorption)
                         const float4 bt = s_bin[k];
@@ -431,43 +459,72 @@ __global__ void __launch_bounds__(kBlock, 3) dies_track(DeviceModel D, RunParams
                         ev_absorb = (cA <= cS);
                         col = fminf(cA, cS);
                     }
-                    st = ST_FLY;
+                    // next flight: from shell j towards its inner (s < 0) or outer surface
+                    pi = ldS + ((s < 0.f) ? -j : j + 1);
+                    pi0 = pi; adj = 0;
+                    rho = s_tab[ldS - (j + 1)].y;
+                    E = s_tab[pi];
+                    cn = 0.f;
+                } else {
+                    // park the lane: its crossing attempts fail without side effects
+                    s = 0.f; b2 = 0.f; col = -1.f; rho = 0.f; cn = -1.f; E = make_float2(1.f, 0.f);
+                    pi = ldS + 1; pi0 = pi; adj = 0;
                 }
+            } else if (!has) {
+                s = 0.f; b2 = 0.f; col = -1.f; rho = 0.f; cn = -1.f; E = make_float2(1.f, 0.f);
+                pi = ldS + 1; pi0 = pi; adj = 0;
             }
 
             // ======== crossing phase (Eq. 4): no RNG, no global memory ========
-            const int thr = max(1, (__popc(live) * R.thr_num) >> 5);
+            // One attempt: distance to the candidate surface sn - s, remaining column cn = col - rho^ (sn - s);
+            // cn >= 0 commits the passage (R7: an event exactly on a surface is a passage); otherwise the lane
+            // leaves the unrolled block untouched and waits for the warp, so a lane with a pending event (or no
+            // package) costs one failing attempt per block.  rho carries the sign bit of its table entry.
+            const int thr = max(1, (__popc(__ballot_sync(kFull, has)) * R.thr_num) >> 5);
+            const float2* pE = s_tab + pi;
             for (;;) {
-                if (st == ST_FLY) {
-                    const bool inward = (s < 0.f) && (b2 < r2in);
-                    const float root = fast_sqrt(fmaxf((inward ? r2in : r2out) - b2, 0.f));
-                    const float sn = inward ? -root : root;
-                    const float dcol = rho * (sn - s);
-                    if (col < dcol) {
-                        st = ev_absorb ? ST_ABSORB : ST_SCATTER;
+#pragma unroll
+                for (int u = 0; u < kUnroll; u++) {
+                    const float d = E.x - b2;
+                    if (d < 0.f) break;                          // tangent shell (or rounding): fixed up below
+                    const float sn = __int_as_float(__float_as_int(sqrt_ftz(d)) | (__float_as_int(E.y) & 0x80000000));
+                    cn = fmaf(-fabsf(rho), sn - s, col);
+                    if (!(cn >= 0.f)) break;                     // event (or escape) before the surface
+                    col = cn;
+                    s = sn;
+                    rho = E.y;
+                    pE++;
+                    E = *pE;
+                }
+                if (E.x - b2 < 0.f) {
+                    if (__float_as_int(E.y) < 0) {
+                        // the inner surface is not reached (tangent shell): head for the outer one instead
+                        const int c = (int)(pE - s_tab) - ldS;
+                        adj += 2 * c - 1;
+                        pE = s_tab + (ldS + 1 - c);
+                        E = *pE;
                     } else {
-                        col -= dcol;
-                        s = sn;
-                        ncross++;
-                        j += inward ? -1 : 1;
-                        const float2 p = s_stab[2 * j + (inward ? 0 : 1)];
-                        if (inward) { r2out = r2in; r2in = p.x; } else { r2in = r2out; r2out = p.x; }
-                        rho = p.y;
-                        if (j == Np) st = ST_ESCAPED;
+                        b2 = E.x;                                // outward, b2 > r^2 by rounding only: graze
                     }
                 }
-                const unsigned fl = __ballot_sync(kFull, st == ST_FLY);
-                if (__popc(fl) < thr) break;
+                if (__popc(__ballot_sync(kFull, cn >= 0.f)) < thr) break;
             }
+            pi = (int)(pE - s_tab);
         }
 
         if (TRACE) break;
         // ---------------- flush the block's privatised tallies
         __syncthreads();
         unsigned long long* const gesc = D.esc + (size_t)m * K;
-        for (int x = tid; x < K; x += kBlock) { const unsigned long long v = s_esc[x]; if (v) atomicAdd(&gesc[x], v); }
+        for (int x = tid; x < K; x += kBlock) {
+            const unsigned long long v = (unsigned long long)s_esc[x] | ((unsigned long long)s_esc[K + x] << 32);
+            if (v) atomicAdd(&gesc[x], v);
+        }
         if (MODE == 1)
-            for (int x = tid; x < Np; x += kBlock) { const unsigned long long v = s_A[x]; if (v) atomicAdd(&gA[x], v); }
+            for (int x = tid; x < Np; x += kBlock) {
+                const unsigned long long v = (unsigned long long)s_A[x] | ((unsigned long long)s_A[ldS + x] << 32);
+                if (v) atomicAdd(&gA[x], v);
+            }
     }
 
     if (TRACE) return;
