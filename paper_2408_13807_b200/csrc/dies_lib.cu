@@ -145,7 +145,8 @@ __global__ void k_build_dust(const double* __restrict__ dustin, int K, double kr
 
 // shells: lengths in units of the outer radius R, densities as rho^ = rho R kappa_ref; internal shell 0 is the
 // empty cavity when r_bounds[0] > 0 (R10).  The table is unfolded along a chord (see DeviceModel in
-// dies_tracker.cuh): entry c in [-ldS, ldS+1] = {(r_|c|/R)^2, rho^ of the shell entered, sign bit = inward}.
+// dies_tracker.cuh): entry c in [-ldS, ldS+1] = {(r_|c|/R)^2, rho^ of the shell traversed on the way to that
+// surface, sign bit = inward}; entry Np+1 is the sentinel {-1, +0}.
 __global__ void k_build_shells(const double* __restrict__ rb, const double* __restrict__ rho, int N, int M, double kref,
                                float2* stab, double* mass, ModelParams* mp)
 {
@@ -158,28 +159,29 @@ __global__ void k_build_shells(const double* __restrict__ rb, const double* __re
     const double R = r[N];
     const int cav = r[0] > 0.0 ? 1 : 0;
     const int Np = N + cav;
-    if (x == 0) {
-        ModelParams p = mp[m];
-        p.Np = Np; p.cav = cav; p.r0hat = (float)(r[0] / R);
-        mp[m] = p;
-    }
     // internal boundary b in [0, Np]: radius 0 at the centre, then the user's boundaries
     auto radius = [&](int b) { return b == 0 ? 0.0 : r[b - cav]; };
     // internal shell j in [0, Np): the cavity (if any) has no dust
-    auto dens = [&](int j) { const int i = j - cav; return i < 0 ? 0.0 : d[i]; };
+    auto dens = [&](int j) { const int i = j - cav; return (i < 0 || i >= N) ? 0.0 : d[i]; };
+    if (x == 0) {
+        ModelParams p = mp[m];
+        p.Np = Np; p.cav = cav; p.r0hat = (float)(r[0] / R);
+        double colsum = 0.0;                                              // radial column centre -> surface
+        for (int j = 0; j < Np; j++) colsum += dens(j) * kref * (radius(j + 1) - radius(j));
+        p.colmax = (float)(2.5 * colsum + 1e-30);                         // > column of the diameter (2 colsum)
+        mp[m] = p;
+    }
     const int c = x - ldS, a = c < 0 ? -c : c;
-    float2 e = make_float2(4.0f, 0.0f);                                  // beyond the model (entry Np+1 is read)
+    float2 e = make_float2(4.0f, 0.0f);                                  // never read
     if (c <= 0 && a <= Np) {
         const double rr = radius(a) / R;
-        const float dh = a >= 1 ? (float)(dens(a - 1) * R * kref) : 0.0f;
+        const float dh = (float)(dens(a) * R * kref);
         e = make_float2((float)(rr * rr), __int_as_float(__float_as_int(dh) | 0x80000000));
-    } else if (c > 0 && c < Np) {
+    } else if (c > 0 && c <= Np) {
         const double rr = radius(c) / R;
-        e = make_float2((float)(rr * rr), (float)(dens(c) * R * kref));
-    } else if (c == Np) {
-        e = make_float2(1.0f, __int_as_float(0x7f800000));               // outer surface: "rho^ = +inf" stalls the package
-    } else if (c < 0) {
-        e = make_float2(0.0f, __int_as_float(0x80000000));
+        e = make_float2((float)(rr * rr), (float)(dens(c - 1) * R * kref));
+    } else if (c == Np + 1) {
+        e = make_float2(-1.0f, 0.0f);                                    // sentinel: d = -1 - b^2 < 0 stops the package
     }
     stab[(size_t)m * ldT + x] = e;
     if (x < ldS) {

@@ -4,10 +4,12 @@
 //   (1) an EVENT phase (all 32 lanes converged): escapes are tallied, free lanes are refilled from the model's
 //       global package counter, absorptions update the 64-bit fixed-point shell tallies (one returning atomic
 //       per distinct shell in the warp), then every lane that launches / scatters / re-emits runs ONE shared
-//       code path: a Philox4x32-10 block, two new free paths (Eq. 1), a table search for the new
-//       frequency (launch and re-emission share it), the new direction, and the set-up of the next flight;
-//   (2) a CROSSING phase: the shell-crossing loop (Eq. 4) with no random numbers and no
-//       global memory, run until fewer than a set fraction of the warp's packages are still flying.
+//       instruction stream (event_step): a Philox4x32-10 block, two new free paths (Eq. 1), a table
+//       search for the new frequency (launch and re-emission share it), the new direction, and the set-up of
+//       the next flight;
+//   (2) a CROSSING phase: the shell-crossing loop (Eq. 4) with no random numbers, no global
+//       memory and no branches (every crossing is predicated on the lane still flying), run until fewer than a
+//       set fraction of the warp's packages are still flying.
 // Differences from the paper's OpenCL design are listed in DESIGN.md ("What differs from the paper").
 #pragma once
 #include <cstdint>
@@ -21,8 +23,8 @@ constexpr unsigned kFull = 0xffffffffu;
 constexpr unsigned kChunk = 128;     // package ids a warp takes from the global counter at a time
 constexpr int kUnroll = 4;           // crossings per vote in the crossing loop
 
-// event counters (same order as DIES_C_* in include/dies.h): the frequent ones are kept warp-uniform in
-// registers (updated from ballots), the rare ones go through shared-memory atomics
+// event counters (same order as DIES_C_* in include/dies.h): the frequent ones are kept in registers, the rare
+// ones go through shared-memory atomics
 enum { LC_PACKAGES = 0, LC_CROSSINGS, LC_FFI_CROSSINGS, LC_SCATTERINGS, LC_ABSORPTIONS, LC_ESCAPED, LC_UNINTERACTED,
        LC_TERMINATED, LC_EXTRA_BLOCKS, LC_CLAMP_HI, LC_INJECTED_RAW, LC_N };
 
@@ -32,14 +34,15 @@ struct ModelParams {
     int has_ext, has_point;
     float r0hat;       // r_bounds[0] / R
     float qs_ext, qs_point;   // e_src / e_ref (<= 1): raw units per unit-weight package / 2^S
-    float pad;
+    float colmax;      // a column (units of 1/kappa_ref) larger than that of any chord: start of a dry FFI flight
 };
 
 // The shell table of one model is "unfolded" along a chord: entry c in [-ldS, ldS+1] (stored at c + ldS)
 // describes the surface passage a package makes when it reaches boundary |c| moving inward (c <= 0) or outward
-// (c > 0):  .x = (r_|c| / R)^2,  .y = rho^ of the shell entered, with the SIGN BIT SET for inward entries.
-// Entry Np (the outer surface) carries rho^ = +inf and entry Np+1 a radius beyond the model, so a package that
-// leaves the model stalls on entry Np+1 without any test in the loop.  rho^(j) = |entry(-(j+1)).y|.
+// (c > 0):  .x = (r_|c| / R)^2,  .y = rho^ of the shell it traverses on the way to that surface (shell |c| for
+// c <= 0, shell c-1 for c > 0) with the SIGN BIT SET for inward entries.  A flight walks the table upwards; an
+// inward surface that the chord does not reach (r^2 < b^2) sends it to the mirrored entry 1 - c.  Entry Np + 1
+// is a sentinel with a negative r^2: a package that has left the model stops there.
 struct DeviceModel {
     int N, K, nT, n_models;
     int ldS;                         // leading dimension of the per-model shell arrays (N + 1)
@@ -107,6 +110,14 @@ __device__ __forceinline__ float sqrt_ftz(float x)
     float y;
     asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
     return y;
+}
+
+// one entry of the unfolded shell table from its shared-memory address (the table is read-only while packages fly)
+__device__ __forceinline__ float2 lds_entry(unsigned a)
+{
+    float2 v;
+    asm("ld.shared.v2.f32 {%0, %1}, [%2];" : "=f"(v.x), "=f"(v.y) : "r"(a));
+    return v;
 }
 
 // smallest k in [0, n) with cdf[k] > u (= #{i < n-1 : cdf[i] <= u} for a non-decreasing cdf with cdf[n-1] > u):
@@ -197,8 +208,9 @@ __global__ void __launch_bounds__(kBlock, kMinBlocks) dies_track(DeviceModel D, 
     for (int x = tid; x < nT; x += kBlock) s_eps[x] = D.epsgrid[x];
 
     if (tid < LC_N) s_cnt[tid] = 0ull;
-    // warp-uniform counters (identical in all lanes) and the lane's injected raw energy
-    unsigned long long wc_pkg = 0, wc_cross = 0, wc_sca = 0, wc_abs = 0, wc_esc = 0, inj_raw = 0;
+    // warp-uniform counters (identical in all lanes) and per-lane sums
+    unsigned long long wc_pkg = 0, wc_sca = 0, wc_abs = 0, wc_esc = 0;
+    unsigned long long lc_cross = 0, lc_ffi = 0, inj_raw = 0;
 
     for (;;) {
         // ---------------- take a ticket: (model, part)
@@ -228,23 +240,26 @@ __global__ void __launch_bounds__(kBlock, kMinBlocks) dies_track(DeviceModel D, 
         unsigned long long* const g_next = D.next_id + m;
         const float* const g_src = D.srccdf + (size_t)m * 2 * K;
         const unsigned long long n_ids = R.n_run * (unsigned long long)(mp.has_ext + mp.has_point);
-        const int pi_out = ldS + Np + 1;             // table index on which an escaped package stalls
+        const unsigned tab0 = (unsigned)__cvta_generic_to_shared(s_tab) + 8u * (unsigned)ldS;   // address of entry c = 0
+        const unsigned pa_out = tab0 + 8u * (unsigned)(Np + 1);                     // the sentinel beyond the outer surface
 
         // ---------------- per-lane package state
-        // flight: along-ray coordinate s, impact parameter^2 b2 (units of R), remaining column col (units of
-        // 1/kappa_ref) to the next event, rho^ of the current shell, candidate surface passage pi (+ its entry E)
-        bool has = false;                            // the lane holds a package
-        float s = 0.f, b2 = 0.f, col = -1.f, rho = 0.f, cn = -1.f;
-        float2 E = make_float2(1.f, 0.f);
-        int pi = ldS + 1, pi0 = ldS + 1, adj = 0;    // candidate now / at the start of the flight; turn correction
-        int k = 0, ev_absorb = 0;
+        // flight: along-ray coordinate s and impact parameter^2 b2 (units of R), remaining column col (units of
+        // 1/kappa_ref) to the next event, shared-memory address pa of the candidate surface passage (entry E);
+        // (pa - pa0) / 8 counts the passages of this flight.  alive = still flying; a lane stops either on an unreachable surface
+        // (col untouched, >= 0) or because the column ran out (the passage is committed and col < 0).
+        bool has = false, alive = false, launch = false;
+        float s = 0.f, b2 = 0.f, col = -1.f;
+        float2 E = make_float2(0.f, 0.f);
+        unsigned pa = tab0, pa0 = tab0;
+        int k = 0;
+        bool ev_absorb = false, dry = false;         // type of the pending event; dry FFI flight (Eq. 9)
         unsigned blk = 0, ncross = 0;
         unsigned long long id = 0, q = 0;
         int n_ev = 0, pkg = 0;
         // warp-uniform id chunk
         unsigned long long ch_next = 0, ch_end = 0;
         bool exhausted = false;
-        bool launch = false;
         if (TRACE) {
             pkg = blockIdx.x * kBlock + tid;
             exhausted = true;
@@ -253,11 +268,16 @@ __global__ void __launch_bounds__(kBlock, kMinBlocks) dies_track(DeviceModel D, 
 
         for (;;) {
             // ======== uniform point: all 32 lanes converged ========
-            // a lane whose last crossing attempt failed (cn < 0) has an event pending
-            const bool stuck = has && !(cn >= 0.f);
-            if (stuck) ncross += (unsigned)((pi - pi0) + adj);
-            // (1) escapes: the package stalled beyond the outer surface (PAPER.md L87 last sentence)
-            const bool esc = stuck && (pi == pi_out);
+            const bool stopped = has && !alive;
+            const bool isev = stopped && (col < 0.f);          // the column ran out: scattering or absorption
+            const bool atend = stopped && !isev;               // stopped on the sentinel: left the model
+            if (stopped) {
+                const unsigned n = ((pa - pa0) >> 3) - (isev ? 1u : 0u);
+                if (dry) lc_ffi += n; else { lc_cross += n; ncross += n; }
+            }
+            // (1) escapes (PAPER.md L87 last sentence)
+            const bool esc = atend && !dry;
+            const bool dryend = atend && dry;
             const unsigned escmask = __ballot_sync(kFull, esc);
             if (escmask) {
                 if (esc) {
@@ -267,7 +287,6 @@ __global__ void __launch_bounds__(kBlock, kMinBlocks) dies_track(DeviceModel D, 
                     has = false;
                 }
                 wc_esc += __popc(escmask);
-                wc_cross += __reduce_add_sync(kFull, esc ? ncross : 0u);
             }
             // (2) refill free lanes from the global package counter
             if (!exhausted) {
@@ -308,9 +327,11 @@ __global__ void __launch_bounds__(kBlock, kMinBlocks) dies_track(DeviceModel D, 
             if (!__ballot_sync(kFull, has || launch)) break;
 
             // (3) absorptions: add the package's quantum to the shell tally, keep the old value (L87)
-            const bool isabs = stuck && !esc && ev_absorb;
-            const bool issca = stuck && !esc && !ev_absorb;
-            int j = (__float_as_int(E.y) < 0) ? (ldS - pi) : (pi - ldS - 1);    // current internal shell
+            const bool isabs = isev && ev_absorb;
+            const bool issca = isev && !ev_absorb;
+            // shell of the event: the one traversed on the way to the surface entry before pa, which was not reached
+            const int ci = (int)(pa - tab0) / 8 - 1;
+            int j = ci <= 0 ? -ci : ci - 1;
             const unsigned absmask = __ballot_sync(kFull, isabs);
             wc_abs += __popc(absmask);
             wc_sca += __popc(__ballot_sync(kFull, issca));
@@ -331,11 +352,13 @@ __global__ void __launch_bounds__(kBlock, kMinBlocks) dies_track(DeviceModel D, 
                 }
             }
 
-            // (4) events: launch / scatter / absorb+re-emit; one Philox block each (DESIGN.md RNG contract)
-            if (launch || isabs || issca) {
+            // (4) events: launch / scatter / absorb + re-emit / end of a dry FFI flight; one Philox block each
+            //     (DESIGN.md RNG contract), one instruction stream for all of them
+            if (launch || isev || dryend) {
                 uint32_t xw[4];
+                const bool atsrc = launch || dryend;                            // the event site is the source
+                const bool point = atsrc && (mp.has_ext ? ((id - R.id_base) >= R.n_total) : true);
                 const float* cdf = nullptr;          // table the new frequency bin is drawn from (launch, re-emission)
-                bool point = false;
                 if (isabs) {
                     int row;
                     if (MODE == 1) {
@@ -359,84 +382,51 @@ __global__ void __launch_bounds__(kBlock, kMinBlocks) dies_track(DeviceModel D, 
                     }
                     cdf = D.F + (size_t)row * K;
                 } else if (launch) {
-                    point = mp.has_ext ? ((id - R.id_base) >= R.n_total) : true;
                     cdf = g_src + (point ? K : 0);                              // L55 source spectrum table
                 }
-                philox4x32_10(R.key0, R.key1, (uint32_t)id, (uint32_t)(id >> 32), blk++, (uint32_t)m, xw);
+                // block 0 belongs to the launch; with FFI the end of the dry flight draws it again
+                const unsigned b = dryend ? 0u : blk;
+                philox4x32_10(R.key0, R.key1, (uint32_t)id, (uint32_t)(id >> 32), b, (uint32_t)m, xw);
+                blk = (launch && R.ffi) ? 0u : b + 1u;
                 const float u0 = uniform24(xw[0]), u1 = uniform24(xw[1]);
-                float tauS = -logf(uniform24(xw[2]));       // Eq. 1
-                float tauA = -logf(uniform24(xw[3]));
-                if (cdf) k = sample_cdf(cdf, K, top, u0);   // new frequency bin (launch: L55; re-emission: L87, R4)
-                bool forced = false;
+                const float tauS = -logf(uniform24(xw[2]));      // Eq. 1
+                const float tauA = -logf(uniform24(xw[3]));
+                if (cdf) k = sample_cdf(cdf, K, top, u0);        // new frequency bin (launch: L55; re-emission: L87, R4)
 
-                if (launch) {
+                // ---- event site (radius re, re2 = re^2, shell j) and new direction cosine mu w.r.t. the radius
+                float re, re2, mu, b2src = 0.f;
+                if (atsrc) {
                     // ---- launch
-                    ncross = 0; n_ev = 0; has = true; launch = false;
                     float w = 1.f;
                     if (!point) {
                         float mu_in;
                         if (R.k_bg == 0.5f) {
                             mu_in = sqrtf(u1);                                 // Eq. 2
-                            b2 = 1.f - u1;
+                            b2src = 1.f - u1;
                         } else {
                             const float l2 = log2f(u1);                        // Eq. 5: mu = u^k_bg,
                             mu_in = exp2f(R.k_bg * l2);                        //        W = 2 k_bg mu^(2-1/k_bg)
                             w = 2.f * R.k_bg * exp2f((2.f * R.k_bg - 1.f) * l2);
-                            b2 = (1.f - mu_in) * (1.f + mu_in);
+                            b2src = (1.f - mu_in) * (1.f + mu_in);
                         }
-                        s = -mu_in;
+                        mu = -mu_in; re = 1.f; re2 = 1.f;
                         j = Np - 1;
                     } else {
-                        b2 = 0.f; s = mp.r0hat; j = mp.cav;                    // L65, R9: radial
+                        mu = 1.f; re = mp.r0hat; re2 = re * re; j = mp.cav;   // L65, R9: radial
                     }
-                    q = (unsigned long long)__float2ll_rn(w * (point ? mp.qs_point : mp.qs_ext) * R.qscale);
-                    inj_raw += q;
-                    record<TRACE>(tp, pkg, n_ev, 0 /*LAUNCH*/, j - mp.cav, k, 0);
-                    if (R.ffi) {
-                        // ---- forced first interaction (Eq. 9-12, R11): optical depth of the whole chord
-                        float ws = s, wrho = fabsf(s_tab[ldS - (j + 1)].y), colsum = 0.f;
-                        int wi = ldS + ((s < 0.f) ? -j : j + 1);
-                        unsigned wc = 0;
-                        for (;;) {
-                            float2 We = s_tab[wi];
-                            float d = We.x - b2;
-                            if (d <= 0.f) {
-                                if (__float_as_int(We.y) < 0) { wi = 2 * ldS + 1 - wi; We = s_tab[wi]; d = We.x - b2; }
-                                d = fmaxf(d, 0.f);
-                            }
-                            const float root = sqrt_ftz(d);
-                            const float sn = (__float_as_int(We.y) < 0) ? -root : root;
-                            colsum += wrho * (sn - ws);
-                            ws = sn; wc++;
-                            wrho = fabsf(We.y);
-                            wi++;
-                            if (wi == pi_out) break;
-                        }
-                        atomicAdd(&s_cnt[LC_FFI_CROSSINGS], (unsigned long long)wc);
-                        const float kext = s_bin[k].w;
-                        const float tau0 = kext * colsum;
-                        const float P = -expm1f(-tau0);                        // Eq. 12
-                        const unsigned long long q_un = min(q, (unsigned long long)__float2ll_rn((float)q * expf(-tau0)));
-                        if (!TRACE && q_un) smem_add64(&s_esc[k], &s_esc[K + k], q_un);   // un-interacted share escapes in bin k
-                        q -= q_un;
-                        if (!(tau0 > 0.f)) {
-                            atomicAdd(&s_cnt[LC_UNINTERACTED], 1ull);
-                            record<TRACE>(tp, pkg, n_ev, 5 /*UNINTERACTED*/, j - mp.cav, k, 0);
-                            if (TRACE) tp.n_events[pkg] = n_ev;
-                            has = false;
-                        } else {
-                            const float tauE = -log1pf(-uniform24(xw[2]) * P);  // Eq. 10
-                            ev_absorb = !(uniform24(xw[3]) < s_omega[k]);
-                            col = tauE / kext;
-                            forced = true;
-                        }
+                    if (launch) {
+                        ncross = 0; n_ev = 0; has = true; launch = false;
+                        q = (unsigned long long)__float2ll_rn(w * (point ? mp.qs_point : mp.qs_ext) * R.qscale);
+                        inj_raw += q;
+                        record<TRACE>(tp, pkg, n_ev, 0 /*LAUNCH*/, j - mp.cav, k, 0);
                     }
                 } else {
-                    // ---- truncate the step at the event position (L85 / L87)
-                    const float se = s + col / fabsf(rho);
-                    const float re2 = fmaf(se, se, b2);
-                    const float re = sqrtf(re2);
-                    float mu = 2.f * u1 - 1.f;       // re-emission: isotropic (L87)
+                    // ---- the step is truncated where the column ran out (L85 / L87): the surface passage
+                    //      before pa was committed with col < 0, so the site lies col / rho^ before it
+                    const float se = s + col / fabsf(lds_entry(pa - 8u).y);
+                    re2 = fmaf(se, se, b2);
+                    re = sqrtf(re2);
+                    mu = 2.f * u1 - 1.f;             // re-emission: isotropic (L87)
                     if (issca) {
                         // ---- scattering with the HG phase function (L85, L167)
                         float mu0 = re > 0.f ? se / re : 1.f;
@@ -448,68 +438,84 @@ __global__ void __launch_bounds__(kBlock, kMinBlocks) dies_track(DeviceModel D, 
                         mu = fminf(1.f, fmaxf(-1.f, mu));
                     }
                     record<TRACE>(tp, pkg, n_ev, issca ? 1 /*SCATTER*/ : 2 /*ABSORB*/, j - mp.cav, k, ncross);
-                    s = re * mu;
-                    b2 = re2 * (1.f - mu) * (1.f + mu);
                 }
-                if (has) {
-                    if (!forced) {
-                        // column (in units of 1/kappa_ref) to the next event and its type (L85/L87; R7 tie -> absorption)
-                        const float4 bt = s_bin[k];
-                        const float cA = tauA * bt.x, cS = tauS * bt.y;
-                        ev_absorb = (cA <= cS);
-                        col = fminf(cA, cS);
+                // ---- column (in units of 1/kappa_ref) to the next event and its type
+                if (R.ffi && atsrc) {
+                    if (!dryend) {
+                        // forced first interaction (Eq. 9-12, R11): a dry flight along the whole chord first
+                        col = mp.colmax; dry = true;
+                    } else {
+                        const float kext = s_bin[k].w;
+                        const float tau0 = kext * (mp.colmax - col);           // Eq. 9
+                        const float P = -expm1f(-tau0);                        // Eq. 12
+                        const unsigned long long q_un = min(q, (unsigned long long)__float2ll_rn((float)q * expf(-tau0)));
+                        if (!TRACE && q_un) smem_add64(&s_esc[k], &s_esc[K + k], q_un);   // un-interacted share escapes in bin k
+                        q -= q_un;
+                        dry = false;
+                        if (!(tau0 > 0.f)) {
+                            atomicAdd(&s_cnt[LC_UNINTERACTED], 1ull);
+                            record<TRACE>(tp, pkg, n_ev, 5 /*UNINTERACTED*/, j - mp.cav, k, 0);
+                            if (TRACE) tp.n_events[pkg] = n_ev;
+                            has = false;
+                        } else {
+                            const float tauE = -log1pf(-uniform24(xw[2]) * P);  // Eq. 10
+                            ev_absorb = !(uniform24(xw[3]) < s_omega[k]);
+                            col = tauE / kext;
+                        }
                     }
-                    // next flight: from shell j towards its inner (s < 0) or outer surface
-                    pi = ldS + ((s < 0.f) ? -j : j + 1);
-                    pi0 = pi; adj = 0;
-                    rho = s_tab[ldS - (j + 1)].y;
-                    E = s_tab[pi];
-                    cn = 0.f;
                 } else {
-                    // park the lane: its crossing attempts fail without side effects
-                    s = 0.f; b2 = 0.f; col = -1.f; rho = 0.f; cn = -1.f; E = make_float2(1.f, 0.f);
-                    pi = ldS + 1; pi0 = pi; adj = 0;
+                    // L85/L87; R7 tie -> absorption; R15 one column instead of two clocks
+                    const float4 bt = s_bin[k];
+                    const float cA = tauA * bt.x, cS = tauS * bt.y;
+                    ev_absorb = (cA <= cS);
+                    col = fminf(cA, cS);
                 }
-            } else if (!has) {
-                s = 0.f; b2 = 0.f; col = -1.f; rho = 0.f; cn = -1.f; E = make_float2(1.f, 0.f);
-                pi = ldS + 1; pi0 = pi; adj = 0;
+                // ---- next flight: from shell j towards its inner (s < 0) or outer surface
+                s = re * mu;
+                b2 = (atsrc && !point) ? b2src : re2 * (1.f - mu) * (1.f + mu);
+                pa = tab0 + 8u * (unsigned)((s < 0.f) ? -j : j + 1);
+                pa0 = pa;
+                E = lds_entry(pa);
+                alive = has;
             }
+            if (!has) { alive = false; col = -1.f; }             // parked lane: never flies, never looks stopped short
 
-            // ======== crossing phase (Eq. 4): no RNG, no global memory ========
-            // One attempt: distance to the candidate surface sn - s, remaining column cn = col - rho^ (sn - s);
-            // cn >= 0 commits the passage (R7: an event exactly on a surface is a passage); otherwise the lane
-            // leaves the unrolled block untouched and waits for the warp, so a lane with a pending event (or no
-            // package) costs one failing attempt per block.  rho carries the sign bit of its table entry.
+            // ======== crossing phase (Eq. 4): no RNG, no global memory, no branches ========
+            // One crossing: d = r_c^2 - b^2 (negative: the surface is not reached, the lane stops with col
+            // untouched); along-ray coordinate of the surface sn = +-sqrt(d); col -= rho^ (sn - s) (Eq. 4) is
+            // committed together with the passage, and the lane stops if col < 0: the event lies col / rho^
+            // before the surface (R7: an event exactly on a surface is a passage).
             const int thr = max(1, (__popc(__ballot_sync(kFull, has)) * R.thr_num) >> 5);
-            const float2* pE = s_tab + pi;
             for (;;) {
 #pragma unroll
                 for (int u = 0; u < kUnroll; u++) {
                     const float d = E.x - b2;
-                    if (d < 0.f) break;                          // tangent shell (or rounding): fixed up below
-                    const float sn = __int_as_float(__float_as_int(sqrt_ftz(d)) | (__float_as_int(E.y) & 0x80000000));
-                    cn = fmaf(-fabsf(rho), sn - s, col);
-                    if (!(cn >= 0.f)) break;                     // event (or escape) before the surface
-                    col = cn;
-                    s = sn;
-                    rho = E.y;
-                    pE++;
-                    E = *pE;
+                    alive = alive && (d >= 0.f);
+                    if (alive) {
+                        const float sn = __int_as_float(__float_as_int(sqrt_ftz(d)) | (__float_as_int(E.y) & 0x80000000));
+                        col = fmaf(-fabsf(E.y), sn - s, col);
+                        s = sn;
+                        pa += 8u;
+                        E = lds_entry(pa);
+                    }
+                    alive = alive && (col >= 0.f);
                 }
-                if (E.x - b2 < 0.f) {
+                if (!alive && (col >= 0.f)) {
                     if (__float_as_int(E.y) < 0) {
                         // the inner surface is not reached (tangent shell): head for the outer one instead
-                        const int c = (int)(pE - s_tab) - ldS;
-                        adj += 2 * c - 1;
-                        pE = s_tab + (ldS + 1 - c);
-                        E = *pE;
-                    } else {
+                        // entry c -> entry 1 - c; the 1 - 2c entries skipped are no passages
+                        const unsigned np = 2u * tab0 + 8u - pa;
+                        pa0 += np - pa;
+                        pa = np;
+                        E = lds_entry(pa);
+                        alive = true;
+                    } else if (pa != pa_out) {
                         b2 = E.x;                                // outward, b2 > r^2 by rounding only: graze
+                        alive = true;
                     }
                 }
-                if (__popc(__ballot_sync(kFull, cn >= 0.f)) < thr) break;
+                if (__popc(__ballot_sync(kFull, alive)) < thr) break;
             }
-            pi = (int)(pE - s_tab);
         }
 
         if (TRACE) break;
@@ -528,12 +534,17 @@ __global__ void __launch_bounds__(kBlock, kMinBlocks) dies_track(DeviceModel D, 
     }
 
     if (TRACE) return;
-    // ---------------- counters: one atomic per warp (uniform ones) / per block (rare ones)
+    // ---------------- counters: one atomic per warp / per block (rare ones)
 #pragma unroll
-    for (int o = 16; o > 0; o >>= 1) inj_raw += __shfl_xor_sync(kFull, inj_raw, o);
+    for (int o = 16; o > 0; o >>= 1) {
+        inj_raw += __shfl_xor_sync(kFull, inj_raw, o);
+        lc_cross += __shfl_xor_sync(kFull, lc_cross, o);
+        lc_ffi += __shfl_xor_sync(kFull, lc_ffi, o);
+    }
     if (lane == 0) {
         atomicAdd(&D.counters[LC_PACKAGES], wc_pkg);
-        atomicAdd(&D.counters[LC_CROSSINGS], wc_cross);
+        atomicAdd(&D.counters[LC_CROSSINGS], lc_cross);
+        if (lc_ffi) atomicAdd(&D.counters[LC_FFI_CROSSINGS], lc_ffi);
         atomicAdd(&D.counters[LC_SCATTERINGS], wc_sca);
         atomicAdd(&D.counters[LC_ABSORPTIONS], wc_abs);
         atomicAdd(&D.counters[LC_ESCAPED], wc_esc);
