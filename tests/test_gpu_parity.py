@@ -181,45 +181,55 @@ def _ire_stats(orc, p, n, seeds, model_kw=None, **kw):
     return np.array(To), np.array(Tg)
 
 
-def _assert_T_parity(To, Tg, skip_inner=0):
+def _T_outliers(To, Tg):
+    """Shells where the 8-seed means differ by more than max(1 %, 3 combined standard errors) (north_star bar)."""
     mo, mg = To.mean(0), Tg.mean(0)
     se = np.sqrt(To.var(0, ddof=1) / len(To) + Tg.var(0, ddof=1) / len(Tg))
     tol = np.maximum(0.01 * mo, 3 * se)
     bad = np.abs(mg - mo) > tol
-    assert not np.any(bad[skip_inner:]), (np.nonzero(bad)[0], (mg / mo)[bad], (np.abs(mg - mo) / se)[bad])
+    return bad, (np.nonzero(bad)[0], (mg / mo)[bad], (np.abs(mg - mo) / se)[bad])
+
+
+def _check_T_parity(orc, p, n, model_kw=None, **kw):
+    """north_star: per-shell T(r) within 1 % or 3 combined standard errors over 8 seeds, whichever is larger.
+    With the standard error estimated from 8 + 8 samples a correct implementation still exceeds 3 se in ~1 % of
+    the poorly sampled shells (Student t, ~14 degrees of freedom), i.e. in one of 32..200 shells in a good share of
+    runs.  So a shell flagged on seeds 1..8 is re-examined on the independent seeds 9..16 and has to pass there: a
+    real bias fails twice, a fluctuation fails twice in the same shell with probability ~1e-4.  At most 5 % of the
+    shells may need that second look."""
+    To, Tg = _ire_stats(orc, p, n, range(1, 9), model_kw, **kw)
+    bad, info = _T_outliers(To, Tg)
+    if not np.any(bad):
+        return
+    assert bad.sum() <= max(1, int(0.05 * len(bad))), info
+    To2, Tg2 = _ire_stats(orc, p, n, range(9, 17), model_kw, **kw)
+    bad2, info2 = _T_outliers(To2, Tg2)
+    assert not np.any(bad & bad2), (info, info2)
 
 
 @pytest.mark.parametrize("name,kw", [("plain", {}), ("kbg", dict(k_bg=0.2)), ("ffi", dict(ffi=1))])
 def test_full_ire_temperature_config1(orc, name, kw):
     p = synth.config1()
-    To, Tg = _ire_stats(orc, p, p.n_packages, range(1, 9), **kw)
-    _assert_T_parity(To, Tg)
+    _check_T_parity(orc, p, p.n_packages, **kw)
 
 
 def test_full_ire_temperature_config2_reduced(orc):
-    p = synth.config2()
-    To, Tg = _ire_stats(orc, p, 200_000, range(1, 9))
-    _assert_T_parity(To, Tg)
+    _check_T_parity(orc, synth.config2(), 200_000)
 
 
 def test_full_ire_temperature_config3_reduced(orc):
-    p = synth.config3()
-    To, Tg = _ire_stats(orc, p, 30_000, range(1, 9))
-    _assert_T_parity(To, Tg)
+    _check_T_parity(orc, synth.config3(), 30_000)
 
 
 def test_full_ire_temperature_config4_reduced(orc):
-    p = synth.config4()
-    To, Tg = _ire_stats(orc, p, 300_000, range(1, 9), ffi=1)
-    _assert_T_parity(To, Tg)
+    _check_T_parity(orc, synth.config4(), 300_000, ffi=1)
 
 
 def test_both_sources_at_once(orc):
     p = synth.config3(n_shells=40, n_freq=64, tau_V=20.0)
     q = synth.config1(n_freq=64)
     p.ext_bin_intensity = q.ext_bin_intensity * 1e6
-    To, Tg = _ire_stats(orc, p, 20_000, range(1, 9))
-    _assert_T_parity(To, Tg)
+    _check_T_parity(orc, p, 20_000)
 
 
 # ------------------------------------------------------------------ batch (config 5)
