@@ -87,7 +87,8 @@ struct dies_model {
     int shift;
     cudaStream_t stream;
     int grid_max, blocks_per_sm, n_sms;
-    size_t smem_bytes;
+    int pool;                             // pool slots per warp of the tracker
+    size_t smem_bytes, smem_trace_bytes;
     unsigned long long launches;
 };
 
@@ -329,11 +330,20 @@ static int check_device()
     return DIES_OK;
 }
 
-static size_t tracker_smem(int N, int K, int nT)
+static int env_int(const char* name, int lo, int hi, int dflt)
 {
-    const size_t ldS = (size_t)N + 1, ldT = 2 * ldS + 2;
-    return (size_t)K * 16 + ldS * 8 + ldT * 8 + (size_t)nT * 4 + (size_t)K * 4 + ldS * 4 + (size_t)2 * K * 4 +
-           2 * ldS * 4 + 64;
+    const char* e = getenv(name);
+    if (e) { int v = atoi(e); if (v >= lo && v <= hi) return v; }
+    return dflt;
+}
+
+// pool slots per warp: a multiple of 8 in [32, kMaxPool]
+static int pool_slots() { return env_int("DIES_POOL", 32, kMaxPool, 96) & ~7; }
+
+static size_t tracker_smem(int N, int K, int nT, int P, bool trace)
+{
+    const int ldS = N + 1, ldT = 2 * ldS + 2;
+    return plan_smem(K, nT, ldS, ldT, P, trace).total;
 }
 
 template <int MODE, bool TRACE>
@@ -356,7 +366,7 @@ extern "C" int dies_device_info(int* n_sms, int* blocks_per_sm, int* threads_per
     int dev = 0, sms = 0, bps = 0;
     CUDA_TRY(cudaGetDevice(&dev));
     CUDA_TRY(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
-    CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&bps, dies_track<0, false>, kBlock, tracker_smem(100, 200, 1000)));
+    CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&bps, dies_track<0, false>, kBlock, tracker_smem(100, 200, 1000, pool_slots(), false)));
     if (n_sms) *n_sms = sms;
     if (blocks_per_sm) *blocks_per_sm = bps;
     if (threads_per_block) *threads_per_block = kBlock;
@@ -398,8 +408,9 @@ extern "C" int dies_create_batch(int n_models, int n_shells, const double* r_bou
     if (rc) return rc;
     const Layout L = make_layout(N, K, nT, M);
     if (workspace_bytes < L.total) return fail(DIES_ENOMEM, "workspace too small: %zu < %zu", workspace_bytes, L.total);
-    const size_t smem = tracker_smem(N, K, nT);
-    if (smem > 200 * 1024) return fail(DIES_EINVAL, "tables do not fit in shared memory (%zu bytes)", smem);
+    const int pool = pool_slots();
+    const size_t smem = tracker_smem(N, K, nT, pool, false), smem_trace = tracker_smem(N, K, nT, pool, true);
+    if (smem_trace > 200 * 1024) return fail(DIES_EINVAL, "tables do not fit in shared memory (%zu bytes)", smem_trace);
 
     dies_model* m = new (std::nothrow) dies_model();
     if (!m) return fail(DIES_ENOMEM, "host allocation failed");
@@ -408,7 +419,7 @@ extern "C" int dies_create_batch(int n_models, int n_shells, const double* r_bou
     m->sources_set = m->fixed_set = m->ran = false;
     m->done = m->n_total = 0; m->shift = 24; m->stream = 0; m->launches = 0;
     m->L_ext.assign(M, 0.0); m->L_point.assign(M, 0.0); m->has_ext.assign(M, 0); m->has_point.assign(M, 0);
-    m->smem_bytes = smem;
+    m->smem_bytes = smem; m->smem_trace_bytes = smem_trace; m->pool = pool;
     DeviceModel& D = m->D;
     D.N = N; D.K = K; D.nT = nT; D.n_models = M; D.ldS = N + 1; D.ldT = 2 * (N + 1) + 2;
     D.bintab = wsp<float4>(m, L.bintab); D.omega = wsp<float>(m, L.omega); D.epsgrid = wsp<float>(m, L.epsgrid);
@@ -445,8 +456,8 @@ extern "C" int dies_create_batch(int n_models, int n_shells, const double* r_bou
     if (hflags[0] & 2) { delete m; return fail(DIES_EINVAL, "row sums of emis must strictly increase with T"); }
     TRY_OR_FREE((set_smem<0, false>(smem)));
     TRY_OR_FREE((set_smem<1, false>(smem)));
-    TRY_OR_FREE((set_smem<0, true>(smem)));
-    TRY_OR_FREE((set_smem<1, true>(smem)));
+    TRY_OR_FREE((set_smem<0, true>(smem_trace)));
+    TRY_OR_FREE((set_smem<1, true>(smem_trace)));
     int dev = 0;
     TRY_OR_FREE(cudaGetDevice(&dev));
     TRY_OR_FREE(cudaDeviceGetAttribute(&m->n_sms, cudaDevAttrMultiProcessorCount, dev));
@@ -542,12 +553,6 @@ extern "C" int dies_set_fixed_temperature(dies_model* m, const double* T, int n)
 }
 
 // ------------------------------------------------------------------ run
-static int thr_from_env()
-{
-    const char* e = getenv("DIES_THRESH");
-    if (e) { int v = atoi(e); if (v >= 0 && v <= 32) return v; }
-    return 16;
-}
 
 static int fill_run_params(dies_model* m, uint64_t n_packages, uint64_t seed, const dies_run_opts* o, RunParams* R,
                            int* mode, int* accumulate, int* shift, uint64_t* n_total)
@@ -568,7 +573,10 @@ static int fill_run_params(dies_model* m, uint64_t n_packages, uint64_t seed, co
     R->k_bg = (float)d.k_bg; R->ffi = d.ffi ? 1 : 0;
     R->uniform_q = (d.k_bg == 0.5 && !d.ffi && !two) ? 1 : 0;
     R->qscale = (float)(1u << d.fixed_shift);
-    R->thr_num = thr_from_env();
+    R->pool = m->pool;
+    R->thr_hi = env_int("DIES_THR_HI", 1, 32, 24);
+    R->thr_lo = env_int("DIES_THR_LO", 1, 32, 12);
+    R->min_ready = env_int("DIES_MIN_READY", 1, kMaxPool, 32);
     R->n_tickets = 0; R->parts = 1;
     return DIES_OK;
 }
@@ -598,7 +606,8 @@ extern "C" int dies_run(dies_model* m, uint64_t n_packages, uint64_t seed, const
     // grid: persistent blocks, at most blocks_per_sm per SM, fewer for tiny runs
     unsigned long long ids = 0;
     for (int i = 0; i < m->M; i++) ids += n_packages * (unsigned long long)(m->has_ext[i] + m->has_point[i]);
-    unsigned long long want = (ids + 2ull * kBlock - 1) / (2ull * kBlock);
+    const unsigned long long per_block = (unsigned long long)kWarps * m->pool;    // packages a block keeps in flight
+    unsigned long long want = (ids + 2ull * per_block - 1) / (2ull * per_block);
     int grid = (int)(want < 1 ? 1 : (want > (unsigned long long)m->grid_max ? m->grid_max : want));
     if (m->M == 1) { R.parts = grid; R.n_tickets = grid; }
     else { R.parts = (8 * grid + m->M - 1) / m->M; if (R.parts < 1) R.parts = 1; R.n_tickets = m->M * R.parts; }
@@ -608,7 +617,7 @@ extern "C" int dies_run(dies_model* m, uint64_t n_packages, uint64_t seed, const
                                                     wsp<double>(m, m->L.epsref), wsp<double>(m, m->L.cscale),
                                                     wsp<double>(m, m->L.eunit), wsp<ModelParams>(m, m->L.mp),
                                                     (double)n_total, (double)R.qscale, accumulate ? 0 : 1);
-    TraceParams tp = {0, 0, 0, nullptr, 0, nullptr};
+    TraceParams tp = {0, 0, 0, nullptr, 0, nullptr, nullptr};
     if (mode == DIES_MODE_IRE) dies_track<0, false><<<grid, kBlock, m->smem_bytes, st>>>(m->D, R, tp);
     else dies_track<1, false><<<grid, kBlock, m->smem_bytes, st>>>(m->D, R, tp);
     m->launches += 2;
@@ -736,12 +745,16 @@ extern "C" int dies_trace_packages(dies_model* m, int model_index, uint64_t firs
     R.n_run = nt; R.id_base = 0;
     int32_t *d_ev = nullptr, *d_n = nullptr;
     CUDA_TRY(cudaMalloc(&d_ev, (size_t)count * max_events * 16));
-    if (cudaMalloc(&d_n, (size_t)count * 4) != cudaSuccess) { cudaFree(d_ev); return fail(DIES_ECUDA, "cudaMalloc failed"); }
-    cudaMemset(d_n, 0, (size_t)count * 4);
-    TraceParams tp = {model_index, first_id, count, d_ev, max_events, d_n};
-    const int grid = (count + kBlock - 1) / kBlock;
-    if (mode == DIES_MODE_IRE) dies_track<0, true><<<grid, kBlock, m->smem_bytes>>>(m->D, R, tp);
-    else dies_track<1, true><<<grid, kBlock, m->smem_bytes>>>(m->D, R, tp);
+    // n_events (count ints) followed by the 64-bit counter the traced package indices are taken from
+    const size_t n_bytes = (((size_t)count * 4 + 7) & ~(size_t)7) + 8;
+    if (cudaMalloc(&d_n, n_bytes) != cudaSuccess) { cudaFree(d_ev); return fail(DIES_ECUDA, "cudaMalloc failed"); }
+    cudaMemset(d_n, 0, n_bytes);
+    TraceParams tp = {model_index, first_id, count, d_ev, max_events, d_n,
+                      reinterpret_cast<unsigned long long*>(reinterpret_cast<unsigned char*>(d_n) + n_bytes - 8)};
+    int grid = (count + kBlock - 1) / kBlock;
+    if (grid > m->grid_max) grid = m->grid_max;
+    if (mode == DIES_MODE_IRE) dies_track<0, true><<<grid, kBlock, m->smem_trace_bytes>>>(m->D, R, tp);
+    else dies_track<1, true><<<grid, kBlock, m->smem_trace_bytes>>>(m->D, R, tp);
     m->launches += 1;
     cudaError_t e = cudaDeviceSynchronize();
     if (e == cudaSuccess) e = cudaMemcpy(events, d_ev, (size_t)count * max_events * 16, cudaMemcpyDeviceToHost);

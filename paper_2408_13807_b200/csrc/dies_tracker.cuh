@@ -1,15 +1,20 @@
 // dies_tracker.cuh -- the persistent-thread IRE package tracker for sm_100a (hot path of include/dies.h).
 //
-// One photon package per lane.  A warp alternates between
-//   (1) an EVENT phase (all 32 lanes converged): escapes are tallied, free lanes are refilled from the model's
-//       global package counter, absorptions update the 64-bit fixed-point shell tallies (one returning atomic
-//       per distinct shell in the warp), then every lane that launches / scatters / re-emits runs ONE shared
-//       instruction stream (event_step): a Philox4x32-10 block, two new free paths (Eq. 1), a table
-//       search for the new frequency (launch and re-emission share it), the new direction, and the set-up of
-//       the next flight;
-//   (2) a CROSSING phase: the shell-crossing loop (Eq. 4) with no random numbers, no global
-//       memory and no branches (every crossing is predicated on the lane still flying), run until fewer than a
-//       set fraction of the warp's packages are still flying.
+// Every warp owns a POOL of P photon packages whose state lives in shared memory (40 bytes per package) and four
+// small queues of pool slots: packages ready to fly, and packages waiting for an absorption, a scattering, or a
+// source event (escape tally + launch of the next package id, or the end of a dry FFI flight).  The warp alternates
+// between
+//   (1) a CROSSING phase: 32 flying packages in registers run the shell-crossing loop (Eq. 4) with
+//       no random numbers, no global memory and no branches (every crossing is predicated on the lane still flying).
+//       When fewer than thr_hi lanes still fly, the stopped lanes write their package back, queue it by event type
+//       and take the next ready package from the pool, so the loop keeps (nearly) all lanes busy until the ready
+//       queue is empty;
+//   (2) an EVENT phase: batches of 32 queued events, of ONE type whenever a queue holds 32 (mixed only when the
+//       crossing phase would starve), run one shared instruction stream: escapes are tallied, new package ids taken
+//       from the model's global counter, absorptions update the 64-bit fixed-point shell tallies (one returning
+//       atomic per distinct shell in the warp, issued before and consumed after the Philox block), then a
+//       Philox4x32-10 block, two new free paths (Eq. 1), the table search for the new frequency, the new
+//       direction and the set-up of the next flight.
 // Differences from the paper's OpenCL design are listed in DESIGN.md ("What differs from the paper").
 #pragma once
 #include <cstdint>
@@ -18,15 +23,21 @@
 namespace dies {
 
 constexpr int kBlock = 256;          // threads per block
-constexpr int kMinBlocks = 3;        // resident blocks per SM asked from the compiler
+constexpr int kWarps = kBlock / 32;
+constexpr int kMinBlocks = 4;        // resident blocks per SM asked from the compiler (64 registers)
 constexpr unsigned kFull = 0xffffffffu;
 constexpr unsigned kChunk = 128;     // package ids a warp takes from the global counter at a time
 constexpr int kUnroll = 4;           // crossings per vote in the crossing loop
+constexpr int kMaxPool = 248;        // pool slots per warp (queue entries are bytes)
 
-// event counters (same order as DIES_C_* in include/dies.h): the frequent ones are kept in registers, the rare
-// ones go through shared-memory atomics
+// event counters (same order as DIES_C_* in include/dies.h), accumulated per block in shared memory
 enum { LC_PACKAGES = 0, LC_CROSSINGS, LC_FFI_CROSSINGS, LC_SCATTERINGS, LC_ABSORPTIONS, LC_ESCAPED, LC_UNINTERACTED,
        LC_TERMINATED, LC_EXTRA_BLOCKS, LC_CLAMP_HI, LC_INJECTED_RAW, LC_N };
+
+// per-slot flag word: frequency bin | type of the pending event | dry FFI flight | slot holds a package
+constexpr unsigned KF_K = 0xffffu, KF_EVABS = 1u << 16, KF_DRY = 1u << 17, KF_OCC = 1u << 18;
+// the queues of a warp
+enum { QT_ABS = 0, QT_SCA, QT_SRC, QT_READY, QT_N };
 
 struct ModelParams {
     int Np;            // internal shells = n_shells + cav
@@ -73,7 +84,10 @@ struct RunParams {
     int uniform_q;                   // all packages carry the same raw quantum (no k_bg, no FFI, one source)
     float qscale;                    // 2^S
     int n_tickets, parts;            // tickets = n_models * parts
-    int thr_num;                     // leave the crossing loop when flying lanes < live * thr_num / 32
+    int pool;                        // P: pool slots per warp (multiple of 8, 32 <= P <= kMaxPool)
+    int thr_hi;                      // crossing phase: swap stopped lanes for ready packages when fewer fly
+    int thr_lo;                      // crossing phase: with no ready package left, leave when fewer fly
+    int min_ready;                   // event phase: mixed batches only while fewer packages are ready
 };
 
 struct TraceParams {
@@ -83,7 +97,33 @@ struct TraceParams {
     int32_t* events;                 // count x max_events x 4
     int max_events;
     int32_t* n_events;               // count
+    unsigned long long* counter;     // zeroed: next traced package
 };
+
+// shared-memory plan of a block (byte offsets), used by the kernel and by the host to size the launch
+struct SmemPlan { unsigned bin, cs, tab, eps, omega, row, esc, A, poolA, poolB, poolQ, queues, trace, total; };
+__host__ __device__ inline SmemPlan plan_smem(int K, int nT, int ldS, int ldT, int P, bool trace)
+{
+    SmemPlan p;
+    unsigned o = 0;
+    p.bin = o;   o += 16u * K;                       // float4 K
+    p.cs = o;    o += 8u * ldS;                      // double ldS
+    p.tab = o;   o += 8u * ldT;                      // float2 ldT
+    p.eps = o;   o += 4u * nT;
+    p.omega = o; o += 4u * K;
+    p.row = o;   o += 4u * ldS;
+    p.esc = o;   o += 8u * K;                        // low words, high words
+    p.A = o;     o += 8u * ldS;                      // low words, high words (fixed-T mode)
+    o = (o + 15u) & ~15u;
+    p.poolA = o; o += 16u * kWarps * P;              // float4 {s, b2, col, pa}
+    p.poolB = o; o += 16u * kWarps * P;              // uint4  {id lo, id hi, blk, flags}
+    p.poolQ = o; o += 8u * kWarps * P;               // raw quantum of the package
+    p.queues = o; o += (unsigned)(QT_N * kWarps * P);
+    o = (o + 15u) & ~15u;
+    p.trace = o; if (trace) o += 12u * kWarps * P;   // pkg, n_ev, crossings so far
+    p.total = o;
+    return p;
+}
 
 // ------------------------------------------------------------------ RNG contract (include/dies.h)
 __device__ __forceinline__ void philox4x32_10(uint32_t k0, uint32_t k1, uint32_t c0, uint32_t c1, uint32_t c2,
@@ -166,6 +206,7 @@ __device__ __forceinline__ void smem_add64(unsigned* lo, unsigned* hi, unsigned 
     if (up) atomicAdd(hi, up);
 }
 
+// per-slot trace state (TRACE kernels only): pkg, number of events so far, crossings so far
 template <bool TRACE>
 __device__ __forceinline__ void record(const TraceParams& tp, int pkg, int& n_ev, int type, int shell, int bin,
                                        unsigned ncross)
@@ -181,36 +222,46 @@ __device__ __forceinline__ void record(const TraceParams& tp, int pkg, int& n_ev
 // ------------------------------------------------------------------ the tracker
 // MODE 0: full IRE (returning 64-bit atomics on the global shell tallies, row from eps_old/eps_new)
 // MODE 1: fixed temperature (row from fixed_row; tallies privatised in shared memory)
-// TRACE : replay tp.count packages of one model, one per lane, tallies read-only, events recorded
+// TRACE : replay tp.count packages of one model, tallies read-only, events recorded
 template <int MODE, bool TRACE>
 __global__ void __launch_bounds__(kBlock, kMinBlocks) dies_track(DeviceModel D, RunParams R, TraceParams tp)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    const int K = D.K, nT = D.nT, ldS = D.ldS, ldT = D.ldT;
-    // shared-memory layout
-    float4* s_bin = reinterpret_cast<float4*>(smem_raw);                          // K
-    double* s_cs = reinterpret_cast<double*>(s_bin + K);                          // ldS
-    float2* s_tab = reinterpret_cast<float2*>(s_cs + ldS);                        // ldT unfolded shell table
-    float* s_eps = reinterpret_cast<float*>(s_tab + ldT);                         // nT
-    float* s_omega = s_eps + nT;                                                  // K
-    int* s_row = reinterpret_cast<int*>(s_omega + K);                             // ldS: fixed rows / row hints
-    unsigned* s_esc = reinterpret_cast<unsigned*>(s_row + ldS);                   // 2K: low words, high words
-    unsigned* s_A = s_esc + 2 * K;                                                // 2 ldS (MODE 1)
+    const int K = D.K, nT = D.nT, ldS = D.ldS, ldT = D.ldT, P = R.pool;
+    const SmemPlan sp = plan_smem(K, nT, ldS, ldT, P, TRACE);
+    float4* const s_bin = reinterpret_cast<float4*>(smem_raw + sp.bin);             // K
+    double* const s_cs = reinterpret_cast<double*>(smem_raw + sp.cs);               // ldS
+    float2* const s_tab = reinterpret_cast<float2*>(smem_raw + sp.tab);             // ldT unfolded shell table
+    float* const s_eps = reinterpret_cast<float*>(smem_raw + sp.eps);               // nT
+    float* const s_omega = reinterpret_cast<float*>(smem_raw + sp.omega);           // K
+    int* const s_row = reinterpret_cast<int*>(smem_raw + sp.row);                   // ldS: fixed rows / row hints
+    unsigned* const s_esc = reinterpret_cast<unsigned*>(smem_raw + sp.esc);         // 2K: low words, high words
+    unsigned* const s_A = reinterpret_cast<unsigned*>(smem_raw + sp.A);             // 2 ldS (MODE 1)
     __shared__ unsigned int s_ticket;
-    __shared__ unsigned long long s_cnt[LC_N];      // rare counters, flushed at kernel end
+    __shared__ unsigned long long s_cnt[LC_N];      // counters of the block, flushed at kernel end
 
-    const int tid = threadIdx.x, lane = tid & 31;
+    const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
     const unsigned lt_mask = (1u << lane) - 1u;
+    // the pool and the queues of this warp
+    float4* const pA = reinterpret_cast<float4*>(smem_raw + sp.poolA) + wid * P;
+    uint4* const pB = reinterpret_cast<uint4*>(smem_raw + sp.poolB) + wid * P;
+    unsigned long long* const pQ = reinterpret_cast<unsigned long long*>(smem_raw + sp.poolQ) + wid * P;
+    unsigned char* const qA = smem_raw + sp.queues + (size_t)wid * QT_N * P;
+    unsigned char* const qS = qA + P;
+    unsigned char* const qL = qS + P;
+    unsigned char* const qR = qL + P;
+    int* const pT = reinterpret_cast<int*>(smem_raw + sp.trace) + wid * 3 * P;      // TRACE only
+
     int top = 0;                                     // largest power of two <= K-1 (trip count of sample_cdf)
     for (int t = 1; t <= K - 1; t <<= 1) top = t;
 
     for (int x = tid; x < K; x += kBlock) { s_bin[x] = D.bintab[x]; s_omega[x] = D.omega[x]; }
     for (int x = tid; x < nT; x += kBlock) s_eps[x] = D.epsgrid[x];
-
     if (tid < LC_N) s_cnt[tid] = 0ull;
-    // warp-uniform counters (identical in all lanes) and per-lane sums
-    unsigned long long wc_pkg = 0, wc_sca = 0, wc_abs = 0, wc_esc = 0;
-    unsigned long long lc_cross = 0, lc_ffi = 0, inj_raw = 0;
+
+    const int thr_hi = R.thr_hi, thr_lo = R.thr_lo, min_ready = R.min_ready;
+    // warp-uniform event counts and per-lane crossing counts since the last flush into s_cnt
+    unsigned wc_pkg = 0, wc_sca = 0, wc_abs = 0, wc_esc = 0, lc_cross = 0, lc_ffi = 0;
 
     for (;;) {
         // ---------------- take a ticket: (model, part)
@@ -234,67 +285,110 @@ __global__ void __launch_bounds__(kBlock, kMinBlocks) dies_track(DeviceModel D, 
             s_A[x] = 0u; s_A[ldS + x] = 0u;
         }
         for (int x = tid; x < 2 * K; x += kBlock) s_esc[x] = 0u;
+        // every slot of the pool is free and waits for a package id
+        for (int x = lane; x < P; x += 32) { qL[x] = (unsigned char)x; pB[x] = make_uint4(0u, 0u, 0u, 0u); }
         __syncthreads();
 
         unsigned long long* const gA = D.A + (size_t)m * ldS;
-        unsigned long long* const g_next = D.next_id + m;
+        unsigned long long* const g_next = TRACE ? tp.counter : D.next_id + m;
         const float* const g_src = D.srccdf + (size_t)m * 2 * K;
-        const unsigned long long n_ids = R.n_run * (unsigned long long)(mp.has_ext + mp.has_point);
+        const unsigned long long n_ids = TRACE ? (unsigned long long)tp.count
+                                               : R.n_run * (unsigned long long)(mp.has_ext + mp.has_point);
         const unsigned tab0 = (unsigned)__cvta_generic_to_shared(s_tab) + 8u * (unsigned)ldS;   // address of entry c = 0
         const unsigned pa_out = tab0 + 8u * (unsigned)(Np + 1);                     // the sentinel beyond the outer surface
+        // raw quantum when every package carries the same one
+        const unsigned long long q_uni =
+            (unsigned long long)__float2ll_rn((mp.has_ext ? mp.qs_ext : mp.qs_point) * R.qscale);
 
-        // ---------------- per-lane package state
-        // flight: along-ray coordinate s and impact parameter^2 b2 (units of R), remaining column col (units of
-        // 1/kappa_ref) to the next event, shared-memory address pa of the candidate surface passage (entry E);
-        // (pa - pa0) / 8 counts the passages of this flight.  alive = still flying; a lane stops either on an unreachable surface
-        // (col untouched, >= 0) or because the column ran out (the passage is committed and col < 0).
-        bool has = false, alive = false, launch = false;
-        float s = 0.f, b2 = 0.f, col = -1.f;
-        float2 E = make_float2(0.f, 0.f);
-        unsigned pa = tab0, pa0 = tab0;
-        int k = 0;
-        bool ev_absorb = false, dry = false;         // type of the pending event; dry FFI flight (Eq. 9)
-        unsigned blk = 0, ncross = 0;
-        unsigned long long id = 0, q = 0;
-        int n_ev = 0, pkg = 0;
-        // warp-uniform id chunk
-        unsigned long long ch_next = 0, ch_end = 0;
+        int nA = 0, nS = 0, nL = P, nR = 0;          // queue lengths (warp-uniform)
+        unsigned long long ch_next = 0, ch_end = 0;  // warp-uniform id chunk
         bool exhausted = false;
-        if (TRACE) {
-            pkg = blockIdx.x * kBlock + tid;
-            exhausted = true;
-            if (pkg < tp.count) { launch = true; id = tp.first_id + (unsigned long long)pkg; }
-        }
 
         for (;;) {
-            // ======== uniform point: all 32 lanes converged ========
-            const bool stopped = has && !alive;
-            const bool isev = stopped && (col < 0.f);          // the column ran out: scattering or absorption
-            const bool atend = stopped && !isev;               // stopped on the sentinel: left the model
-            if (stopped) {
-                const unsigned n = ((pa - pa0) >> 3) - (isev ? 1u : 0u);
-                if (dry) lc_ffi += n; else { lc_cross += n; ncross += n; }
-            }
-            // (1) escapes (PAPER.md L87 last sentence)
-            const bool esc = atend && !dry;
-            const bool dryend = atend && dry;
-            const unsigned escmask = __ballot_sync(kFull, esc);
-            if (escmask) {
-                if (esc) {
-                    if (!TRACE) smem_add64(&s_esc[k], &s_esc[K + k], q);
-                    record<TRACE>(tp, pkg, n_ev, 3 /*ESCAPE*/, D.N - 1, k, ncross);
-                    if (TRACE) tp.n_events[pkg] = n_ev;
-                    has = false;
+            // =====================================================================================
+            // EVENT phase: batches of up to 32 queued events
+            // =====================================================================================
+            for (;;) {
+                if (nA + nS + nL == 0) break;
+                int cA = 0, cS = 0, cL = 0;
+                if (nA >= 32) cA = 32;
+                else if (nL >= 32) cL = 32;
+                else if (nS >= 32) cS = 32;
+                else {
+                    if (nR >= min_ready) break;                  // enough to fly: let the partial batches grow
+                    cA = nA; cS = min(nS, 32 - cA); cL = min(nL, 32 - cA - cS);
                 }
-                wc_esc += __popc(escmask);
-            }
-            // (2) refill free lanes from the global package counter
-            if (!exhausted) {
-                const bool need = !has;
+                int type = -1;
+                unsigned slot = 0;
+                {
+                    int l = lane;
+                    if (l < cA) { type = QT_ABS; slot = qA[nA - 1 - l]; }
+                    else if ((l -= cA) < cS) { type = QT_SCA; slot = qS[nS - 1 - l]; }
+                    else if ((l -= cS) < cL) { type = QT_SRC; slot = qL[nL - 1 - l]; }
+                }
+                nA -= cA; nS -= cS; nL -= cL;
+                const bool isabs = type == QT_ABS, issca = type == QT_SCA, issrc = type == QT_SRC;
+                const bool isev = isabs || issca;
+
+                // ---- the package of the slot
+                float s = 0.f, b2 = 0.f, col = 0.f;
+                unsigned pa = tab0, blk = 0, kf = 0;
+                unsigned long long id = 0, q = q_uni;
+                int pkg = 0, n_ev = 0;
+                unsigned ncross = 0;
+                if (type >= 0) {
+                    const float4 a = pA[slot];
+                    const uint4 b = pB[slot];
+                    s = a.x; b2 = a.y; col = a.z; pa = __float_as_uint(a.w);
+                    id = (unsigned long long)b.x | ((unsigned long long)b.y << 32); blk = b.z; kf = b.w;
+                    if (!R.uniform_q) q = pQ[slot];
+                    if (TRACE) { pkg = pT[slot]; n_ev = pT[P + slot]; ncross = (unsigned)pT[2 * P + slot]; }
+                }
+                int k = (int)(kf & KF_K);
+                const bool dryend = issrc && (kf & KF_DRY);      // the dry FFI flight reached the far surface
+                const bool esc = issrc && !dryend && (kf & KF_OCC);
+
+                // (1) absorptions first: add the package's quantum to the shell tally, keep the old value (L87).
+                //     The returning atomic is issued here and its result is only needed after the Philox block.
+                // shell of the event: the one traversed on the way to the surface entry before pa, which was not reached
+                const int ci = (int)(pa - tab0) / 8 - 1;
+                int j = ci <= 0 ? -ci : ci - 1;
+                const unsigned absmask = __ballot_sync(kFull, isabs);
+                unsigned long long old = 0;
+                if (absmask) {
+                    if (TRACE) {
+                        if (isabs && MODE == 0) old = gA[j];
+                    } else if (MODE == 1) {
+                        if (isabs) smem_add64(&s_A[j], &s_A[ldS + j], q);
+                    } else if (R.uniform_q) {
+                        const unsigned peers = __match_any_sync(kFull, isabs ? j : -1 - lane);
+                        const int leader = __ffs(peers) - 1;
+                        if (isabs && lane == leader) old = atomicAdd(&gA[j], q * (unsigned long long)__popc(peers));
+                        old = __shfl_sync(kFull, old, leader) + q * (unsigned long long)__popc(peers & lt_mask);
+                    } else if (isabs) {
+                        old = atomicAdd(&gA[j], q);
+                    }
+                    wc_abs += __popc(absmask);
+                }
+                wc_sca += __popc(__ballot_sync(kFull, issca));
+
+                // (2) escapes (PAPER.md L87 last sentence)
+                const unsigned escmask = __ballot_sync(kFull, esc);
+                if (escmask) {
+                    if (esc) {
+                        if (!TRACE) smem_add64(&s_esc[k], &s_esc[K + k], q);
+                        record<TRACE>(tp, pkg, n_ev, 3 /*ESCAPE*/, D.N - 1, k, ncross);
+                        if (TRACE) tp.n_events[pkg] = n_ev;
+                    }
+                    wc_esc += __popc(escmask);
+                }
+                // (3) free slots take the next package id from the global counter
+                bool launch = false;
+                const bool need = issrc && !dryend;
                 const unsigned needmask = __ballot_sync(kFull, need);
-                if (needmask) {
+                if (needmask && !exhausted) {
                     const unsigned cnt = __popc(needmask);
-                    unsigned rank = __popc(needmask & lt_mask);
+                    const unsigned rank = __popc(needmask & lt_mask);
                     const unsigned long long avail = ch_end - ch_next;
                     unsigned long long jdx = ch_next + rank;
                     bool got = need && (rank < avail);
@@ -316,206 +410,312 @@ __global__ void __launch_bounds__(kBlock, kMinBlocks) dies_track(DeviceModel D, 
                         ch_end = nend;
                     }
                     if (got) {
-                        // run-local index -> source and global package id (R2)
-                        const bool second = jdx >= R.n_run;
-                        id = (second ? R.n_total + (jdx - R.n_run) : jdx) + R.id_base;
+                        if (TRACE) {
+                            pkg = (int)jdx;
+                            id = tp.first_id + jdx;
+                        } else {
+                            // run-local index -> source and global package id (R2)
+                            const bool second = jdx >= R.n_run;
+                            id = (second ? R.n_total + (jdx - R.n_run) : jdx) + R.id_base;
+                        }
                         launch = true;
                         blk = 0;
                     }
+                    wc_pkg += __popc(__ballot_sync(kFull, launch));
                 }
-            }
-            if (!__ballot_sync(kFull, has || launch)) break;
 
-            // (3) absorptions: add the package's quantum to the shell tally, keep the old value (L87)
-            const bool isabs = isev && ev_absorb;
-            const bool issca = isev && !ev_absorb;
-            // shell of the event: the one traversed on the way to the surface entry before pa, which was not reached
-            const int ci = (int)(pa - tab0) / 8 - 1;
-            int j = ci <= 0 ? -ci : ci - 1;
-            const unsigned absmask = __ballot_sync(kFull, isabs);
-            wc_abs += __popc(absmask);
-            wc_sca += __popc(__ballot_sync(kFull, issca));
-            wc_pkg += __popc(__ballot_sync(kFull, launch));
-            unsigned long long old = 0;
-            if (absmask) {
-                if (TRACE) {
-                    if (isabs && MODE == 0) old = gA[j];
-                } else if (MODE == 1) {
-                    if (isabs) smem_add64(&s_A[j], &s_A[ldS + j], q);
-                } else if (R.uniform_q) {
-                    const unsigned peers = __match_any_sync(kFull, isabs ? j : -1 - lane);
-                    const int leader = __ffs(peers) - 1;
-                    if (isabs && lane == leader) old = atomicAdd(&gA[j], q * (unsigned long long)__popc(peers));
-                    old = __shfl_sync(kFull, old, leader) + q * (unsigned long long)__popc(peers & lt_mask);
-                } else if (isabs) {
-                    old = atomicAdd(&gA[j], q);
-                }
-            }
-
-            // (4) events: launch / scatter / absorb + re-emit / end of a dry FFI flight; one Philox block each
-            //     (DESIGN.md RNG contract), one instruction stream for all of them
-            if (launch || isev || dryend) {
-                uint32_t xw[4];
-                const bool atsrc = launch || dryend;                            // the event site is the source
-                const bool point = atsrc && (mp.has_ext ? ((id - R.id_base) >= R.n_total) : true);
-                const float* cdf = nullptr;          // table the new frequency bin is drawn from (launch, re-emission)
-                if (isabs) {
-                    int row;
-                    if (MODE == 1) {
-                        row = s_row[j];
-                    } else {
-                        // emitted power per mass before and after this absorption; rows of the table (R4)
-                        const double cs = s_cs[j];
-                        const float eps_old = (float)((double)old * cs);
-                        const float eps_new = (float)((double)(old + q) * cs);
-                        const int hint = s_row[j];
-                        row = row_from(s_eps, nT, hint, eps_old);
-                        if (row > hint) atomicMax(&s_row[j], row);
-                        const bool same = (row == nT - 1) || (eps_new < s_eps[row]);
-                        if (eps_new >= s_eps[nT - 1]) atomicAdd(&s_cnt[LC_CLAMP_HI], 1ull);
-                        if (!same) {
-                            philox4x32_10(R.key0, R.key1, (uint32_t)id, (uint32_t)(id >> 32), blk++, (uint32_t)m, xw);
-                            const float es = eps_old + uniform24(xw[0]) * (eps_new - eps_old);
-                            row = row_from(s_eps, nT, row, es);
-                            atomicAdd(&s_cnt[LC_EXTRA_BLOCKS], 1ull);
-                        }
-                    }
-                    cdf = D.F + (size_t)row * K;
-                } else if (launch) {
-                    cdf = g_src + (point ? K : 0);                              // L55 source spectrum table
-                }
-                // block 0 belongs to the launch; with FFI the end of the dry flight draws it again
-                const unsigned b = dryend ? 0u : blk;
-                philox4x32_10(R.key0, R.key1, (uint32_t)id, (uint32_t)(id >> 32), b, (uint32_t)m, xw);
-                blk = (launch && R.ffi) ? 0u : b + 1u;
-                const float u0 = uniform24(xw[0]), u1 = uniform24(xw[1]);
-                const float tauS = -logf(uniform24(xw[2]));      // Eq. 1
-                const float tauA = -logf(uniform24(xw[3]));
-                if (cdf) k = sample_cdf(cdf, K, top, u0);        // new frequency bin (launch: L55; re-emission: L87, R4)
-
-                // ---- event site (radius re, re2 = re^2, shell j) and new direction cosine mu w.r.t. the radius
-                float re, re2, mu, b2src = 0.f;
-                if (atsrc) {
-                    // ---- launch
-                    float w = 1.f;
-                    if (!point) {
-                        float mu_in;
-                        if (R.k_bg == 0.5f) {
-                            mu_in = sqrtf(u1);                                 // Eq. 2
-                            b2src = 1.f - u1;
+                // (4) events: launch / scatter / absorb + re-emit / end of a dry FFI flight; one Philox block each
+                //     (DESIGN.md RNG contract), one instruction stream for all of them
+                bool fly = false, ev_absorb = false, dry = false, uninter = false;
+                if (launch || isev || dryend) {
+                    uint32_t xw[4];
+                    const bool atsrc = launch || dryend;                            // the event site is the source
+                    const bool point = atsrc && (mp.has_ext ? ((id - R.id_base) >= R.n_total) : true);
+                    // block 0 belongs to the launch; with FFI the end of the dry flight draws it again
+                    unsigned b = dryend ? 0u : blk;
+                    philox4x32_10(R.key0, R.key1, (uint32_t)id, (uint32_t)(id >> 32), b, (uint32_t)m, xw);
+                    const float* cdf = nullptr;      // table the new frequency bin is drawn from (launch, re-emission)
+                    if (isabs) {
+                        int row;
+                        if (MODE == 1) {
+                            row = s_row[j];
                         } else {
-                            const float l2 = log2f(u1);                        // Eq. 5: mu = u^k_bg,
-                            mu_in = exp2f(R.k_bg * l2);                        //        W = 2 k_bg mu^(2-1/k_bg)
-                            w = 2.f * R.k_bg * exp2f((2.f * R.k_bg - 1.f) * l2);
-                            b2src = (1.f - mu_in) * (1.f + mu_in);
+                            // emitted power per mass before and after this absorption; rows of the table (R4)
+                            const double cs = s_cs[j];
+                            const float eps_old = (float)((double)old * cs);
+                            const float eps_new = (float)((double)(old + q) * cs);
+                            const int hint = s_row[j];
+                            row = row_from(s_eps, nT, hint, eps_old);
+                            if (row > hint) atomicMax(&s_row[j], row);
+                            const bool same = (row == nT - 1) || (eps_new < s_eps[row]);
+                            if (eps_new >= s_eps[nT - 1]) atomicAdd(&s_cnt[LC_CLAMP_HI], 1ull);
+                            if (!same) {
+                                // the interval spans table rows: block b gives eps*, the event block is b + 1
+                                const float es = eps_old + uniform24(xw[0]) * (eps_new - eps_old);
+                                row = row_from(s_eps, nT, row, es);
+                                atomicAdd(&s_cnt[LC_EXTRA_BLOCKS], 1ull);
+                                b++;
+                                philox4x32_10(R.key0, R.key1, (uint32_t)id, (uint32_t)(id >> 32), b, (uint32_t)m, xw);
+                            }
                         }
-                        mu = -mu_in; re = 1.f; re2 = 1.f;
-                        j = Np - 1;
-                    } else {
-                        mu = 1.f; re = mp.r0hat; re2 = re * re; j = mp.cav;   // L65, R9: radial
+                        cdf = D.F + (size_t)row * K;
+                    } else if (launch) {
+                        cdf = g_src + (point ? K : 0);                              // L55 source spectrum table
                     }
-                    if (launch) {
-                        ncross = 0; n_ev = 0; has = true; launch = false;
-                        q = (unsigned long long)__float2ll_rn(w * (point ? mp.qs_point : mp.qs_ext) * R.qscale);
-                        inj_raw += q;
-                        record<TRACE>(tp, pkg, n_ev, 0 /*LAUNCH*/, j - mp.cav, k, 0);
-                    }
-                } else {
-                    // ---- the step is truncated where the column ran out (L85 / L87): the surface passage
-                    //      before pa was committed with col < 0, so the site lies col / rho^ before it
-                    const float se = s + col / fabsf(lds_entry(pa - 8u).y);
-                    re2 = fmaf(se, se, b2);
-                    re = sqrtf(re2);
-                    mu = 2.f * u1 - 1.f;             // re-emission: isotropic (L87)
-                    if (issca) {
-                        // ---- scattering with the HG phase function (L85, L167)
-                        float mu0 = re > 0.f ? se / re : 1.f;
-                        mu0 = fminf(1.f, fmaxf(-1.f, mu0));
-                        const float ct = hg_cos(s_bin[k].z, u0);
-                        const float sm = sqrtf(fmaxf(1.f - mu0 * mu0, 0.f));
-                        const float sth = sqrtf(fmaxf(1.f - ct * ct, 0.f));
-                        mu = mu0 * ct + sm * sth * cospif(2.f * u1);
-                        mu = fminf(1.f, fmaxf(-1.f, mu));
-                    }
-                    record<TRACE>(tp, pkg, n_ev, issca ? 1 /*SCATTER*/ : 2 /*ABSORB*/, j - mp.cav, k, ncross);
-                }
-                // ---- column (in units of 1/kappa_ref) to the next event and its type
-                if (R.ffi && atsrc) {
-                    if (!dryend) {
-                        // forced first interaction (Eq. 9-12, R11): a dry flight along the whole chord first
-                        col = mp.colmax; dry = true;
-                    } else {
-                        const float kext = s_bin[k].w;
-                        const float tau0 = kext * (mp.colmax - col);           // Eq. 9
-                        const float P = -expm1f(-tau0);                        // Eq. 12
-                        const unsigned long long q_un = min(q, (unsigned long long)__float2ll_rn((float)q * expf(-tau0)));
-                        if (!TRACE && q_un) smem_add64(&s_esc[k], &s_esc[K + k], q_un);   // un-interacted share escapes in bin k
-                        q -= q_un;
-                        dry = false;
-                        if (!(tau0 > 0.f)) {
-                            atomicAdd(&s_cnt[LC_UNINTERACTED], 1ull);
-                            record<TRACE>(tp, pkg, n_ev, 5 /*UNINTERACTED*/, j - mp.cav, k, 0);
-                            if (TRACE) tp.n_events[pkg] = n_ev;
-                            has = false;
-                        } else {
-                            const float tauE = -log1pf(-uniform24(xw[2]) * P);  // Eq. 10
-                            ev_absorb = !(uniform24(xw[3]) < s_omega[k]);
-                            col = tauE / kext;
-                        }
-                    }
-                } else {
-                    // L85/L87; R7 tie -> absorption; R15 one column instead of two clocks
-                    const float4 bt = s_bin[k];
-                    const float cA = tauA * bt.x, cS = tauS * bt.y;
-                    ev_absorb = (cA <= cS);
-                    col = fminf(cA, cS);
-                }
-                // ---- next flight: from shell j towards its inner (s < 0) or outer surface
-                s = re * mu;
-                b2 = (atsrc && !point) ? b2src : re2 * (1.f - mu) * (1.f + mu);
-                pa = tab0 + 8u * (unsigned)((s < 0.f) ? -j : j + 1);
-                pa0 = pa;
-                E = lds_entry(pa);
-                alive = has;
-            }
-            if (!has) { alive = false; col = -1.f; }             // parked lane: never flies, never looks stopped short
+                    blk = (launch && R.ffi) ? 0u : b + 1u;
+                    const float u0 = uniform24(xw[0]), u1 = uniform24(xw[1]);
+                    const float tauS = -logf(uniform24(xw[2]));      // Eq. 1
+                    const float tauA = -logf(uniform24(xw[3]));
+                    if (cdf) k = sample_cdf(cdf, K, top, u0);        // new frequency bin (launch: L55; re-emission: L87, R4)
 
-            // ======== crossing phase (Eq. 4): no RNG, no global memory, no branches ========
+                    // ---- event site (radius re, re2 = re^2, shell j) and new direction cosine mu w.r.t. the radius
+                    float re, re2, mu, b2src = 0.f;
+                    fly = true;
+                    if (atsrc) {
+                        // ---- launch
+                        float w = 1.f;
+                        if (!point) {
+                            float mu_in;
+                            if (R.k_bg == 0.5f) {
+                                mu_in = sqrtf(u1);                                 // Eq. 2
+                                b2src = 1.f - u1;
+                            } else {
+                                const float l2 = log2f(u1);                        // Eq. 5: mu = u^k_bg,
+                                mu_in = exp2f(R.k_bg * l2);                        //        W = 2 k_bg mu^(2-1/k_bg)
+                                w = 2.f * R.k_bg * exp2f((2.f * R.k_bg - 1.f) * l2);
+                                b2src = (1.f - mu_in) * (1.f + mu_in);
+                            }
+                            mu = -mu_in; re = 1.f; re2 = 1.f;
+                            j = Np - 1;
+                        } else {
+                            mu = 1.f; re = mp.r0hat; re2 = re * re; j = mp.cav;   // L65, R9: radial
+                        }
+                        if (launch) {
+                            ncross = 0; n_ev = 0;
+                            q = (unsigned long long)__float2ll_rn(w * (point ? mp.qs_point : mp.qs_ext) * R.qscale);
+                            record<TRACE>(tp, pkg, n_ev, 0 /*LAUNCH*/, j - mp.cav, k, 0);
+                        }
+                    } else {
+                        // ---- the step is truncated where the column ran out (L85 / L87): the surface passage
+                        //      before pa was committed with col < 0, so the site lies col / rho^ before it
+                        const float se = s + col / fabsf(lds_entry(pa - 8u).y);
+                        re2 = fmaf(se, se, b2);
+                        re = sqrtf(re2);
+                        mu = 2.f * u1 - 1.f;             // re-emission: isotropic (L87)
+                        if (issca) {
+                            // ---- scattering with the HG phase function (L85, L167)
+                            float mu0 = re > 0.f ? se / re : 1.f;
+                            mu0 = fminf(1.f, fmaxf(-1.f, mu0));
+                            const float ct = hg_cos(s_bin[k].z, u0);
+                            const float sm = sqrtf(fmaxf(1.f - mu0 * mu0, 0.f));
+                            const float sth = sqrtf(fmaxf(1.f - ct * ct, 0.f));
+                            mu = mu0 * ct + sm * sth * cospif(2.f * u1);
+                            mu = fminf(1.f, fmaxf(-1.f, mu));
+                        }
+                        record<TRACE>(tp, pkg, n_ev, issca ? 1 /*SCATTER*/ : 2 /*ABSORB*/, j - mp.cav, k, ncross);
+                    }
+                    // ---- column (in units of 1/kappa_ref) to the next event and its type
+                    if (R.ffi && atsrc) {
+                        if (!dryend) {
+                            // forced first interaction (Eq. 9-12, R11): a dry flight along the whole chord first
+                            col = mp.colmax; dry = true;
+                        } else {
+                            const float kext = s_bin[k].w;
+                            const float tau0 = kext * (mp.colmax - col);           // Eq. 9
+                            const float Pint = -expm1f(-tau0);                     // Eq. 12
+                            const unsigned long long q_un = min(q, (unsigned long long)__float2ll_rn((float)q * expf(-tau0)));
+                            if (!TRACE && q_un) smem_add64(&s_esc[k], &s_esc[K + k], q_un);   // un-interacted share escapes in bin k
+                            q -= q_un;
+                            if (!(tau0 > 0.f)) {
+                                atomicAdd(&s_cnt[LC_UNINTERACTED], 1ull);
+                                record<TRACE>(tp, pkg, n_ev, 5 /*UNINTERACTED*/, j - mp.cav, k, 0);
+                                if (TRACE) tp.n_events[pkg] = n_ev;
+                                fly = false; uninter = true;
+                            } else {
+                                const float tauE = -log1pf(-uniform24(xw[2]) * Pint);  // Eq. 10
+                                ev_absorb = !(uniform24(xw[3]) < s_omega[k]);
+                                col = tauE / kext;
+                            }
+                        }
+                    } else {
+                        // L85/L87; R7 tie -> absorption; R15 one column instead of two clocks
+                        const float4 bt = s_bin[k];
+                        const float cA_ = tauA * bt.x, cS_ = tauS * bt.y;
+                        ev_absorb = (cA_ <= cS_);
+                        col = fminf(cA_, cS_);
+                    }
+                    // ---- next flight: from shell j towards its inner (s < 0) or outer surface
+                    s = re * mu;
+                    b2 = (atsrc && !point) ? b2src : re2 * (1.f - mu) * (1.f + mu);
+                    pa = tab0 + 8u * (unsigned)((s < 0.f) ? -j : j + 1);
+                }
+                // ---- write the package back; flying packages join the ready queue, a slot whose package ended
+                //      without escaping through the sentinel (FFI, tau0 = 0) is free again; a slot that got no id dies
+                if (fly || uninter) {
+                    const unsigned nkf = uninter ? 0u
+                        : ((unsigned)k | (ev_absorb ? KF_EVABS : 0u) | (dry ? KF_DRY : 0u) | KF_OCC);
+                    pA[slot] = make_float4(s, b2, col, __uint_as_float(pa));
+                    pB[slot] = make_uint4((unsigned)id, (unsigned)(id >> 32), blk, nkf);
+                    if (!R.uniform_q) pQ[slot] = q;
+                    if (TRACE) { pT[slot] = pkg; pT[P + slot] = n_ev; pT[2 * P + slot] = (int)ncross; }
+                }
+                if (!R.uniform_q) {
+                    // raw units injected by the launches of this batch
+                    unsigned long long inj = launch ? q : 0ull;
+                    const unsigned lm = __ballot_sync(kFull, launch);
+                    if (lm) {
+#pragma unroll
+                        for (int o = 16; o > 0; o >>= 1) inj += __shfl_xor_sync(kFull, inj, o);
+                        if (lane == 0) atomicAdd(&s_cnt[LC_INJECTED_RAW], inj);
+                    }
+                }
+                const unsigned flym = __ballot_sync(kFull, fly);
+                if (fly) qR[nR + __popc(flym & lt_mask)] = (unsigned char)slot;
+                nR += __popc(flym);
+                const unsigned unm = __ballot_sync(kFull, uninter);
+                if (unm) {
+                    if (uninter) qL[nL + __popc(unm & lt_mask)] = (unsigned char)slot;
+                    nL += __popc(unm);
+                }
+                __syncwarp();
+            }
+            if (nR == 0) break;                      // every slot of the pool is dead: the ticket is drained
+
+            // =====================================================================================
+            // CROSSING phase (Eq. 4): no RNG, no global memory, no branches in the crossing itself.
             // One crossing: d = r_c^2 - b^2 (negative: the surface is not reached, the lane stops with col
             // untouched); along-ray coordinate of the surface sn = +-sqrt(d); col -= rho^ (sn - s) (Eq. 4) is
             // committed together with the passage, and the lane stops if col < 0: the event lies col / rho^
             // before the surface (R7: an event exactly on a surface is a passage).
-            const int thr = max(1, (__popc(__ballot_sync(kFull, has)) * R.thr_num) >> 5);
-            for (;;) {
+            // Flight state: along-ray coordinate s and impact parameter^2 b2 (units of R), remaining column col
+            // (units of 1/kappa_ref) to the next event, shared-memory address pa of the candidate surface passage
+            // (entry E); (pa - pa0) / 8 counts the passages since the package was taken from the pool.
+            // =====================================================================================
+            {
+                bool has = lane < nR;
+                unsigned slot = 0, pa = tab0;
+                float s = 0.f, b2 = 0.f, col = -1.f;
+                if (has) {
+                    slot = qR[nR - 1 - lane];
+                    const float4 a = pA[slot];
+                    s = a.x; b2 = a.y; col = a.z; pa = __float_as_uint(a.w);
+                }
+                nR -= min(nR, 32);
+                unsigned pa0 = pa;
+                float2 E = lds_entry(pa);
+                bool alive = has;
+                for (;;) {
 #pragma unroll
-                for (int u = 0; u < kUnroll; u++) {
-                    const float d = E.x - b2;
-                    alive = alive && (d >= 0.f);
-                    if (alive) {
-                        const float sn = __int_as_float(__float_as_int(sqrt_ftz(d)) | (__float_as_int(E.y) & 0x80000000));
-                        col = fmaf(-fabsf(E.y), sn - s, col);
-                        s = sn;
-                        pa += 8u;
-                        E = lds_entry(pa);
+                    for (int u = 0; u < kUnroll; u++) {
+                        const float d = E.x - b2;
+                        alive = alive && (d >= 0.f);
+                        if (alive) {
+                            const float sn = __int_as_float(__float_as_int(sqrt_ftz(d)) | (__float_as_int(E.y) & 0x80000000));
+                            col = fmaf(-fabsf(E.y), sn - s, col);
+                            s = sn;
+                            pa += 8u;
+                            E = lds_entry(pa);
+                        }
+                        alive = alive && (col >= 0.f);
                     }
-                    alive = alive && (col >= 0.f);
-                }
-                if (!alive && (col >= 0.f)) {
-                    if (__float_as_int(E.y) < 0) {
-                        // the inner surface is not reached (tangent shell): head for the outer one instead
-                        // entry c -> entry 1 - c; the 1 - 2c entries skipped are no passages
-                        const unsigned np = 2u * tab0 + 8u - pa;
-                        pa0 += np - pa;
-                        pa = np;
-                        E = lds_entry(pa);
-                        alive = true;
-                    } else if (pa != pa_out) {
-                        b2 = E.x;                                // outward, b2 > r^2 by rounding only: graze
-                        alive = true;
+                    if (!alive && (col >= 0.f)) {
+                        if (__float_as_int(E.y) < 0) {
+                            // the inner surface is not reached (tangent shell): head for the outer one instead
+                            // entry c -> entry 1 - c; the 1 - 2c entries skipped are no passages
+                            const unsigned np = 2u * tab0 + 8u - pa;
+                            pa0 += np - pa;
+                            pa = np;
+                            E = lds_entry(pa);
+                            alive = true;
+                        } else if (pa != pa_out) {
+                            b2 = E.x;                                // outward, b2 > r^2 by rounding only: graze
+                            alive = true;
+                        }
                     }
+                    const unsigned am = __ballot_sync(kFull, alive);
+                    const int n_alive = __popc(am);
+                    if (n_alive >= thr_hi) continue;
+                    const bool leave = (nR == 0);
+                    if (leave && n_alive >= thr_lo) continue;
+
+                    // ---- stopped packages (all of them when leaving) go back to the pool and into their queues
+                    const bool out = has && (leave || !alive);
+                    int t = -1;
+                    if (out) {
+                        const unsigned kf = pB[slot].w;
+                        const bool isev = !alive && (col < 0.f);         // the column ran out: scattering or absorption
+                        const unsigned n = ((pa - pa0) >> 3) - (isev ? 1u : 0u);
+                        if (kf & KF_DRY) lc_ffi += n;
+                        else { lc_cross += n; if (TRACE) pT[2 * P + slot] += (int)n; }
+                        pA[slot] = make_float4(s, b2, col, __uint_as_float(pa));
+                        // stopped on the sentinel: left the model (escape, or the end of a dry FFI flight)
+                        t = alive ? QT_READY : (isev ? ((kf & KF_EVABS) ? QT_ABS : QT_SCA) : QT_SRC);
+                    }
+                    {
+                        unsigned mk;
+                        mk = __ballot_sync(kFull, t == QT_ABS);
+                        if (t == QT_ABS) qA[nA + __popc(mk & lt_mask)] = (unsigned char)slot;
+                        nA += __popc(mk);
+                        mk = __ballot_sync(kFull, t == QT_SCA);
+                        if (t == QT_SCA) qS[nS + __popc(mk & lt_mask)] = (unsigned char)slot;
+                        nS += __popc(mk);
+                        mk = __ballot_sync(kFull, t == QT_SRC);
+                        if (t == QT_SRC) qL[nL + __popc(mk & lt_mask)] = (unsigned char)slot;
+                        nL += __popc(mk);
+                        if (leave) {
+                            mk = __ballot_sync(kFull, t == QT_READY);
+                            if (t == QT_READY) qR[nR + __popc(mk & lt_mask)] = (unsigned char)slot;
+                            nR += __popc(mk);
+                        }
+                    }
+                    __syncwarp();
+                    if (leave) break;
+                    // ---- idle lanes take the next ready packages
+                    const unsigned fm = ~am;
+                    const int r = __popc(fm & lt_mask);
+                    const bool take = !alive && (r < nR);
+                    if (take) {
+                        slot = qR[nR - 1 - r];
+                        const float4 a = pA[slot];
+                        s = a.x; b2 = a.y; col = a.z; pa = __float_as_uint(a.w);
+                        pa0 = pa;
+                        E = lds_entry(pa);
+                    } else if (!alive) {
+                        col = -1.f;                              // idle lane: never flies, never looks stopped short
+                    }
+                    has = alive || take;
+                    alive = has;
+                    nR -= min(nR, __popc(fm));
                 }
-                if (__popc(__ballot_sync(kFull, alive)) < thr) break;
             }
+            // counters: flush before a 32-bit count can wrap
+            if (__any_sync(kFull, ((lc_cross | lc_ffi | wc_pkg | wc_sca | wc_abs | wc_esc) >> 30) != 0u)) {
+                atomicAdd(&s_cnt[LC_CROSSINGS], (unsigned long long)lc_cross);
+                if (lc_ffi) atomicAdd(&s_cnt[LC_FFI_CROSSINGS], (unsigned long long)lc_ffi);
+                if (lane == 0) {
+                    atomicAdd(&s_cnt[LC_PACKAGES], (unsigned long long)wc_pkg);
+                    atomicAdd(&s_cnt[LC_SCATTERINGS], (unsigned long long)wc_sca);
+                    atomicAdd(&s_cnt[LC_ABSORPTIONS], (unsigned long long)wc_abs);
+                    atomicAdd(&s_cnt[LC_ESCAPED], (unsigned long long)wc_esc);
+                }
+                lc_cross = lc_ffi = wc_pkg = wc_sca = wc_abs = wc_esc = 0u;
+            }
+        }
+        // ---------------- per-ticket flush of the warp's counts (identical quanta: injected raw units = launches x quantum)
+        {
+            unsigned long long c = lc_cross, f = lc_ffi;
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) { c += __shfl_xor_sync(kFull, c, o); f += __shfl_xor_sync(kFull, f, o); }
+            if (lane == 0) {
+                atomicAdd(&s_cnt[LC_CROSSINGS], c);
+                if (f) atomicAdd(&s_cnt[LC_FFI_CROSSINGS], f);
+                atomicAdd(&s_cnt[LC_PACKAGES], (unsigned long long)wc_pkg);
+                atomicAdd(&s_cnt[LC_SCATTERINGS], (unsigned long long)wc_sca);
+                atomicAdd(&s_cnt[LC_ABSORPTIONS], (unsigned long long)wc_abs);
+                atomicAdd(&s_cnt[LC_ESCAPED], (unsigned long long)wc_esc);
+                if (R.uniform_q) atomicAdd(&s_cnt[LC_INJECTED_RAW], q_uni * (unsigned long long)wc_pkg);
+            }
+            lc_cross = lc_ffi = wc_pkg = wc_sca = wc_abs = wc_esc = 0u;
         }
 
         if (TRACE) break;
@@ -534,22 +734,7 @@ __global__ void __launch_bounds__(kBlock, kMinBlocks) dies_track(DeviceModel D, 
     }
 
     if (TRACE) return;
-    // ---------------- counters: one atomic per warp / per block (rare ones)
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) {
-        inj_raw += __shfl_xor_sync(kFull, inj_raw, o);
-        lc_cross += __shfl_xor_sync(kFull, lc_cross, o);
-        lc_ffi += __shfl_xor_sync(kFull, lc_ffi, o);
-    }
-    if (lane == 0) {
-        atomicAdd(&D.counters[LC_PACKAGES], wc_pkg);
-        atomicAdd(&D.counters[LC_CROSSINGS], lc_cross);
-        if (lc_ffi) atomicAdd(&D.counters[LC_FFI_CROSSINGS], lc_ffi);
-        atomicAdd(&D.counters[LC_SCATTERINGS], wc_sca);
-        atomicAdd(&D.counters[LC_ABSORPTIONS], wc_abs);
-        atomicAdd(&D.counters[LC_ESCAPED], wc_esc);
-        atomicAdd(&D.counters[LC_INJECTED_RAW], inj_raw);
-    }
+    // ---------------- counters: one atomic per block and counter
     __syncthreads();
     if (tid < LC_N && s_cnt[tid]) atomicAdd(&D.counters[tid], s_cnt[tid]);
 }

@@ -187,7 +187,8 @@ def _T_outliers(To, Tg):
     se = np.sqrt(To.var(0, ddof=1) / len(To) + Tg.var(0, ddof=1) / len(Tg))
     tol = np.maximum(0.01 * mo, 3 * se)
     bad = np.abs(mg - mo) > tol
-    return bad, (np.nonzero(bad)[0], (mg / mo)[bad], (np.abs(mg - mo) / se)[bad])
+    with np.errstate(divide="ignore", invalid="ignore"):
+        return bad, (np.nonzero(bad)[0], (mg / mo)[bad], (np.abs(mg - mo) / se)[bad])
 
 
 def _check_T_parity(orc, p, n, model_kw=None, **kw):
