@@ -32,7 +32,7 @@ extern "C" const char* dies_last_error(void) { return g_err; }
 
 // ------------------------------------------------------------------ workspace layout
 struct Layout {
-    size_t emis, eps, Tgrid, epsgrid, F, bintab, omega, dustin, rb, rho, mass, stab, cscale, srccdf, srcin, Lsrc, mp,
+    size_t emis, eps, Tgrid, epsgrid, F, guideF, guideS, bintab, omega, dustin, rb, rho, mass, stab, cscale, srccdf, srcin, Lsrc, mp,
         fixed_row, Tfix, A, esc, next_id, counters, ticket, T_out, Lesc_out, eunit, flags, epsref, total;
 };
 static size_t al(size_t x) { return (x + 255) & ~(size_t)255; }
@@ -47,6 +47,8 @@ static Layout make_layout(int N, int K, int nT, int M)
     L.Tgrid = take((size_t)nT * 8);
     L.epsgrid = take((size_t)nT * 4);
     L.F = take((size_t)nT * K * 4);
+    L.guideF = take((size_t)nT * kGuide * 2);
+    L.guideS = take((size_t)M * 2 * kGuide * 2);
     L.bintab = take((size_t)K * 16);
     L.omega = take((size_t)K * 4);
     L.dustin = take((size_t)3 * K * 8);
@@ -121,6 +123,19 @@ __global__ void k_build_tables(const double* __restrict__ emis, int nT, int K, d
         f[k] = (float)(c / tot);
     }
     f[K - 1] = 1.0f;
+}
+
+// guide tables of the cut-point sampler: guide[row][c] = smallest k with cdf[row][k] > c / kGuide
+__global__ void k_build_guide(const float* __restrict__ cdf, int n_rows, int K, unsigned short* __restrict__ guide)
+{
+    const int idx = blockIdx.x * blockDim.x + threadIdx.x;
+    if (idx >= n_rows * kGuide) return;
+    const int row = idx / kGuide, c = idx % kGuide;
+    const float u = (float)c / (float)kGuide;
+    const float* f = cdf + (size_t)row * K;
+    int lo = 0, hi = K - 1;               // cdf[K-1] = 1 > u
+    while (lo < hi) { const int mid = (lo + hi) >> 1; if (f[mid] > u) hi = mid; else lo = mid + 1; }
+    guide[idx] = (unsigned short)lo;
 }
 
 __global__ void k_build_epsgrid(const double* __restrict__ eps, int nT, float* __restrict__ grid, double* epsref,
@@ -423,7 +438,8 @@ extern "C" int dies_create_batch(int n_models, int n_shells, const double* r_bou
     DeviceModel& D = m->D;
     D.N = N; D.K = K; D.nT = nT; D.n_models = M; D.ldS = N + 1; D.ldT = 2 * (N + 1) + 2;
     D.bintab = wsp<float4>(m, L.bintab); D.omega = wsp<float>(m, L.omega); D.epsgrid = wsp<float>(m, L.epsgrid);
-    D.F = wsp<float>(m, L.F); D.stab = wsp<float2>(m, L.stab); D.cscale = wsp<double>(m, L.cscale);
+    D.F = wsp<float>(m, L.F); D.guideF = wsp<unsigned short>(m, L.guideF); D.guideS = wsp<unsigned short>(m, L.guideS);
+    D.stab = wsp<float2>(m, L.stab); D.cscale = wsp<double>(m, L.cscale);
     D.srccdf = wsp<float>(m, L.srccdf); D.mp = wsp<ModelParams>(m, L.mp); D.fixed_row = wsp<int>(m, L.fixed_row);
     D.A = wsp<unsigned long long>(m, L.A); D.esc = wsp<unsigned long long>(m, L.esc);
     D.next_id = wsp<unsigned long long>(m, L.next_id); D.counters = wsp<unsigned long long>(m, L.counters);
@@ -444,11 +460,12 @@ extern "C" int dies_create_batch(int n_models, int n_shells, const double* r_bou
     TRY_OR_FREE(cudaMemcpyAsync(m->ws + L.rho, rho, (size_t)M * N * 8, cudaMemcpyHostToDevice, 0));
     int* flags = wsp<int>(m, L.flags);
     k_build_tables<<<(nT + 127) / 128, 128>>>(wsp<double>(m, L.emis), nT, K, wsp<double>(m, L.eps), wsp<float>(m, L.F), flags);
+    k_build_guide<<<(nT * kGuide + 255) / 256, 256>>>(wsp<float>(m, L.F), nT, K, wsp<unsigned short>(m, L.guideF));
     k_build_epsgrid<<<(nT + 127) / 128, 128>>>(wsp<double>(m, L.eps), nT, wsp<float>(m, L.epsgrid), wsp<double>(m, L.epsref), flags);
     k_build_dust<<<(K + 127) / 128, 128>>>(wsp<double>(m, L.dustin), K, kref, wsp<float4>(m, L.bintab), wsp<float>(m, L.omega));
     k_build_shells<<<(M * (2 * N + 4) + 127) / 128, 128>>>(wsp<double>(m, L.rb), wsp<double>(m, L.rho), N, M, kref,
                                                        wsp<float2>(m, L.stab), wsp<double>(m, L.mass), wsp<ModelParams>(m, L.mp));
-    m->launches += 4;
+    m->launches += 5;
     int hflags[2] = {0, 0};
     TRY_OR_FREE(cudaMemcpy(hflags, flags, sizeof(hflags), cudaMemcpyDeviceToHost));
     TRY_OR_FREE(cudaGetLastError());
@@ -522,7 +539,9 @@ extern "C" int dies_set_sources_batch(dies_model* m, const double* ext, const do
     CUDA_TRY(cudaMemcpy(m->ws + m->L.mp, mp.data(), (size_t)M * sizeof(ModelParams), cudaMemcpyHostToDevice));
     k_build_sources<<<(2 * M + 127) / 128, 128>>>(wsp<double>(m, m->L.srcin), wsp<double>(m, m->L.rb), N, K, M,
                                                   wsp<float>(m, m->L.srccdf), wsp<double>(m, m->L.Lsrc));
-    m->launches += 1;
+    k_build_guide<<<(2 * M * kGuide + 255) / 256, 256>>>(wsp<float>(m, m->L.srccdf), 2 * M, K,
+                                                        wsp<unsigned short>(m, m->L.guideS));
+    m->launches += 2;
     CUDA_TRY(cudaMemcpy(Ls.data(), m->ws + m->L.Lsrc, Ls.size() * 8, cudaMemcpyDeviceToHost));
     CUDA_TRY(cudaGetLastError());
     for (int i = 0; i < M; i++) m->L_ext[i] = m->has_ext[i] ? Ls[2 * i] : 0.0;
@@ -574,8 +593,8 @@ static int fill_run_params(dies_model* m, uint64_t n_packages, uint64_t seed, co
     R->uniform_q = (d.k_bg == 0.5 && !d.ffi && !two) ? 1 : 0;
     R->qscale = (float)(1u << d.fixed_shift);
     R->pool = m->pool;
-    R->thr_hi = env_int("DIES_THR_HI", 1, 32, 24);
-    R->thr_lo = env_int("DIES_THR_LO", 1, 32, 12);
+    R->thr_hi = env_int("DIES_THR_HI", 1, 32, 20);
+    R->thr_lo = env_int("DIES_THR_LO", 1, 32, 16);
     R->min_ready = env_int("DIES_MIN_READY", 1, kMaxPool, 32);
     R->n_tickets = 0; R->parts = 1;
     return DIES_OK;

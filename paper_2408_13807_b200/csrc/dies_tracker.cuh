@@ -29,6 +29,7 @@ constexpr unsigned kFull = 0xffffffffu;
 constexpr unsigned kChunk = 128;     // package ids a warp takes from the global counter at a time
 constexpr int kUnroll = 4;           // crossings per vote in the crossing loop
 constexpr int kMaxPool = 248;        // pool slots per warp (queue entries are bytes)
+constexpr int kGuide = 256;          // cut-points per CDF row of the guide tables
 
 // event counters (same order as DIES_C_* in include/dies.h), accumulated per block in shared memory
 enum { LC_PACKAGES = 0, LC_CROSSINGS, LC_FFI_CROSSINGS, LC_SCATTERINGS, LC_ABSORPTIONS, LC_ESCAPED, LC_UNINTERACTED,
@@ -62,6 +63,8 @@ struct DeviceModel {
     const float* omega;              // K: albedo
     const float* epsgrid;            // nT: eps_t / eps_ref
     const float* F;                  // nT x K row CDFs of the re-emission spectra
+    const unsigned short* guideF;    // nT x kGuide: smallest k with F[t][k] > c / kGuide
+    const unsigned short* guideS;    // n_models x 2 x kGuide: the same for the source CDFs
     const float2* stab;              // n_models x ldT unfolded shell table
     const double* cscale;            // n_models x ldS: eps^ per raw tally unit
     const float* srccdf;             // n_models x 2 x K: external, point
@@ -131,19 +134,32 @@ __device__ __forceinline__ void philox4x32_10(uint32_t k0, uint32_t k1, uint32_t
 {
 #pragma unroll
     for (int r = 0; r < 10; r++) {
-        const uint32_t hi0 = __umulhi(0xD2511F53u, c0), lo0 = 0xD2511F53u * c0;
-        const uint32_t hi1 = __umulhi(0xCD9E8D57u, c2), lo1 = 0xCD9E8D57u * c2;
-        c0 = hi1 ^ c1 ^ k0;
-        c1 = lo1;
-        c2 = hi0 ^ c3 ^ k1;
-        c3 = lo0;
+        const unsigned long long p0 = (unsigned long long)0xD2511F53u * c0;   // one IMAD.WIDE gives both halves
+        const unsigned long long p1 = (unsigned long long)0xCD9E8D57u * c2;
+        c0 = (uint32_t)(p1 >> 32) ^ c1 ^ k0;
+        c1 = (uint32_t)p1;
+        c2 = (uint32_t)(p0 >> 32) ^ c3 ^ k1;
+        c3 = (uint32_t)p0;
         k0 += 0x9E3779B9u;
         k1 += 0xBB67AE85u;
     }
     out[0] = c0; out[1] = c1; out[2] = c2; out[3] = c3;
 }
 
-__device__ __forceinline__ float uniform24(uint32_t x) { return (__uint2float_rn(x >> 9) + 0.5f) * 1.1920928955078125e-07f; }
+// u = ((x >> 9) + 0.5) 2^-23 (R1) without an integer-to-float conversion: 1.m - (1 - 2^-24) is exact
+__device__ __forceinline__ float uniform24(uint32_t x)
+{
+    return __uint_as_float(0x3f800000u | (x >> 9)) - 0.99999994039535522461f;
+}
+
+// -ln u for u in (0,1) through the hardware log2 (absolute error of lg2.approx <= 2^-22 on [0.5, 2), 2 ulp elsewhere:
+// <= 1.7e-7 in optical depth, the size of the fp32 rounding of the path itself; R14)
+__device__ __forceinline__ float neg_log(float u)
+{
+    float y;
+    asm("lg2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(u));
+    return y * -0.69314718055994530942f;
+}
 
 __device__ __forceinline__ float sqrt_ftz(float x)
 {
@@ -160,15 +176,13 @@ __device__ __forceinline__ float2 lds_entry(unsigned a)
     return v;
 }
 
-// smallest k in [0, n) with cdf[k] > u (= #{i < n-1 : cdf[i] <= u} for a non-decreasing cdf with cdf[n-1] > u):
-// binary lifting with a warp-uniform trip count (top = largest power of two <= n-1, 0 if n == 1)
-__device__ __forceinline__ int sample_cdf(const float* __restrict__ cdf, int n, int top, float u)
+// smallest k with cdf[k] > u for a non-decreasing cdf whose last entry exceeds every u (inverse-CDF sampling, R3),
+// by the cut-point method: guide[c] is the answer for u = c / kGuide, so the answer for u in [c, c+1) / kGuide is
+// found by walking up from it -- one or two table reads instead of a bisection over the whole row
+__device__ __forceinline__ int sample_cdf(const float* __restrict__ cdf, const unsigned short* __restrict__ guide, float u)
 {
-    int k = 0;
-    for (int step = top; step > 0; step >>= 1) {
-        const int t = k + step;
-        if (t < n && __ldg(cdf + t - 1) <= u) k = t;
-    }
+    int k = __ldg(guide + (int)(u * (float)kGuide));
+    while (__ldg(cdf + k) <= u) k++;
     return k;
 }
 
@@ -252,9 +266,6 @@ __global__ void __launch_bounds__(kBlock, kMinBlocks) dies_track(DeviceModel D, 
     unsigned char* const qR = qL + P;
     int* const pT = reinterpret_cast<int*>(smem_raw + sp.trace) + wid * 3 * P;      // TRACE only
 
-    int top = 0;                                     // largest power of two <= K-1 (trip count of sample_cdf)
-    for (int t = 1; t <= K - 1; t <<= 1) top = t;
-
     for (int x = tid; x < K; x += kBlock) { s_bin[x] = D.bintab[x]; s_omega[x] = D.omega[x]; }
     for (int x = tid; x < nT; x += kBlock) s_eps[x] = D.epsgrid[x];
     if (tid < LC_N) s_cnt[tid] = 0ull;
@@ -292,6 +303,7 @@ __global__ void __launch_bounds__(kBlock, kMinBlocks) dies_track(DeviceModel D, 
         unsigned long long* const gA = D.A + (size_t)m * ldS;
         unsigned long long* const g_next = TRACE ? tp.counter : D.next_id + m;
         const float* const g_src = D.srccdf + (size_t)m * 2 * K;
+        const unsigned short* const g_srcguide = D.guideS + (size_t)m * 2 * kGuide;
         const unsigned long long n_ids = TRACE ? (unsigned long long)tp.count
                                                : R.n_run * (unsigned long long)(mp.has_ext + mp.has_point);
         const unsigned tab0 = (unsigned)__cvta_generic_to_shared(s_tab) + 8u * (unsigned)ldS;   // address of entry c = 0
@@ -435,6 +447,7 @@ __global__ void __launch_bounds__(kBlock, kMinBlocks) dies_track(DeviceModel D, 
                     unsigned b = dryend ? 0u : blk;
                     philox4x32_10(R.key0, R.key1, (uint32_t)id, (uint32_t)(id >> 32), b, (uint32_t)m, xw);
                     const float* cdf = nullptr;      // table the new frequency bin is drawn from (launch, re-emission)
+                    const unsigned short* guide = nullptr;
                     if (isabs) {
                         int row;
                         if (MODE == 1) {
@@ -459,14 +472,16 @@ __global__ void __launch_bounds__(kBlock, kMinBlocks) dies_track(DeviceModel D, 
                             }
                         }
                         cdf = D.F + (size_t)row * K;
+                        guide = D.guideF + (size_t)row * kGuide;
                     } else if (launch) {
                         cdf = g_src + (point ? K : 0);                              // L55 source spectrum table
+                        guide = g_srcguide + (point ? kGuide : 0);
                     }
                     blk = (launch && R.ffi) ? 0u : b + 1u;
                     const float u0 = uniform24(xw[0]), u1 = uniform24(xw[1]);
-                    const float tauS = -logf(uniform24(xw[2]));      // Eq. 1
-                    const float tauA = -logf(uniform24(xw[3]));
-                    if (cdf) k = sample_cdf(cdf, K, top, u0);        // new frequency bin (launch: L55; re-emission: L87, R4)
+                    const float tauS = neg_log(uniform24(xw[2]));       // Eq. 1
+                    const float tauA = neg_log(uniform24(xw[3]));
+                    if (cdf) k = sample_cdf(cdf, guide, u0);          // new frequency bin (launch: L55; re-emission: L87, R4)
 
                     // ---- event site (radius re, re2 = re^2, shell j) and new direction cosine mu w.r.t. the radius
                     float re, re2, mu, b2src = 0.f;
@@ -605,16 +620,18 @@ __global__ void __launch_bounds__(kBlock, kMinBlocks) dies_track(DeviceModel D, 
                 float2 E = lds_entry(pa);
                 bool alive = has;
                 for (;;) {
+                    const unsigned pb = pa;                      // the table is walked from here with constant offsets
 #pragma unroll
                     for (int u = 0; u < kUnroll; u++) {
                         const float d = E.x - b2;
                         alive = alive && (d >= 0.f);
                         if (alive) {
-                            const float sn = __int_as_float(__float_as_int(sqrt_ftz(d)) | (__float_as_int(E.y) & 0x80000000));
-                            col = fmaf(-fabsf(E.y), sn - s, col);
-                            s = sn;
-                            pa += 8u;
-                            E = lds_entry(pa);
+                            // col -= rho^ (sn - s) as (col + rho^ s) - rho^ sn: the first half does not wait for the sqrt
+                            const float t = fmaf(fabsf(E.y), s, col);
+                            s = __int_as_float(__float_as_int(sqrt_ftz(d)) | (__float_as_int(E.y) & 0x80000000));
+                            col = fmaf(-fabsf(E.y), s, t);
+                            E = lds_entry(pb + 8u * (u + 1));
+                            pa = pb + 8u * (u + 1);
                         }
                         alive = alive && (col >= 0.f);
                     }
@@ -652,21 +669,13 @@ __global__ void __launch_bounds__(kBlock, kMinBlocks) dies_track(DeviceModel D, 
                         t = alive ? QT_READY : (isev ? ((kf & KF_EVABS) ? QT_ABS : QT_SCA) : QT_SRC);
                     }
                     {
-                        unsigned mk;
-                        mk = __ballot_sync(kFull, t == QT_ABS);
-                        if (t == QT_ABS) qA[nA + __popc(mk & lt_mask)] = (unsigned char)slot;
-                        nA += __popc(mk);
-                        mk = __ballot_sync(kFull, t == QT_SCA);
-                        if (t == QT_SCA) qS[nS + __popc(mk & lt_mask)] = (unsigned char)slot;
-                        nS += __popc(mk);
-                        mk = __ballot_sync(kFull, t == QT_SRC);
-                        if (t == QT_SRC) qL[nL + __popc(mk & lt_mask)] = (unsigned char)slot;
-                        nL += __popc(mk);
-                        if (leave) {
-                            mk = __ballot_sync(kFull, t == QT_READY);
-                            if (t == QT_READY) qR[nR + __popc(mk & lt_mask)] = (unsigned char)slot;
-                            nR += __popc(mk);
-                        }
+                        // one store per leaving package: queue t at position (length of t) + (rank among the lanes of t)
+                        const unsigned mA = __ballot_sync(kFull, t == QT_ABS), mS = __ballot_sync(kFull, t == QT_SCA);
+                        const unsigned mL = __ballot_sync(kFull, t == QT_SRC), mR = __ballot_sync(kFull, t == QT_READY);
+                        const unsigned mine = t == QT_ABS ? mA : t == QT_SCA ? mS : t == QT_SRC ? mL : mR;
+                        const int base = t == QT_ABS ? nA : t == QT_SCA ? P + nS : t == QT_SRC ? 2 * P + nL : 3 * P + nR;
+                        if (out) qA[base + __popc(mine & lt_mask)] = (unsigned char)slot;
+                        nA += __popc(mA); nS += __popc(mS); nL += __popc(mL); nR += __popc(mR);
                     }
                     __syncwarp();
                     if (leave) break;
