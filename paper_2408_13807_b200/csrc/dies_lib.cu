@@ -589,6 +589,7 @@ static int fill_run_params(dies_model* m, uint64_t n_packages, uint64_t seed, co
     for (int i = 0; i < m->M; i++) two |= (m->has_ext[i] && m->has_point[i]);
     R->n_run = n_packages; R->n_total = d.n_total; R->id_base = 0;
     R->key0 = (uint32_t)seed; R->key1 = (uint32_t)(seed >> 32);
+    for (int r = 0; r < 10; r++) { R->rk[2 * r] = R->key0 + (uint32_t)r * 0x9E3779B9u; R->rk[2 * r + 1] = R->key1 + (uint32_t)r * 0xBB67AE85u; }
     R->k_bg = (float)d.k_bg; R->ffi = d.ffi ? 1 : 0;
     R->uniform_q = (d.k_bg == 0.5 && !d.ffi && !two) ? 1 : 0;
     R->qscale = (float)(1u << d.fixed_shift);

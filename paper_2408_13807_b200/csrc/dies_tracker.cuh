@@ -27,7 +27,7 @@ constexpr int kWarps = kBlock / 32;
 constexpr int kMinBlocks = 4;        // resident blocks per SM asked from the compiler (64 registers)
 constexpr unsigned kFull = 0xffffffffu;
 constexpr unsigned kChunk = 128;     // package ids a warp takes from the global counter at a time
-constexpr int kUnroll = 4;           // crossings per vote in the crossing loop
+constexpr int kUnroll = 12;           // crossings per vote in the crossing loop
 constexpr int kMaxPool = 248;        // pool slots per warp (queue entries are bytes)
 constexpr int kGuide = 256;          // cut-points per CDF row of the guide tables
 
@@ -77,32 +77,6 @@ struct DeviceModel {
     unsigned int* ticket;            // 1
 };
 
-struct RunParams {
-    unsigned long long n_run;        // packages per source in this call
-    unsigned long long id_base;      // packages per source done by earlier calls (accumulate)
-    unsigned long long n_total;      // packages per source over the whole run
-    uint32_t key0, key1;
-    float k_bg;
-    int ffi;
-    int uniform_q;                   // all packages carry the same raw quantum (no k_bg, no FFI, one source)
-    float qscale;                    // 2^S
-    int n_tickets, parts;            // tickets = n_models * parts
-    int pool;                        // P: pool slots per warp (multiple of 8, 32 <= P <= kMaxPool)
-    int thr_hi;                      // crossing phase: swap stopped lanes for ready packages when fewer fly
-    int thr_lo;                      // crossing phase: with no ready package left, leave when fewer fly
-    int min_ready;                   // event phase: mixed batches only while fewer packages are ready
-};
-
-struct TraceParams {
-    int model;
-    unsigned long long first_id;     // global package id of the first traced package
-    int count;
-    int32_t* events;                 // count x max_events x 4
-    int max_events;
-    int32_t* n_events;               // count
-    unsigned long long* counter;     // zeroed: next traced package
-};
-
 // shared-memory plan of a block (byte offsets), used by the kernel and by the host to size the launch
 struct SmemPlan { unsigned bin, cs, tab, eps, omega, row, esc, A, poolA, poolB, poolQ, queues, trace, total; };
 __host__ __device__ inline SmemPlan plan_smem(int K, int nT, int ldS, int ldT, int P, bool trace)
@@ -128,7 +102,49 @@ __host__ __device__ inline SmemPlan plan_smem(int K, int nT, int ldS, int ldT, i
     return p;
 }
 
+struct RunParams {
+    unsigned long long n_run;        // packages per source in this call
+    unsigned long long id_base;      // packages per source done by earlier calls (accumulate)
+    unsigned long long n_total;      // packages per source over the whole run
+    uint32_t key0, key1;
+    uint32_t rk[20];                 // Philox round keys: rk[2r] = key0 + r 0x9E3779B9, rk[2r+1] = key1 + r 0xBB67AE85
+    float k_bg;
+    int ffi;
+    int uniform_q;                   // all packages carry the same raw quantum (no k_bg, no FFI, one source)
+    float qscale;                    // 2^S
+    int n_tickets, parts;            // tickets = n_models * parts
+    int pool;                        // P: pool slots per warp (multiple of 8, 32 <= P <= kMaxPool)
+    int thr_hi;                      // crossing phase: swap stopped lanes for ready packages when fewer fly
+    int thr_lo;                      // crossing phase: with no ready package left, leave when fewer fly
+    int min_ready;                   // event phase: mixed batches only while fewer packages are ready
+};
+
+struct TraceParams {
+    int model;
+    unsigned long long first_id;     // global package id of the first traced package
+    int count;
+    int32_t* events;                 // count x max_events x 4
+    int max_events;
+    int32_t* n_events;               // count
+    unsigned long long* counter;     // zeroed: next traced package
+};
+
 // ------------------------------------------------------------------ RNG contract (include/dies.h)
+__device__ __forceinline__ void philox4x32_10_rk(const uint32_t (&rk)[20], uint32_t c0, uint32_t c1, uint32_t c2,
+                                                 uint32_t c3, uint32_t out[4])
+{
+#pragma unroll
+    for (int r = 0; r < 10; r++) {
+        const unsigned long long p0 = (unsigned long long)0xD2511F53u * c0;
+        const unsigned long long p1 = (unsigned long long)0xCD9E8D57u * c2;
+        c0 = (uint32_t)(p1 >> 32) ^ c1 ^ rk[2 * r];
+        c1 = (uint32_t)p1;
+        c2 = (uint32_t)(p0 >> 32) ^ c3 ^ rk[2 * r + 1];
+        c3 = (uint32_t)p0;
+    }
+    out[0] = c0; out[1] = c1; out[2] = c2; out[3] = c3;
+}
+
 __device__ __forceinline__ void philox4x32_10(uint32_t k0, uint32_t k1, uint32_t c0, uint32_t c1, uint32_t c2,
                                               uint32_t c3, uint32_t out[4])
 {
@@ -445,7 +461,7 @@ __global__ void __launch_bounds__(kBlock, kMinBlocks) dies_track(DeviceModel D, 
                     const bool point = atsrc && (mp.has_ext ? ((id - R.id_base) >= R.n_total) : true);
                     // block 0 belongs to the launch; with FFI the end of the dry flight draws it again
                     unsigned b = dryend ? 0u : blk;
-                    philox4x32_10(R.key0, R.key1, (uint32_t)id, (uint32_t)(id >> 32), b, (uint32_t)m, xw);
+                    philox4x32_10_rk(R.rk, (uint32_t)id, (uint32_t)(id >> 32), b, (uint32_t)m, xw);
                     const float* cdf = nullptr;      // table the new frequency bin is drawn from (launch, re-emission)
                     const unsigned short* guide = nullptr;
                     if (isabs) {
@@ -468,7 +484,7 @@ __global__ void __launch_bounds__(kBlock, kMinBlocks) dies_track(DeviceModel D, 
                                 row = row_from(s_eps, nT, row, es);
                                 atomicAdd(&s_cnt[LC_EXTRA_BLOCKS], 1ull);
                                 b++;
-                                philox4x32_10(R.key0, R.key1, (uint32_t)id, (uint32_t)(id >> 32), b, (uint32_t)m, xw);
+                                philox4x32_10_rk(R.rk, (uint32_t)id, (uint32_t)(id >> 32), b, (uint32_t)m, xw);
                             }
                         }
                         cdf = D.F + (size_t)row * K;
