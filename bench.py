@@ -26,11 +26,15 @@ ROOT = os.path.dirname(os.path.abspath(__file__))
 if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
 
-from paper_2408_13807_b200 import synth  # noqa: E402
+from paper_2408_13807_b200 import sharding, synth  # noqa: E402
 
-# Algorithmic thread-instructions per unit of work, read from the SASS of the shipped tracker kernel
-# (straight-line path of each unit, profiles/ and DESIGN.md "Roofline"): crossing, scattering, absorption, package.
-INSTR = dict(crossing=24, scattering=230, absorption=330, package=210)
+# Algorithmic thread-instructions per unit of work in the shipped tracker (profiles/r1g_units.md):
+# crossing = SASS instructions of one predicated crossing step; scattering / absorption / package = predicated-on
+# thread-instructions executed on the unit's own source lines (shared event stream + its own branch) per unit,
+# from the ncu source page of the same workload.  Queue handling, swaps, votes, fix-ups and idle lanes are NOT work.
+INSTR = dict(crossing=9, scattering=298, absorption=329, package=268)
+# dram__bytes_read.sum + dram__bytes_write.sum of one dies_track launch (ncu --set full, profiles/r1g_ncu_full.md)
+TRAFFIC_BYTES_PER_LAUNCH = 314112
 SM_COUNT, SCHEDULERS, LANES = 148, 4, 32
 
 
@@ -125,7 +129,8 @@ def run_reference(args, rank, world):
     if rank != 0:
         return
     p = make_problem(args.workload, args.packages)
-    n_sample = min(p.n_packages, args.ref_sample)
+    # bounded sample per step: the whole --steps K run follows about --ref-total packages (tens of seconds of CPU)
+    n_sample = min(p.n_packages, args.ref_sample, max(2000, args.ref_total // max(args.steps, 1)))
     for _ in range(args.warmup):
         oracle_rate(p, max(1, n_sample // 10))
     times, cross = [], 0
@@ -170,7 +175,7 @@ def run_ours(args, rank, world, local_rank):
         torch.cuda.synchronize(dev)
 
     for w in range(args.warmup):
-        m.dies_run(n, seed=1000 + w + 7919 * rank, **opts)
+        m.dies_run(n, seed=sharding.replica_seed(1000, w, rank), **opts)
     torch.cuda.synchronize(dev)
     c0 = m.dies_get_counters()
 
@@ -184,7 +189,7 @@ def run_ours(args, rank, world, local_rank):
     for s in range(args.steps):
         flush.fill_(s & 0xFF)
         ev[s][0].record(stream)
-        m.dies_run(n, seed=1 + s + 7919 * rank, **opts)
+        m.dies_run(n, seed=sharding.replica_seed(1, s, rank), **opts)
         ev[s][1].record(stream)
     barrier()
     t_wall = time.perf_counter() - t_wall
@@ -195,10 +200,7 @@ def run_ours(args, rank, world, local_rank):
     for k in tot_counts:
         tot_counts[k] = c1[k]
     step_ms = float(np.sum(ms)) / args.steps
-    t = torch.tensor([float(np.sum(ms))], dtype=torch.float64, device=dev)
-    if world > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    total_ms = float(t.item())
+    total_ms = sharding.max_over_ranks(float(np.sum(ms)), dev)
     value = world * n * args.steps / (total_ms * 1e-3)
     crossings_per_s = world * c1["crossings"] * args.steps / (total_ms * 1e-3)
 
@@ -219,6 +221,12 @@ def run_ours(args, rank, world, local_rank):
 
     if rank != 0:
         return
+    # the atomic side of the roofline: the absorption step's returning 64-bit atomicAdd pattern alone on n_shells
+    # tallies (merged per warp when all quanta are equal, as in this run), measured on this GPU outside the timed region
+    uniform_q = (p.k_bg == 0.5 and not p.ffi and not (p.ext_bin_intensity is not None and p.L_point > 0))
+    raw_abs, _, _ = m.dies_get_absorbed()                     # per-shell absorption histogram of the last step
+    atom = dies.dies_bench_atomics(p.n_shells, weights=np.asarray(raw_abs, dtype=np.float64).reshape(-1),
+                                   aggregate=1 if uniform_q else 0)
     sm_max, peak_src = load_peaks()
     peak = SM_COUNT * SCHEDULERS * LANES * sm_max * 1e6 / 1e12          # thread-instructions/s, 1e12
     work = (c1["crossings"] * INSTR["crossing"] + c1["scatterings"] * INSTR["scattering"] +
@@ -240,7 +248,12 @@ def run_ours(args, rank, world, local_rank):
                          ms_per_step=1e3 * float(np.median(e2e_t))),
                 gpu_launches=int(2 * args.steps),
                 roofline=dict(bound="alu", achieved=achieved, peak=peak, unit="Tinstr/s", frac=achieved / peak,
-                              frac_at_held_clock=achieved / (peak * held / sm_max), traffic=None,
+                              frac_at_held_clock=achieved / (peak * held / sm_max), traffic=TRAFFIC_BYTES_PER_LAUNCH,
+                              atomic=dict(absorptions_per_s=c1["absorptions"] / (step_ms * 1e-3),
+                                          peak_absorptions_per_s=atom["lane_ops_per_s"],
+                                          peak_atomic_instr_per_s=atom["atomics_per_s"],
+                                          frac=c1["absorptions"] / (step_ms * 1e-3) / atom["lane_ops_per_s"],
+                                          peak_source=f"dies_bench_atomics({p.n_shells} tallies, the run's shell histogram, warp-merged={int(uniform_q)}) on this GPU"),
                               peak_source=f"148 SMs x 4 schedulers x 32 lanes x {sm_max:.0f} MHz ({peak_src})",
                               instr_per_unit=INSTR, kernel="dies_track<0,false>", kernel_ms=step_ms),
                 wall_s=t_wall)
@@ -257,13 +270,14 @@ def run_ours(args, rank, world, local_rank):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--steps", type=int, default=200)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="config2")
     ap.add_argument("--packages", type=float, default=0)
     ap.add_argument("--cpu-sample", type=int, default=6_000_000)
     ap.add_argument("--ref-sample", type=int, default=1_000_000)
+    ap.add_argument("--ref-total", type=int, default=20_000_000)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
     rank = int(os.environ.get("RANK", "0"))

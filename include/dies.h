@@ -138,6 +138,15 @@ int dies_test_philox(uint64_t seed, uint64_t first_id, uint32_t block, uint32_t 
 /* Device tables as built (for table parity): eps n_T (double), F n_T x n_freq (float). Either may be NULL. */
 int dies_get_tables(dies_model*, double* eps, float* F);
 
+/* Measurement support (the atomic side of the roofline): throughput of the absorption
+ * step's memory operation alone -- every lane of every resident warp draws one of n_addr (<= 65535) 64-bit tallies,
+ * uniformly (weights == NULL) or with the probabilities weights[n_addr] (host, >= 0: the workload's per-shell
+ * absorption histogram); equal draws of a warp are merged when aggregate != 0 (as the tracker does when all quanta
+ * are equal), and one RETURNING 64-bit atomicAdd per distinct tally per warp is issued and consumed; iters rounds
+ * per lane.  lane_ops_per_s = absorptions/s this pattern sustains, atomics_per_s = atomic instructions/s issued. */
+int dies_bench_atomics(int n_addr, const double* weights, int aggregate, int iters, double* lane_ops_per_s,
+                       double* atomics_per_s);
+
 int dies_destroy(dies_model*);
 const char* dies_last_error(void);
 /* "sm_100a" build tag, number of SMs and resident blocks per SM of the tracker (for the bench log). */

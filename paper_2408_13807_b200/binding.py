@@ -24,7 +24,7 @@ EXPORTS = ("dies_workspace_bytes", "dies_create_model", "dies_create_batch", "di
            "dies_set_sources_batch", "dies_run", "dies_run_batch", "dies_get_temperature", "dies_get_escape_spectrum",
            "dies_set_fixed_temperature", "dies_get_absorbed", "dies_get_counters", "dies_trace_packages",
            "dies_trace_package", "dies_test_philox", "dies_get_tables", "dies_destroy", "dies_last_error",
-           "dies_device_info")
+           "dies_device_info", "dies_bench_atomics")
 
 
 class DiesError(RuntimeError):
@@ -74,6 +74,7 @@ def lib():
     L.dies_destroy.argtypes = [vp]
     L.dies_last_error.restype = C.c_char_p
     L.dies_device_info.argtypes = [C.POINTER(C.c_int)] * 3
+    L.dies_bench_atomics.argtypes = [C.c_int, _dp, C.c_int, C.c_int, _dp, _dp]
     _lib = L
     return L
 
@@ -101,6 +102,19 @@ def dies_device_info():
     a, b, c = C.c_int(), C.c_int(), C.c_int()
     _chk(lib().dies_device_info(C.byref(a), C.byref(b), C.byref(c)))
     return dict(n_sms=a.value, blocks_per_sm=b.value, threads_per_block=c.value)
+
+
+def dies_bench_atomics(n_addr, weights=None, aggregate=1, iters=2000):
+    """Absorptions/s and atomic instructions/s of the returning 64-bit atomicAdd pattern on n_addr tallies, drawn
+    uniformly or with the probabilities `weights` (the workload's per-shell absorption histogram)."""
+    a, b = C.c_double(), C.c_double()
+    w = None
+    if weights is not None:
+        wa = np.ascontiguousarray(weights, dtype=np.float64)
+        assert wa.size == n_addr
+        w = wa.ctypes.data_as(_dp)
+    _chk(lib().dies_bench_atomics(int(n_addr), w, int(aggregate), int(iters), C.byref(a), C.byref(b)))
+    return dict(lane_ops_per_s=a.value, atomics_per_s=b.value)
 
 
 def dies_test_philox(seed, first_id, block, model_index, n):

@@ -806,3 +806,92 @@ extern "C" int dies_test_philox(uint64_t seed, uint64_t first_id, uint32_t block
     if (e != cudaSuccess) return fail(DIES_ECUDA, "philox test: %s", cudaGetErrorString(e));
     return DIES_OK;
 }
+
+// ------------------------------------------------------------------ atomic-unit microbenchmark (measurement support)
+// The absorption step of the tracker as a stand-alone loop: every lane draws a shell (uniform over n_addr tallies,
+// 8 bytes apart like the tallies of a model), the warp aggregates equal shells with __match_any_sync when asked to,
+// and one lane per distinct shell issues a RETURNING 64-bit atomicAdd whose result every lane consumes.
+__global__ void k_bench_atomics(unsigned long long* tallies, int n_addr, const unsigned short* __restrict__ lut,
+                                int aggregate, int iters, unsigned long long* sink, unsigned long long* n_atomics)
+{
+    const unsigned lane = threadIdx.x & 31u;
+    const unsigned lt_mask = (1u << lane) - 1u;
+    uint32_t x = (blockIdx.x * blockDim.x + threadIdx.x) * 2654435761u + 12345u;
+    unsigned long long acc = 0, issued = 0;
+    for (int it = 0; it < iters; it++) {
+        x = x * 1664525u + 1013904223u;
+        // uniform over the tallies, or the workload's shell histogram through a 4096-entry look-up table
+        const int j = lut ? (int)__ldg(lut + (x >> 20)) : (int)(((unsigned long long)(x >> 8) * (unsigned)n_addr) >> 24);
+        unsigned long long old;
+        if (aggregate) {
+            const unsigned peers = __match_any_sync(0xffffffffu, j);
+            const int leader = __ffs(peers) - 1;
+            old = 0;
+            if ((int)lane == leader) { old = atomicAdd(&tallies[j], (unsigned long long)__popc(peers)); issued++; }
+            old = __shfl_sync(0xffffffffu, old, leader) + (unsigned long long)__popc(peers & lt_mask);
+        } else {
+            old = atomicAdd(&tallies[j], 1ull);
+            issued++;
+        }
+        acc += old;
+    }
+    if (acc == 0x123456789abcdefull) *sink = acc;       // keeps the returned values alive
+    for (int o = 16; o > 0; o >>= 1) issued += __shfl_xor_sync(0xffffffffu, issued, o);
+    if (lane == 0) atomicAdd(n_atomics, issued);
+}
+
+extern "C" int dies_bench_atomics(int n_addr, const double* weights, int aggregate, int iters, double* lane_ops_per_s,
+                                  double* atomics_per_s)
+{
+    if (n_addr < 1 || n_addr > 65535 || iters < 1 || !lane_ops_per_s || !atomics_per_s)
+        return fail(DIES_EINVAL, "bad arguments");
+    // look-up table of the histogram: entry e holds the tally whose cumulative weight covers (e + 0.5) / 4096
+    std::vector<unsigned short> lut;
+    if (weights) {
+        double tot = 0.0;
+        for (int i = 0; i < n_addr; i++) { if (!(weights[i] >= 0.0)) return fail(DIES_EINVAL, "negative weight"); tot += weights[i]; }
+        if (!(tot > 0.0)) return fail(DIES_EINVAL, "weights sum to zero");
+        lut.resize(4096);
+        double c = 0.0; int i = 0;
+        for (int e = 0; e < 4096; e++) {
+            const double u = (e + 0.5) / 4096.0 * tot;
+            while (i < n_addr - 1 && c + weights[i] <= u) c += weights[i++];
+            lut[e] = (unsigned short)i;
+        }
+    }
+    int rc = check_device();
+    if (rc) return rc;
+    int dev = 0, sms = 0;
+    CUDA_TRY(cudaGetDevice(&dev));
+    CUDA_TRY(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+    unsigned long long* buf = nullptr;
+    CUDA_TRY(cudaMalloc(&buf, ((size_t)n_addr + 2) * 8 + 4096 * 2));
+    unsigned short* d_lut = nullptr;
+    if (weights) {
+        d_lut = reinterpret_cast<unsigned short*>(buf + n_addr + 2);
+        if (cudaMemcpy(d_lut, lut.data(), 4096 * 2, cudaMemcpyHostToDevice) != cudaSuccess) { cudaFree(buf); return fail(DIES_ECUDA, "copy failed"); }
+    }
+    cudaEvent_t e0, e1;
+    cudaEventCreate(&e0); cudaEventCreate(&e1);
+    const int grid = sms * 4, block = 256;
+    float best = 1e30f;
+    unsigned long long issued = 0;
+    cudaError_t e = cudaSuccess;
+    for (int rep = 0; rep < 4 && e == cudaSuccess; rep++) {          // first repetition warms up
+        cudaMemset(buf, 0, ((size_t)n_addr + 2) * 8);
+        cudaEventRecord(e0);
+        k_bench_atomics<<<grid, block>>>(buf, n_addr, d_lut, aggregate, iters, buf + n_addr, buf + n_addr + 1);
+        cudaEventRecord(e1);
+        e = cudaEventSynchronize(e1);
+        float ms = 0.f;
+        cudaEventElapsedTime(&ms, e0, e1);
+        if (rep > 0 && ms < best) best = ms;
+        if (e == cudaSuccess) e = cudaMemcpy(&issued, buf + n_addr + 1, 8, cudaMemcpyDeviceToHost);
+    }
+    cudaEventDestroy(e0); cudaEventDestroy(e1);
+    cudaFree(buf);
+    if (e != cudaSuccess) return fail(DIES_ECUDA, "atomic benchmark: %s", cudaGetErrorString(e));
+    *lane_ops_per_s = (double)grid * block * iters / (best * 1e-3);
+    *atomics_per_s = (double)issued / (best * 1e-3);
+    return DIES_OK;
+}

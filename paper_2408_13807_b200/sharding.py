@@ -1,0 +1,59 @@
+"""Host-side plan of the multi-GPU runs; no arithmetic of the method lives here.
+
+One process per GPU.  What shards, and how:
+  * full IRE on one model couples all packages through the cell energies: it does NOT shard.
+    `bench.py --gpus N` runs N independent replicas, each with its own seed (`replica_seed`);
+  * fixed-temperature tracking: packages are independent, so the package ids [0, n) are cut into contiguous
+    ranges (`package_range`), each rank follows its range with `dies_run(..., n_total=n, accumulate)` semantics
+    (ids continue, energies are L / n_total), and the 64-bit integer tallies are summed with one all-reduce
+    (`allreduce_tallies`): integer sums are order independent, so the result is bit-identical to one GPU;
+  * config 5 (independent spheres): models are dealt to ranks (`model_range`), no collective at all.
+"""
+from __future__ import annotations
+
+import torch
+import torch.distributed as dist
+
+
+def replica_seed(base_seed: int, step: int, rank: int) -> int:
+    """Seed of replica `rank` at step `step`: distinct Philox keys for every (rank, step)."""
+    return int(base_seed) + int(step) + 7919 * int(rank)
+
+
+def package_range(n_packages: int, rank: int, world: int) -> tuple[int, int]:
+    """Contiguous range [first, first + count) of package ids of rank `rank`; ranges tile [0, n) exactly and
+    differ in length by at most one."""
+    if not (0 <= rank < world):
+        raise ValueError("rank out of range")
+    q, r = divmod(int(n_packages), int(world))
+    first = rank * q + min(rank, r)
+    return first, q + (1 if rank < r else 0)
+
+
+def model_range(n_models: int, rank: int, world: int) -> tuple[int, int]:
+    """Contiguous range of model indices of rank `rank` (config 5: independent spheres, no exchange)."""
+    return package_range(n_models, rank, world)
+
+
+def allreduce_tallies(*tallies: torch.Tensor) -> list[torch.Tensor]:
+    """Sum int64 tally arrays (absorbed raw units per shell, escaped raw units per bin, counters) over all ranks
+    with ONE all-reduce.  The tensors live where the backend wants them (CUDA for nccl, CPU for gloo)."""
+    for t in tallies:
+        if t.dtype != torch.int64:
+            raise TypeError("tallies are 64-bit integers (fixed point): the sum over ranks must be exact")
+    flat = torch.cat([t.reshape(-1) for t in tallies])
+    if dist.is_available() and dist.is_initialized() and dist.get_world_size() > 1:
+        dist.all_reduce(flat, op=dist.ReduceOp.SUM)
+    out, o = [], 0
+    for t in tallies:
+        out.append(flat[o:o + t.numel()].reshape(t.shape))
+        o += t.numel()
+    return out
+
+
+def max_over_ranks(ms: float, device) -> float:
+    """Device time of a multi-rank step = the slowest rank's."""
+    t = torch.tensor([float(ms)], dtype=torch.float64, device=device)
+    if dist.is_available() and dist.is_initialized() and dist.get_world_size() > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())

@@ -1,0 +1,89 @@
+"""The N > 1 path on CPU: world_size 2 over gloo.
+
+Fixed-temperature tracking shards package-id ranges; the integer tallies summed with one all-reduce must equal the
+single-process tallies exactly.  The compute of each rank is played by the oracle here (tests may use it; there is
+no GPU in this container): with unit weights every absorption adds exactly one package energy, so the per-shell
+tallies are integers."""
+import os
+import socket
+import sys
+
+import numpy as np
+import pytest
+import torch
+import torch.distributed as dist
+import torch.multiprocessing as mp
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+from paper_2408_13807_b200 import sharding, synth  # noqa: E402
+
+N_PKG = 6001          # odd on purpose: ragged split
+SEED = 5
+
+
+def _counts(orc, p, first, count):
+    o = orc.Oracle(p)
+    o.set_fixed_temperature(np.linspace(10.0, 20.0, p.n_shells))
+    o.run(N_PKG, seed=SEED, mode=1, first_id=first, n_run=count)
+    e_pkg = o.sums["injected"] / max(count, 1)
+    a = np.rint(o.absorbed / e_pkg).astype(np.int64)
+    assert np.allclose(a * e_pkg, o.absorbed, rtol=1e-9, atol=0)
+    esc = np.rint(o.escaped / e_pkg).astype(np.int64)
+    c = o.counters
+    return a, esc, np.array([c["packages"], c["crossings"], c["scatterings"], c["absorptions"]], dtype=np.int64)
+
+
+def _worker(rank, world, port, out):
+    os.environ["MASTER_ADDR"] = "127.0.0.1"
+    os.environ["MASTER_PORT"] = str(port)
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    try:
+        from oracle import dies_oracle as orc
+        p = synth.config1()
+        first, count = sharding.package_range(N_PKG, rank, world)
+        a, esc, cnt = _counts(orc, p, first, count)
+        ta, te, tc = sharding.allreduce_tallies(torch.from_numpy(a), torch.from_numpy(esc), torch.from_numpy(cnt))
+        slow = sharding.max_over_ranks(10.0 + rank, "cpu")
+        if rank == 0:
+            np.savez(out, a=ta.numpy(), esc=te.numpy(), cnt=tc.numpy(), slow=slow)
+    finally:
+        dist.destroy_process_group()
+
+
+def _free_port():
+    with socket.socket() as s:
+        s.bind(("127.0.0.1", 0))
+        return s.getsockname()[1]
+
+
+def test_package_ranges_tile_exactly():
+    for n in (0, 1, 7, 6001, 10**7):
+        for world in (1, 2, 3, 8):
+            r = [sharding.package_range(n, k, world) for k in range(world)]
+            assert r[0][0] == 0 and sum(c for _, c in r) == n
+            assert all(r[k][0] + r[k][1] == r[k + 1][0] for k in range(world - 1))
+            assert max(c for _, c in r) - min(c for _, c in r) <= 1
+    with pytest.raises(ValueError):
+        sharding.package_range(10, 2, 2)
+    assert len({sharding.replica_seed(1, s, r) for s in range(50) for r in range(8)}) == 400
+
+
+def test_allreduce_refuses_floating_point_tallies():
+    with pytest.raises(TypeError):
+        sharding.allreduce_tallies(torch.zeros(4, dtype=torch.float64))
+
+
+def test_fixed_T_shards_sum_to_the_single_run(tmp_path):
+    from oracle import dies_oracle as orc
+    out = str(tmp_path / "sum.npz")
+    mp.spawn(_worker, args=(2, _free_port(), out), nprocs=2, join=True)
+    got = np.load(out)
+    a, esc, cnt = _counts(orc, synth.config1(), 0, N_PKG)
+    assert np.array_equal(got["a"], a)
+    assert np.array_equal(got["esc"], esc)
+    assert np.array_equal(got["cnt"], cnt)
+    assert got["cnt"][0] == N_PKG and a.sum() > 0
+    assert float(got["slow"]) == 11.0
