@@ -61,6 +61,8 @@ def make_problem(workload, packages):
         p = synth.config4()
     elif workload == "config4_noffi":
         p = synth.config4(ffi=0)
+    elif workload == "config5":
+        p = synth.config5()
     else:
         raise SystemExit(f"unknown workload {workload}")
     if packages:
@@ -117,9 +119,18 @@ class ClockSampler:
 def oracle_rate(p, n_sample, seed=1):
     """The oracle as it stands on one host core: packages/s and crossings/s on a bounded sample."""
     from oracle import dies_oracle as orc
+    if isinstance(p, synth.BatchProblem):
+        # a batch is sampled model by model (8 models, n_sample / 8 packages each)
+        tot_n, tot_c, tot_t = 0, {}, 0.0
+        for mi in range(min(8, p.n_models)):
+            r, cr, dt, c = oracle_rate(p.model(mi), max(1, n_sample // 8), seed)
+            tot_n += max(1, n_sample // 8); tot_t += dt
+            for k, v in c.items():
+                tot_c[k] = tot_c.get(k, 0) + v
+        return tot_n / tot_t, tot_c["crossings"] / tot_t, tot_t, tot_c
     o = orc.Oracle(p)
     t0 = time.perf_counter()
-    o.run(n_sample, seed=seed, k_bg=p.k_bg, ffi=p.ffi)
+    o.run(n_sample, seed=seed, k_bg=getattr(p, "k_bg", 0.5), ffi=getattr(p, "ffi", 0))
     dt = time.perf_counter() - t0
     c = o.counters
     return n_sample / dt, c["crossings"] / dt, dt, c
@@ -143,8 +154,8 @@ def run_reference(args, rank, world):
                 steps=args.steps, warmup=args.warmup, ms_per_step=1e3 * tot / args.steps, higher_is_better=True,
                 scaling="weak", vs_baseline=None, dtype="f64", data="synthetic",
                 crossings_per_s=cross / tot,
-                config=dict(workload=args.workload, n_shells=p.n_shells, n_freq=p.n_freq, n_T=p.n_T,
-                            packages_per_step=n_sample, mode="full IRE", note="serial CPU oracle on a bounded sample"),
+                config=dict(workload=args.workload, n_shells=int(p.rho.shape[-1]), n_freq=int(p.freq.size),
+                            n_T=int(p.T_grid.size), packages_per_step=n_sample, mode="full IRE", note="serial CPU oracle on a bounded sample"),
                 cpu_baseline=dict(value=value, unit="packages/s", cores=1, kind="oracle",
                                   sample=f"{n_sample} packages of {args.workload} per step, {args.steps} steps"),
                 e2e=dict(value=value, unit="packages/s", h2d_bytes_per_step=0, d2h_bytes_per_step=0),
@@ -162,9 +173,15 @@ def run_ours(args, rank, world, local_rank):
     if world > 1:
         dist.init_process_group("nccl", device_id=dev)
     p = make_problem(args.workload, args.packages)
-    n = p.n_packages
-    opts = dict(k_bg=p.k_bg, ffi=p.ffi)
-    m = dies.Model(p, device=str(dev))
+    batch = isinstance(p, synth.BatchProblem)
+    n_models = p.n_models if batch else 1
+    n_per_model = p.n_packages
+    n = n_per_model * n_models                              # packages per step on this rank
+    k_bg, ffi = getattr(p, "k_bg", 0.5), getattr(p, "ffi", 0)
+    n_shells, n_freq, n_T = int(p.rho.shape[-1]), int(p.freq.size), int(p.T_grid.size)
+    opts = dict(k_bg=k_bg, ffi=ffi)
+    make = (lambda: dies.Model(batch=p, device=str(dev))) if batch else (lambda: dies.Model(p, device=str(dev)))
+    m = make()
     info = dies.dies_device_info()
     stream = torch.cuda.current_stream(dev)
     flush = torch.empty(256 * 1024 * 1024, dtype=torch.uint8, device=dev)   # > 126 MB L2
@@ -175,7 +192,7 @@ def run_ours(args, rank, world, local_rank):
         torch.cuda.synchronize(dev)
 
     for w in range(args.warmup):
-        m.dies_run(n, seed=sharding.replica_seed(1000, w, rank), **opts)
+        m.dies_run(n_per_model, seed=sharding.replica_seed(1000, w, rank), **opts)
     torch.cuda.synchronize(dev)
     c0 = m.dies_get_counters()
 
@@ -189,7 +206,7 @@ def run_ours(args, rank, world, local_rank):
     for s in range(args.steps):
         flush.fill_(s & 0xFF)
         ev[s][0].record(stream)
-        m.dies_run(n, seed=sharding.replica_seed(1, s, rank), **opts)
+        m.dies_run(n_per_model, seed=sharding.replica_seed(1, s, rank), **opts)
         ev[s][1].record(stream)
     barrier()
     t_wall = time.perf_counter() - t_wall
@@ -209,23 +226,24 @@ def run_ours(args, rank, world, local_rank):
     for s in range(max(1, min(args.steps, 5))):
         torch.cuda.synchronize(dev)
         t0 = time.perf_counter()
-        m2 = dies.Model(p, device=str(dev))
-        m2.dies_run(n, seed=1 + s, **opts)
+        m2 = make()
+        m2.dies_run(n_per_model, seed=1 + s, **opts)
         T = m2.dies_get_temperature()
         Lesc = m2.dies_get_escape_spectrum()
         e2e_t.append(time.perf_counter() - t0)
         m2.close()
     e2e_val = world * n / float(np.median(e2e_t))
-    h2d = 8 * (p.emis.size + p.T_grid.size + 3 * p.n_freq + p.r_bounds.size + p.rho.size + 2 * p.n_freq)
-    d2h = 8 * (p.n_shells + p.n_freq) + 64
+    h2d = 8 * (p.emis.size + p.T_grid.size + 3 * n_freq + p.r_bounds.size + p.rho.size + 2 * n_freq * n_models)
+    d2h = 8 * n_models * (n_shells + n_freq) + 64
 
     if rank != 0:
         return
     # the atomic side of the roofline: the absorption step's returning 64-bit atomicAdd pattern alone on n_shells
     # tallies (merged per warp when all quanta are equal, as in this run), measured on this GPU outside the timed region
-    uniform_q = (p.k_bg == 0.5 and not p.ffi and not (p.ext_bin_intensity is not None and p.L_point > 0))
+    uniform_q = (k_bg == 0.5 and not ffi and not (p.ext_bin_intensity is not None and getattr(p, "L_point", 0.0) > 0))
     raw_abs, _, _ = m.dies_get_absorbed()                     # per-shell absorption histogram of the last step
-    atom = dies.dies_bench_atomics(p.n_shells, weights=np.asarray(raw_abs, dtype=np.float64).reshape(-1),
+    hist = np.asarray(raw_abs, dtype=np.float64).reshape(n_models, n_shells).sum(0)
+    atom = dies.dies_bench_atomics(n_shells * min(n_models, 64), weights=np.tile(hist, min(n_models, 64)),
                                    aggregate=1 if uniform_q else 0)
     sm_max, peak_src = load_peaks()
     peak = SM_COUNT * SCHEDULERS * LANES * sm_max * 1e6 / 1e12          # thread-instructions/s, 1e12
@@ -237,8 +255,8 @@ def run_ours(args, rank, world, local_rank):
                 warmup=args.warmup, ms_per_step=total_ms / args.steps, higher_is_better=True, scaling="weak",
                 vs_baseline=None, dtype="f32", data="synthetic",
                 crossings_per_s=crossings_per_s,
-                config=dict(workload=args.workload, n_shells=p.n_shells, n_freq=p.n_freq, n_T=p.n_T,
-                            packages_per_step=n, mode="full IRE", k_bg=p.k_bg, ffi=p.ffi,
+                config=dict(workload=args.workload, n_models=n_models, n_shells=n_shells, n_freq=n_freq, n_T=n_T,
+                            packages_per_step=n, mode="full IRE", k_bg=k_bg, ffi=ffi,
                             parallelism="replicas only" if world > 1 else "1 GPU", l2="flushed between steps (256 MiB fill)",
                             per_package=dict(crossings=c1["crossings"] / n, scatterings=c1["scatterings"] / n,
                                              absorptions=c1["absorptions"] / n),
@@ -253,15 +271,18 @@ def run_ours(args, rank, world, local_rank):
                                           peak_absorptions_per_s=atom["lane_ops_per_s"],
                                           peak_atomic_instr_per_s=atom["atomics_per_s"],
                                           frac=c1["absorptions"] / (step_ms * 1e-3) / atom["lane_ops_per_s"],
-                                          peak_source=f"dies_bench_atomics({p.n_shells} tallies, the run's shell histogram, warp-merged={int(uniform_q)}) on this GPU"),
+                                          peak_source=f"dies_bench_atomics({n_shells * min(n_models, 64)} tallies, the run's shell histogram, warp-merged={int(uniform_q)}) on this GPU"),
                               peak_source=f"148 SMs x 4 schedulers x 32 lanes x {sm_max:.0f} MHz ({peak_src})",
                               instr_per_unit=INSTR, kernel="dies_track<0,false>", kernel_ms=step_ms),
                 wall_s=t_wall)
     # ---- the oracle timed beside it on this box's host cores (rank 0, N = 1 only)
     if world == 1 and not args.no_cpu_baseline:
-        r, cr, dt, c = oracle_rate(p, min(n, args.cpu_sample))
+        # bounded sample: a pilot of 4000 packages sizes the sample to about --cpu-seconds of CPU work
+        r0, _, _, _ = oracle_rate(p, 4000)
+        n_cpu = int(min(n, args.cpu_sample, max(4000, r0 * args.cpu_seconds)))
+        r, cr, dt, c = oracle_rate(p, n_cpu)
         line["cpu_baseline"] = dict(value=r, unit="packages/s", cores=1, kind="oracle", crossings_per_s=cr,
-                                    sample=f"{min(n, args.cpu_sample)} packages of {args.workload} ({dt:.1f} s), serial fp64 oracle",
+                                    sample=f"{n_cpu} packages of {args.workload} ({dt:.1f} s), serial fp64 oracle",
                                     host_cores=os.cpu_count())
     print(json.dumps(line))
     m.close()
@@ -275,7 +296,8 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="config2")
     ap.add_argument("--packages", type=float, default=0)
-    ap.add_argument("--cpu-sample", type=int, default=6_000_000)
+    ap.add_argument("--cpu-sample", type=int, default=20_000_000)
+    ap.add_argument("--cpu-seconds", type=float, default=12.0)
     ap.add_argument("--ref-sample", type=int, default=1_000_000)
     ap.add_argument("--ref-total", type=int, default=20_000_000)
     ap.add_argument("--no-cpu-baseline", action="store_true")

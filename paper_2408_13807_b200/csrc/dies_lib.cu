@@ -63,7 +63,7 @@ static Layout make_layout(int N, int K, int nT, int M)
     L.mp = take((size_t)M * sizeof(ModelParams));
     L.fixed_row = take((size_t)M * ldS * 4);
     L.Tfix = take((size_t)M * N * 8);
-    L.A = take((size_t)M * ldS * 8);
+    L.A = take((size_t)M * ldS * kTallyStride * 8);
     L.esc = take((size_t)M * K * 8);
     L.next_id = take((size_t)M * 8);
     L.counters = take((size_t)DIES_N_COUNTERS * 8);
@@ -274,7 +274,7 @@ __global__ void k_prepare_run(DeviceModel D, const double* __restrict__ mass, co
         const double eu = fmax(Le, Lp) / n_total / qscale;
         const double ms = mass[idx];
         cscale[idx] = ms > 0.0 ? eu / (ms * *epsref) : 0.0;
-        if (zero) D.A[idx] = 0ull;
+        if (zero) D.A[(size_t)idx * kTallyStride] = 0ull;
     }
     if (zero && idx < D.n_models * D.K) D.esc[idx] = 0ull;
 }
@@ -294,7 +294,7 @@ __global__ void k_finalize(DeviceModel D, const double* __restrict__ mass, const
     if (idx < D.n_models * N) {
         const int m = idx / N, i = idx % N;
         const int j = i + mp[m].cav;
-        const unsigned long long a = D.A[(size_t)m * ldS + j];
+        const unsigned long long a = D.A[((size_t)m * ldS + j) * kTallyStride];
         if (a > (1ull << 62)) atomicOr(flags + 1, 1);
         const double ms = mass[(size_t)m * ldS + j];
         double T = 0.0;
@@ -703,7 +703,8 @@ extern "C" int dies_get_absorbed(dies_model* m, int64_t* raw, double* energy_per
     CUDA_TRY(cudaStreamSynchronize(m->stream));
     std::vector<unsigned long long> a((size_t)m->M * m->ldS);
     std::vector<ModelParams> mp(m->M);
-    CUDA_TRY(cudaMemcpy(a.data(), m->ws + m->L.A, a.size() * 8, cudaMemcpyDeviceToHost));
+    // the tallies are kTallyStride words apart on the device
+    CUDA_TRY(cudaMemcpy2D(a.data(), 8, m->ws + m->L.A, (size_t)kTallyStride * 8, 8, a.size(), cudaMemcpyDeviceToHost));
     CUDA_TRY(cudaMemcpy(mp.data(), m->ws + m->L.mp, mp.size() * sizeof(ModelParams), cudaMemcpyDeviceToHost));
     for (int i = 0; i < m->M; i++)
         for (int s = 0; s < m->N; s++) {
@@ -811,7 +812,7 @@ extern "C" int dies_test_philox(uint64_t seed, uint64_t first_id, uint32_t block
 // The absorption step of the tracker as a stand-alone loop: every lane draws a shell (uniform over n_addr tallies,
 // 8 bytes apart like the tallies of a model), the warp aggregates equal shells with __match_any_sync when asked to,
 // and one lane per distinct shell issues a RETURNING 64-bit atomicAdd whose result every lane consumes.
-__global__ void k_bench_atomics(unsigned long long* tallies, int n_addr, const unsigned short* __restrict__ lut,
+__global__ void k_bench_atomics(unsigned long long* tallies, int n_addr, int stride, const unsigned short* __restrict__ lut,
                                 int aggregate, int iters, unsigned long long* sink, unsigned long long* n_atomics)
 {
     const unsigned lane = threadIdx.x & 31u;
@@ -827,10 +828,10 @@ __global__ void k_bench_atomics(unsigned long long* tallies, int n_addr, const u
             const unsigned peers = __match_any_sync(0xffffffffu, j);
             const int leader = __ffs(peers) - 1;
             old = 0;
-            if ((int)lane == leader) { old = atomicAdd(&tallies[j], (unsigned long long)__popc(peers)); issued++; }
+            if ((int)lane == leader) { old = atomicAdd(&tallies[(size_t)j * stride], (unsigned long long)__popc(peers)); issued++; }
             old = __shfl_sync(0xffffffffu, old, leader) + (unsigned long long)__popc(peers & lt_mask);
         } else {
-            old = atomicAdd(&tallies[j], 1ull);
+            old = atomicAdd(&tallies[(size_t)j * stride], 1ull);
             issued++;
         }
         acc += old;
@@ -843,6 +844,7 @@ __global__ void k_bench_atomics(unsigned long long* tallies, int n_addr, const u
 extern "C" int dies_bench_atomics(int n_addr, const double* weights, int aggregate, int iters, double* lane_ops_per_s,
                                   double* atomics_per_s)
 {
+    const int stride = env_int("DIES_ATOM_STRIDE", 1, 64, kTallyStride);     // 64-bit words between two tallies
     if (n_addr < 1 || n_addr > 65535 || iters < 1 || !lane_ops_per_s || !atomics_per_s)
         return fail(DIES_EINVAL, "bad arguments");
     // look-up table of the histogram: entry e holds the tally whose cumulative weight covers (e + 0.5) / 4096
@@ -865,10 +867,10 @@ extern "C" int dies_bench_atomics(int n_addr, const double* weights, int aggrega
     CUDA_TRY(cudaGetDevice(&dev));
     CUDA_TRY(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
     unsigned long long* buf = nullptr;
-    CUDA_TRY(cudaMalloc(&buf, ((size_t)n_addr + 2) * 8 + 4096 * 2));
+    CUDA_TRY(cudaMalloc(&buf, ((size_t)n_addr * stride + 2) * 8 + 4096 * 2));
     unsigned short* d_lut = nullptr;
     if (weights) {
-        d_lut = reinterpret_cast<unsigned short*>(buf + n_addr + 2);
+        d_lut = reinterpret_cast<unsigned short*>(buf + (size_t)n_addr * stride + 2);
         if (cudaMemcpy(d_lut, lut.data(), 4096 * 2, cudaMemcpyHostToDevice) != cudaSuccess) { cudaFree(buf); return fail(DIES_ECUDA, "copy failed"); }
     }
     cudaEvent_t e0, e1;
@@ -878,15 +880,15 @@ extern "C" int dies_bench_atomics(int n_addr, const double* weights, int aggrega
     unsigned long long issued = 0;
     cudaError_t e = cudaSuccess;
     for (int rep = 0; rep < 4 && e == cudaSuccess; rep++) {          // first repetition warms up
-        cudaMemset(buf, 0, ((size_t)n_addr + 2) * 8);
+        cudaMemset(buf, 0, ((size_t)n_addr * stride + 2) * 8);
         cudaEventRecord(e0);
-        k_bench_atomics<<<grid, block>>>(buf, n_addr, d_lut, aggregate, iters, buf + n_addr, buf + n_addr + 1);
+        k_bench_atomics<<<grid, block>>>(buf, n_addr, stride, d_lut, aggregate, iters, buf + (size_t)n_addr * stride, buf + (size_t)n_addr * stride + 1);
         cudaEventRecord(e1);
         e = cudaEventSynchronize(e1);
         float ms = 0.f;
         cudaEventElapsedTime(&ms, e0, e1);
         if (rep > 0 && ms < best) best = ms;
-        if (e == cudaSuccess) e = cudaMemcpy(&issued, buf + n_addr + 1, 8, cudaMemcpyDeviceToHost);
+        if (e == cudaSuccess) e = cudaMemcpy(&issued, buf + (size_t)n_addr * stride + 1, 8, cudaMemcpyDeviceToHost);
     }
     cudaEventDestroy(e0); cudaEventDestroy(e1);
     cudaFree(buf);

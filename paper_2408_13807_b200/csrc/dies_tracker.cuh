@@ -30,6 +30,8 @@ constexpr unsigned kChunk = 128;     // package ids a warp takes from the global
 constexpr int kUnroll = 12;           // crossings per vote in the crossing loop
 constexpr int kMaxPool = 248;        // pool slots per warp (queue entries are bytes)
 constexpr int kGuide = 256;          // cut-points per CDF row of the guide tables
+constexpr int kTallyStride = 32;     // 64-bit words between the absorbed-energy tallies of two shells: one tally per
+                                     // 256 bytes, because the L2 atomic unit serialises updates of the same line
 
 // event counters (same order as DIES_C_* in include/dies.h), accumulated per block in shared memory
 enum { LC_PACKAGES = 0, LC_CROSSINGS, LC_FFI_CROSSINGS, LC_SCATTERINGS, LC_ABSORPTIONS, LC_ESCAPED, LC_UNINTERACTED,
@@ -70,7 +72,7 @@ struct DeviceModel {
     const float* srccdf;             // n_models x 2 x K: external, point
     const ModelParams* mp;           // n_models
     const int* fixed_row;            // n_models x ldS
-    unsigned long long* A;           // n_models x ldS   absorbed-energy tallies (raw fixed point)
+    unsigned long long* A;           // n_models x ldS x kTallyStride: absorbed-energy tallies (raw fixed point), strided
     unsigned long long* esc;         // n_models x K     escape tallies (raw fixed point)
     unsigned long long* next_id;     // n_models         run-local package counter
     unsigned long long* counters;    // DIES_N_COUNTERS
@@ -316,7 +318,7 @@ __global__ void __launch_bounds__(kBlock, kMinBlocks) dies_track(DeviceModel D, 
         for (int x = lane; x < P; x += 32) { qL[x] = (unsigned char)x; pB[x] = make_uint4(0u, 0u, 0u, 0u); }
         __syncthreads();
 
-        unsigned long long* const gA = D.A + (size_t)m * ldS;
+        unsigned long long* const gA = D.A + (size_t)m * ldS * kTallyStride;
         unsigned long long* const g_next = TRACE ? tp.counter : D.next_id + m;
         const float* const g_src = D.srccdf + (size_t)m * 2 * K;
         const unsigned short* const g_srcguide = D.guideS + (size_t)m * 2 * kGuide;
@@ -385,16 +387,16 @@ __global__ void __launch_bounds__(kBlock, kMinBlocks) dies_track(DeviceModel D, 
                 unsigned long long old = 0;
                 if (absmask) {
                     if (TRACE) {
-                        if (isabs && MODE == 0) old = gA[j];
+                        if (isabs && MODE == 0) old = gA[j * kTallyStride];
                     } else if (MODE == 1) {
                         if (isabs) smem_add64(&s_A[j], &s_A[ldS + j], q);
                     } else if (R.uniform_q) {
                         const unsigned peers = __match_any_sync(kFull, isabs ? j : -1 - lane);
                         const int leader = __ffs(peers) - 1;
-                        if (isabs && lane == leader) old = atomicAdd(&gA[j], q * (unsigned long long)__popc(peers));
+                        if (isabs && lane == leader) old = atomicAdd(&gA[j * kTallyStride], q * (unsigned long long)__popc(peers));
                         old = __shfl_sync(kFull, old, leader) + q * (unsigned long long)__popc(peers & lt_mask);
                     } else if (isabs) {
-                        old = atomicAdd(&gA[j], q);
+                        old = atomicAdd(&gA[j * kTallyStride], q);
                     }
                     wc_abs += __popc(absmask);
                 }
@@ -754,7 +756,7 @@ __global__ void __launch_bounds__(kBlock, kMinBlocks) dies_track(DeviceModel D, 
         if (MODE == 1)
             for (int x = tid; x < Np; x += kBlock) {
                 const unsigned long long v = (unsigned long long)s_A[x] | ((unsigned long long)s_A[ldS + x] << 32);
-                if (v) atomicAdd(&gA[x], v);
+                if (v) atomicAdd(&gA[x * kTallyStride], v);
             }
     }
 
