@@ -353,12 +353,16 @@ static int env_int(const char* name, int lo, int hi, int dflt)
 }
 
 // pool slots per warp: a multiple of 8 in [32, kMaxPool]
-static int pool_slots() { return env_int("DIES_POOL", 32, kMaxPool, 96) & ~7; }
+// (with per-package quanta | with one quantum for all packages: 8 bytes less per slot, so a deeper pool fits)
+static int pool_slots(bool uniform_q)
+{
+    return (uniform_q ? env_int("DIES_POOL_U", 32, kMaxPool, 120) : env_int("DIES_POOL", 32, kMaxPool, 96)) & ~7;
+}
 
-static size_t tracker_smem(int N, int K, int nT, int P, bool trace)
+static size_t tracker_smem(int N, int K, int nT, int P, bool trace, bool with_q)
 {
     const int ldS = N + 1, ldT = 2 * ldS + 2;
-    return plan_smem(K, nT, ldS, ldT, P, trace).total;
+    return plan_smem(K, nT, ldS, ldT, P, trace, with_q).total;
 }
 
 template <int MODE, bool TRACE>
@@ -381,7 +385,7 @@ extern "C" int dies_device_info(int* n_sms, int* blocks_per_sm, int* threads_per
     int dev = 0, sms = 0, bps = 0;
     CUDA_TRY(cudaGetDevice(&dev));
     CUDA_TRY(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
-    CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&bps, dies_track<0, false>, kBlock, tracker_smem(100, 200, 1000, pool_slots(), false)));
+    CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&bps, dies_track<0, false>, kBlock, tracker_smem(100, 200, 1000, pool_slots(true), false, false)));
     if (n_sms) *n_sms = sms;
     if (blocks_per_sm) *blocks_per_sm = bps;
     if (threads_per_block) *threads_per_block = kBlock;
@@ -423,8 +427,11 @@ extern "C" int dies_create_batch(int n_models, int n_shells, const double* r_bou
     if (rc) return rc;
     const Layout L = make_layout(N, K, nT, M);
     if (workspace_bytes < L.total) return fail(DIES_ENOMEM, "workspace too small: %zu < %zu", workspace_bytes, L.total);
-    const int pool = pool_slots();
-    const size_t smem = tracker_smem(N, K, nT, pool, false), smem_trace = tracker_smem(N, K, nT, pool, true);
+    const int pool = pool_slots(false);
+    size_t smem = tracker_smem(N, K, nT, pool, false, true);
+    const size_t smem_u = tracker_smem(N, K, nT, pool_slots(true), false, false);
+    if (smem_u > smem) smem = smem_u;                       // largest of the two launch shapes
+    const size_t smem_trace = tracker_smem(N, K, nT, pool, true, true);
     if (smem_trace > 200 * 1024) return fail(DIES_EINVAL, "tables do not fit in shared memory (%zu bytes)", smem_trace);
 
     dies_model* m = new (std::nothrow) dies_model();
@@ -593,7 +600,7 @@ static int fill_run_params(dies_model* m, uint64_t n_packages, uint64_t seed, co
     R->k_bg = (float)d.k_bg; R->ffi = d.ffi ? 1 : 0;
     R->uniform_q = (d.k_bg == 0.5 && !d.ffi && !two) ? 1 : 0;
     R->qscale = (float)(1u << d.fixed_shift);
-    R->pool = m->pool;
+    R->pool = pool_slots(R->uniform_q != 0);
     R->thr_hi = env_int("DIES_THR_HI", 1, 32, 20);
     R->thr_lo = env_int("DIES_THR_LO", 1, 32, 16);
     R->min_ready = env_int("DIES_MIN_READY", 1, kMaxPool, 32);
@@ -623,12 +630,18 @@ extern "C" int dies_run(dies_model* m, uint64_t n_packages, uint64_t seed, const
     m->stream = st;
     m->n_total = n_total; m->shift = shift;
 
-    // grid: persistent blocks, at most blocks_per_sm per SM, fewer for tiny runs
+    // launch shape: shared memory of this run's pool, persistent blocks (as many as fit on an SM), fewer for tiny runs
+    const size_t smem_launch = tracker_smem(m->N, m->K, m->nT, R.pool, false, !R.uniform_q);
+    int bps = 0;
+    if (mode == DIES_MODE_IRE) CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&bps, dies_track<0, false>, kBlock, smem_launch));
+    else CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&bps, dies_track<1, false>, kBlock, smem_launch));
+    if (bps < 1) return fail(DIES_ECUDA, "tracker does not fit on an SM");
+    const int grid_max = m->n_sms * bps;
     unsigned long long ids = 0;
     for (int i = 0; i < m->M; i++) ids += n_packages * (unsigned long long)(m->has_ext[i] + m->has_point[i]);
-    const unsigned long long per_block = (unsigned long long)kWarps * m->pool;    // packages a block keeps in flight
+    const unsigned long long per_block = (unsigned long long)kWarps * R.pool;    // packages a block keeps in flight
     unsigned long long want = (ids + 2ull * per_block - 1) / (2ull * per_block);
-    int grid = (int)(want < 1 ? 1 : (want > (unsigned long long)m->grid_max ? m->grid_max : want));
+    int grid = (int)(want < 1 ? 1 : (want > (unsigned long long)grid_max ? grid_max : want));
     if (m->M == 1) { R.parts = grid; R.n_tickets = grid; }
     else { R.parts = (8 * grid + m->M - 1) / m->M; if (R.parts < 1) R.parts = 1; R.n_tickets = m->M * R.parts; }
 
@@ -638,8 +651,8 @@ extern "C" int dies_run(dies_model* m, uint64_t n_packages, uint64_t seed, const
                                                     wsp<double>(m, m->L.eunit), wsp<ModelParams>(m, m->L.mp),
                                                     (double)n_total, (double)R.qscale, accumulate ? 0 : 1);
     TraceParams tp = {0, 0, 0, nullptr, 0, nullptr, nullptr};
-    if (mode == DIES_MODE_IRE) dies_track<0, false><<<grid, kBlock, m->smem_bytes, st>>>(m->D, R, tp);
-    else dies_track<1, false><<<grid, kBlock, m->smem_bytes, st>>>(m->D, R, tp);
+    if (mode == DIES_MODE_IRE) dies_track<0, false><<<grid, kBlock, smem_launch, st>>>(m->D, R, tp);
+    else dies_track<1, false><<<grid, kBlock, smem_launch, st>>>(m->D, R, tp);
     m->launches += 2;
     CUDA_TRY(cudaGetLastError());
     m->done += n_packages;
@@ -764,6 +777,7 @@ extern "C" int dies_trace_packages(dies_model* m, int model_index, uint64_t firs
         m->launches += 1;
     }
     R.n_run = nt; R.id_base = 0;
+    R.uniform_q = 0; R.pool = m->pool;                     // the trace kernels keep the quantum per package
     int32_t *d_ev = nullptr, *d_n = nullptr;
     CUDA_TRY(cudaMalloc(&d_ev, (size_t)count * max_events * 16));
     // n_events (count ints) followed by the 64-bit counter the traced package indices are taken from

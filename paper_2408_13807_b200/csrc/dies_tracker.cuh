@@ -81,7 +81,7 @@ struct DeviceModel {
 
 // shared-memory plan of a block (byte offsets), used by the kernel and by the host to size the launch
 struct SmemPlan { unsigned bin, cs, tab, eps, omega, row, esc, A, poolA, poolB, poolQ, queues, trace, total; };
-__host__ __device__ inline SmemPlan plan_smem(int K, int nT, int ldS, int ldT, int P, bool trace)
+__host__ __device__ inline SmemPlan plan_smem(int K, int nT, int ldS, int ldT, int P, bool trace, bool with_q)
 {
     SmemPlan p;
     unsigned o = 0;
@@ -96,7 +96,7 @@ __host__ __device__ inline SmemPlan plan_smem(int K, int nT, int ldS, int ldT, i
     o = (o + 15u) & ~15u;
     p.poolA = o; o += 16u * kWarps * P;              // float4 {s, b2, col, pa}
     p.poolB = o; o += 16u * kWarps * P;              // uint4  {id lo, id hi, blk, flags}
-    p.poolQ = o; o += 8u * kWarps * P;               // raw quantum of the package
+    p.poolQ = o; if (with_q) o += 8u * kWarps * P;   // raw quantum of the package (not stored when all are equal)
     p.queues = o; o += (unsigned)(QT_N * kWarps * P);
     o = (o + 15u) & ~15u;
     p.trace = o; if (trace) o += 12u * kWarps * P;   // pkg, n_ev, crossings so far
@@ -260,7 +260,7 @@ __global__ void __launch_bounds__(kBlock, kMinBlocks) dies_track(DeviceModel D, 
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const int K = D.K, nT = D.nT, ldS = D.ldS, ldT = D.ldT, P = R.pool;
-    const SmemPlan sp = plan_smem(K, nT, ldS, ldT, P, TRACE);
+    const SmemPlan sp = plan_smem(K, nT, ldS, ldT, P, TRACE, !R.uniform_q);
     float4* const s_bin = reinterpret_cast<float4*>(smem_raw + sp.bin);             // K
     double* const s_cs = reinterpret_cast<double*>(smem_raw + sp.cs);               // ldS
     float2* const s_tab = reinterpret_cast<float2*>(smem_raw + sp.tab);             // ldT unfolded shell table
