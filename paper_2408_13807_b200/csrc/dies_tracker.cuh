@@ -194,6 +194,48 @@ __device__ __forceinline__ float2 lds_entry(unsigned a)
     return v;
 }
 
+// the pool and the queues of a warp are addressed in the shared window directly (32-bit addresses, no generic pointers)
+__device__ __forceinline__ unsigned lds_u8(unsigned a)
+{
+    unsigned v;
+    asm volatile("ld.shared.u8 %0, [%1];" : "=r"(v) : "r"(a) : "memory");
+    return v;
+}
+__device__ __forceinline__ void sts_u8(unsigned a, unsigned v) { asm volatile("st.shared.u8 [%0], %1;" :: "r"(a), "r"(v) : "memory"); }
+__device__ __forceinline__ unsigned lds_u32(unsigned a)
+{
+    unsigned v;
+    asm volatile("ld.shared.u32 %0, [%1];" : "=r"(v) : "r"(a) : "memory");
+    return v;
+}
+__device__ __forceinline__ float4 lds_f4(unsigned a)
+{
+    float4 v;
+    asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(a) : "memory");
+    return v;
+}
+__device__ __forceinline__ void sts_f4(unsigned a, float x, float y, float z, float w)
+{
+    asm volatile("st.shared.v4.f32 [%0], {%1, %2, %3, %4};" :: "r"(a), "f"(x), "f"(y), "f"(z), "f"(w) : "memory");
+}
+__device__ __forceinline__ uint4 lds_u4(unsigned a)
+{
+    uint4 v;
+    asm volatile("ld.shared.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "r"(a) : "memory");
+    return v;
+}
+__device__ __forceinline__ void sts_u4(unsigned a, unsigned x, unsigned y, unsigned z, unsigned w)
+{
+    asm volatile("st.shared.v4.u32 [%0], {%1, %2, %3, %4};" :: "r"(a), "r"(x), "r"(y), "r"(z), "r"(w) : "memory");
+}
+__device__ __forceinline__ unsigned long long lds_u64(unsigned a)
+{
+    unsigned long long v;
+    asm volatile("ld.shared.u64 %0, [%1];" : "=l"(v) : "r"(a) : "memory");
+    return v;
+}
+__device__ __forceinline__ void sts_u64(unsigned a, unsigned long long v) { asm volatile("st.shared.u64 [%0], %1;" :: "r"(a), "l"(v) : "memory"); }
+
 // smallest k with cdf[k] > u for a non-decreasing cdf whose last entry exceeds every u (inverse-CDF sampling, R3),
 // by the cut-point method: guide[c] is the answer for u = c / kGuide, so the answer for u in [c, c+1) / kGuide is
 // found by walking up from it -- one or two table reads instead of a bisection over the whole row
@@ -275,13 +317,12 @@ __global__ void __launch_bounds__(kBlock, kMinBlocks) dies_track(DeviceModel D, 
     const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
     const unsigned lt_mask = (1u << lane) - 1u;
     // the pool and the queues of this warp
-    float4* const pA = reinterpret_cast<float4*>(smem_raw + sp.poolA) + wid * P;
-    uint4* const pB = reinterpret_cast<uint4*>(smem_raw + sp.poolB) + wid * P;
-    unsigned long long* const pQ = reinterpret_cast<unsigned long long*>(smem_raw + sp.poolQ) + wid * P;
-    unsigned char* const qA = smem_raw + sp.queues + (size_t)wid * QT_N * P;
-    unsigned char* const qS = qA + P;
-    unsigned char* const qL = qS + P;
-    unsigned char* const qR = qL + P;
+    const unsigned sbase = (unsigned)__cvta_generic_to_shared(smem_raw);
+    const unsigned aA = sbase + sp.poolA + 16u * (unsigned)(wid * P);          // float4 {s, b2, col, pa} per slot
+    const unsigned aB = sbase + sp.poolB + 16u * (unsigned)(wid * P);          // uint4 {id lo, id hi, blk, flags}
+    const unsigned aQ = sbase + sp.poolQ + 8u * (unsigned)(wid * P);           // raw quantum
+    const unsigned qA = sbase + sp.queues + (unsigned)(wid * QT_N * P);        // byte queues of pool slots
+    const unsigned qS = qA + (unsigned)P, qL = qS + (unsigned)P, qR = qL + (unsigned)P;
     int* const pT = reinterpret_cast<int*>(smem_raw + sp.trace) + wid * 3 * P;      // TRACE only
 
     for (int x = tid; x < K; x += kBlock) { s_bin[x] = D.bintab[x]; s_omega[x] = D.omega[x]; }
@@ -315,7 +356,7 @@ __global__ void __launch_bounds__(kBlock, kMinBlocks) dies_track(DeviceModel D, 
         }
         for (int x = tid; x < 2 * K; x += kBlock) s_esc[x] = 0u;
         // every slot of the pool is free and waits for a package id
-        for (int x = lane; x < P; x += 32) { qL[x] = (unsigned char)x; pB[x] = make_uint4(0u, 0u, 0u, 0u); }
+        for (int x = lane; x < P; x += 32) { sts_u8(qL + x, (unsigned)x); sts_u4(aB + 16u * x, 0u, 0u, 0u, 0u); }
         __syncthreads();
 
         unsigned long long* const gA = D.A + (size_t)m * ldS * kTallyStride;
@@ -352,9 +393,9 @@ __global__ void __launch_bounds__(kBlock, kMinBlocks) dies_track(DeviceModel D, 
                 unsigned slot = 0;
                 {
                     int l = lane;
-                    if (l < cA) { type = QT_ABS; slot = qA[nA - 1 - l]; }
-                    else if ((l -= cA) < cS) { type = QT_SCA; slot = qS[nS - 1 - l]; }
-                    else if ((l -= cS) < cL) { type = QT_SRC; slot = qL[nL - 1 - l]; }
+                    if (l < cA) { type = QT_ABS; slot = lds_u8(qA + (nA - 1 - l)); }
+                    else if ((l -= cA) < cS) { type = QT_SCA; slot = lds_u8(qS + (nS - 1 - l)); }
+                    else if ((l -= cS) < cL) { type = QT_SRC; slot = lds_u8(qL + (nL - 1 - l)); }
                 }
                 nA -= cA; nS -= cS; nL -= cL;
                 const bool isabs = type == QT_ABS, issca = type == QT_SCA, issrc = type == QT_SRC;
@@ -367,11 +408,11 @@ __global__ void __launch_bounds__(kBlock, kMinBlocks) dies_track(DeviceModel D, 
                 int pkg = 0, n_ev = 0;
                 unsigned ncross = 0;
                 if (type >= 0) {
-                    const float4 a = pA[slot];
-                    const uint4 b = pB[slot];
+                    const float4 a = lds_f4(aA + 16u * slot);
+                    const uint4 b = lds_u4(aB + 16u * slot);
                     s = a.x; b2 = a.y; col = a.z; pa = __float_as_uint(a.w);
                     id = (unsigned long long)b.x | ((unsigned long long)b.y << 32); blk = b.z; kf = b.w;
-                    if (!R.uniform_q) q = pQ[slot];
+                    if (!R.uniform_q) q = lds_u64(aQ + 8u * slot);
                     if (TRACE) { pkg = pT[slot]; n_ev = pT[P + slot]; ncross = (unsigned)pT[2 * P + slot]; }
                 }
                 int k = (int)(kf & KF_K);
@@ -587,9 +628,9 @@ __global__ void __launch_bounds__(kBlock, kMinBlocks) dies_track(DeviceModel D, 
                 if (fly || uninter) {
                     const unsigned nkf = uninter ? 0u
                         : ((unsigned)k | (ev_absorb ? KF_EVABS : 0u) | (dry ? KF_DRY : 0u) | KF_OCC);
-                    pA[slot] = make_float4(s, b2, col, __uint_as_float(pa));
-                    pB[slot] = make_uint4((unsigned)id, (unsigned)(id >> 32), blk, nkf);
-                    if (!R.uniform_q) pQ[slot] = q;
+                    sts_f4(aA + 16u * slot, s, b2, col, __uint_as_float(pa));
+                    sts_u4(aB + 16u * slot, (unsigned)id, (unsigned)(id >> 32), blk, nkf);
+                    if (!R.uniform_q) sts_u64(aQ + 8u * slot, q);
                     if (TRACE) { pT[slot] = pkg; pT[P + slot] = n_ev; pT[2 * P + slot] = (int)ncross; }
                 }
                 if (!R.uniform_q) {
@@ -603,11 +644,11 @@ __global__ void __launch_bounds__(kBlock, kMinBlocks) dies_track(DeviceModel D, 
                     }
                 }
                 const unsigned flym = __ballot_sync(kFull, fly);
-                if (fly) qR[nR + __popc(flym & lt_mask)] = (unsigned char)slot;
+                if (fly) sts_u8(qR + nR + __popc(flym & lt_mask), slot);
                 nR += __popc(flym);
                 const unsigned unm = __ballot_sync(kFull, uninter);
                 if (unm) {
-                    if (uninter) qL[nL + __popc(unm & lt_mask)] = (unsigned char)slot;
+                    if (uninter) sts_u8(qL + nL + __popc(unm & lt_mask), slot);
                     nL += __popc(unm);
                 }
                 __syncwarp();
@@ -629,8 +670,8 @@ __global__ void __launch_bounds__(kBlock, kMinBlocks) dies_track(DeviceModel D, 
                 unsigned slot = 0, pa = tab0;
                 float s = 0.f, b2 = 0.f, col = -1.f;
                 if (has) {
-                    slot = qR[nR - 1 - lane];
-                    const float4 a = pA[slot];
+                    slot = lds_u8(qR + (nR - 1 - lane));
+                    const float4 a = lds_f4(aA + 16u * slot);
                     s = a.x; b2 = a.y; col = a.z; pa = __float_as_uint(a.w);
                 }
                 nR -= min(nR, 32);
@@ -677,12 +718,12 @@ __global__ void __launch_bounds__(kBlock, kMinBlocks) dies_track(DeviceModel D, 
                     const bool out = has && (leave || !alive);
                     int t = -1;
                     if (out) {
-                        const unsigned kf = pB[slot].w;
+                        const unsigned kf = lds_u32(aB + 16u * slot + 12u);
                         const bool isev = !alive && (col < 0.f);         // the column ran out: scattering or absorption
                         const unsigned n = ((pa - pa0) >> 3) - (isev ? 1u : 0u);
                         if (kf & KF_DRY) lc_ffi += n;
                         else { lc_cross += n; if (TRACE) pT[2 * P + slot] += (int)n; }
-                        pA[slot] = make_float4(s, b2, col, __uint_as_float(pa));
+                        sts_f4(aA + 16u * slot, s, b2, col, __uint_as_float(pa));
                         // stopped on the sentinel: left the model (escape, or the end of a dry FFI flight)
                         t = alive ? QT_READY : (isev ? ((kf & KF_EVABS) ? QT_ABS : QT_SCA) : QT_SRC);
                     }
@@ -692,7 +733,7 @@ __global__ void __launch_bounds__(kBlock, kMinBlocks) dies_track(DeviceModel D, 
                         const unsigned mL = __ballot_sync(kFull, t == QT_SRC), mR = __ballot_sync(kFull, t == QT_READY);
                         const unsigned mine = t == QT_ABS ? mA : t == QT_SCA ? mS : t == QT_SRC ? mL : mR;
                         const int base = t == QT_ABS ? nA : t == QT_SCA ? P + nS : t == QT_SRC ? 2 * P + nL : 3 * P + nR;
-                        if (out) qA[base + __popc(mine & lt_mask)] = (unsigned char)slot;
+                        if (out) sts_u8(qA + base + __popc(mine & lt_mask), slot);
                         nA += __popc(mA); nS += __popc(mS); nL += __popc(mL); nR += __popc(mR);
                     }
                     __syncwarp();
@@ -702,8 +743,8 @@ __global__ void __launch_bounds__(kBlock, kMinBlocks) dies_track(DeviceModel D, 
                     const int r = __popc(fm & lt_mask);
                     const bool take = !alive && (r < nR);
                     if (take) {
-                        slot = qR[nR - 1 - r];
-                        const float4 a = pA[slot];
+                        slot = lds_u8(qR + (nR - 1 - r));
+                        const float4 a = lds_f4(aA + 16u * slot);
                         s = a.x; b2 = a.y; col = a.z; pa = __float_as_uint(a.w);
                         pa0 = pa;
                         E = lds_entry(pa);
