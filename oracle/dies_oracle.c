@@ -285,7 +285,7 @@ int dies_oracle_chord_walk(int n_shells, const double* rb, int i, double r, doub
 /* ------------------------------------------------------------------ run state */
 enum { C_PACKAGES = 0, C_CROSSINGS, C_FFI_CROSSINGS, C_SCATTERINGS, C_ABSORPTIONS, C_ESCAPED,
        C_UNINTERACTED, C_TERMINATED, C_EXTRA_BLOCKS, C_CLAMP_HI_SAMPLES, C_N };
-enum { D_INJECTED = 0, D_ESCAPED, D_UNINTERACTED, D_TERMINATED, D_N };
+enum { D_INJECTED = 0, D_ESCAPED, D_UNINTERACTED, D_TERMINATED, D_REWEIGHT, D_N };
 enum { EV_LAUNCH = 0, EV_SCATTER = 1, EV_ABSORB = 2, EV_ESCAPE = 3, EV_TERMINATE = 4, EV_UNINTERACTED = 5 };
 
 typedef struct {
@@ -355,7 +355,28 @@ typedef struct {
     double k_bg;             /* Eq. 5; 0.5 = unweighted */
     int ffi;                 /* Eq. 9-12 */
     int mode;                /* 0 = full IRE, 1 = fixed temperature */
+    const double* kA_w;      /* N or NULL: free-path weighting factor k_A of each shell (Eq. 8; L130: may depend on density) */
+    double kS_w;             /* free-path weighting factor k_S (Eq. 8); 1 = unweighted */
 } run_opts;
+
+/* Density-dependent k_A: linear in the logarithm of the density, k_dilute at the lowest
+ * density of the model and k_dense at the highest (3.0 and 1.0 in the paper's test); shells without dust get
+ * k_dense (they have no opacity).  k_dilute = 0 means the same k_dense everywhere. */
+void dies_oracle_kA_profile(const oracle_model* o, double k_dense, double k_dilute, double* kA_w)
+{
+    double lo = 0.0, hi = 0.0; int any = 0;
+    for (int i = 0; i < o->N; i++) if (o->rho[i] > 0.0) {
+        double l = log(o->rho[i]);
+        if (!any) { lo = hi = l; any = 1; }
+        if (l < lo) lo = l;
+        if (l > hi) hi = l;
+    }
+    for (int i = 0; i < o->N; i++) {
+        kA_w[i] = k_dense;
+        if (k_dilute > 0.0 && o->rho[i] > 0.0 && hi > lo)
+            kA_w[i] = k_dense + (k_dilute - k_dense) * (hi - log(o->rho[i])) / (hi - lo);
+    }
+}
 
 /* Launch direction of a background package (Eq. 2: mu = sqrt(u) w.r.t. the inward
  * normal; L99-103, Eq. 5: mu = u^k_bg with weight W = 2 k_bg mu^(2-1/k_bg); k_bg = 0.5 is Eq. 2).
@@ -444,9 +465,11 @@ static void follow_package(const oracle_model* o, const run_opts* opt, tallies* 
         shell_step(o->rb, i, r, mu, &b2, &l, &inward);
         if (rec && mu < 0.0 && o->rb[i] > 0.0) rec_margin(rec, b2, o->rb[i] * o->rb[i]);
         const double rho = o->rho[i];
-        /* Eq. 4 */
-        double dtauA = o->kA[k] * rho * l;
-        double dtauS = o->kS[k] * rho * l;
+        /* Eq. 4; with free-path weighting (L123-130, Eq. 8; reading R17) the two clocks run k_A and k_S times
+         * faster than the true optical depths: p'(tau) = k e^{-k tau} */
+        const double kAw = opt->kA_w ? opt->kA_w[i] : 1.0, kSw = opt->kS_w;
+        double dtauA = kAw * o->kA[k] * rho * l;
+        double dtauS = kSw * o->kS[k] * rho * l;
         int event = 0, absorb = 0;
         double l_e = l;
         if (forced) {
@@ -461,12 +484,20 @@ static void follow_package(const oracle_model* o, const run_opts* opt, tallies* 
             else {
                 /* L85/L87: whichever free path runs out first along the step (reading R7: tie -> absorption) */
                 event = 1;
-                absorb = tauA * o->kS[k] <= tauS * o->kA[k];
-                rec_margin(rec, tauA * o->kS[k], tauS * o->kA[k]);
+                absorb = tauA * (kSw * o->kS[k]) <= tauS * (kAw * o->kA[k]);
+                rec_margin(rec, tauA * (kSw * o->kS[k]), tauS * (kAw * o->kA[k]));
                 l_e = absorb ? l * tauA / dtauA : l * tauS / dtauS;
             }
         }
         if (ta->pathlen) ta->pathlen[i] += W * l_e;
+        if (kAw != 1.0 || kSw != 1.0) {
+            /* Eq. 8 along the step: the true survival probability over the biased one, e^{-dtau} / e^{-k dtau},
+             * for both clocks; the event that ends the step adds the factor 1/k of its own clock */
+            const double W_old = W;
+            W *= exp(((kAw - 1.0) * o->kA[k] + (kSw - 1.0) * o->kS[k]) * rho * l_e);
+            if (event && !forced) W /= absorb ? kAw : kSw;
+            ta->sums[D_REWEIGHT] += (W - W_old) * e;
+        }
         if (!event) {
             if (cross_boundary(o->rb, N, &i, &r, &mu, b2, inward, &crossings)) {
                 /* L87 last sentence: the package leaves the model volume */
@@ -549,12 +580,15 @@ static void follow_package(const oracle_model* o, const run_opts* opt, tallies* 
  * to n_run visits every id once -- used by the order-independence pin). Tallies accumulate. */
 int dies_oracle_run(const oracle_model* o, uint64_t n_total, uint64_t first_id, uint64_t n_run, uint64_t id_stride,
                     uint64_t seed, uint32_t model_index, double k_bg, int ffi, int mode,
+                    const double* kA_w, double kS_w,
                     double* absorbed, double* escaped, double* reemit, double* pathlen,
                     uint64_t* counters, double* sums)
 {
     if (!o || !(o->has_ext || o->has_point) || n_total == 0) return -4;
-    if (!(k_bg > 0.0)) return -1;
-    run_opts opt = { n_total, seed, model_index, k_bg, ffi, mode };
+    if (!(k_bg > 0.0) || !(kS_w > 0.0)) return -1;
+    if (kA_w) for (int i = 0; i < o->N; i++) if (!(kA_w[i] > 0.0)) return -1;
+    if (ffi && (kA_w || kS_w != 1.0)) return -1;             /* alternatives in the paper (Fig. 7), not combined */
+    run_opts opt = { n_total, seed, model_index, k_bg, ffi, mode, kA_w, kS_w };
     tallies ta = { absorbed, escaped, reemit, pathlen, counters, sums };
     for (uint64_t j = 0; j < n_run; j++) {
         uint64_t p = first_id + (uint64_t)(((unsigned __int128)j * id_stride) % n_run);
@@ -565,11 +599,13 @@ int dies_oracle_run(const oracle_model* o, uint64_t n_total, uint64_t first_id, 
 
 /* Replay one package against the given tallies (not modified) and list its events. */
 int dies_oracle_trace(const oracle_model* o, uint64_t n_total, uint64_t package_id, uint64_t seed,
-                      uint32_t model_index, double k_bg, int ffi, int mode, const double* absorbed_state,
+                      uint32_t model_index, double k_bg, int ffi, int mode, const double* kA_w, double kS_w,
+                      const double* absorbed_state,
                       int32_t* events, int max_events, int* n_events, double* min_margin)
 {
     if (!o || !(o->has_ext || o->has_point) || n_total == 0) return -4;
-    run_opts opt = { n_total, seed, model_index, k_bg, ffi, mode };
+    if (ffi && (kA_w || kS_w != 1.0)) return -1;
+    run_opts opt = { n_total, seed, model_index, k_bg, ffi, mode, kA_w, kS_w };
     double* absorbed = (double*)calloc(o->N, sizeof(double));
     double* escaped = (double*)calloc(o->K, sizeof(double));
     if (absorbed_state) memcpy(absorbed, absorbed_state, o->N * sizeof(double));

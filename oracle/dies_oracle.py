@@ -20,7 +20,7 @@ _vp = C.c_void_p
 
 COUNTER_NAMES = ("packages", "crossings", "ffi_crossings", "scatterings", "absorptions", "escaped",
                  "uninteracted", "terminated", "extra_blocks", "clamp_hi_samples")
-SUM_NAMES = ("injected", "escaped", "uninteracted", "terminated")
+SUM_NAMES = ("injected", "escaped", "uninteracted", "terminated", "reweight")
 EVENT_NAMES = {0: "launch", 1: "scatter", 2: "absorb", 3: "escape", 4: "terminate", 5: "uninteracted"}
 
 _lib.dies_oracle_create.restype = _vp
@@ -31,9 +31,10 @@ _lib.dies_oracle_set_fixed_temperature.argtypes = [_vp, _dp]
 _lib.dies_oracle_temperature.argtypes = [_vp, _dp, _dp, C.POINTER(C.c_int), C.POINTER(C.c_int)]
 _lib.dies_oracle_get_tables.argtypes = [_vp, _dp, _dp, _dp]
 _lib.dies_oracle_run.argtypes = [_vp, _u64, _u64, _u64, _u64, _u64, C.c_uint32, C.c_double, C.c_int, C.c_int,
-                                 _dp, _dp, _dp, _dp, C.POINTER(_u64), _dp]
-_lib.dies_oracle_trace.argtypes = [_vp, _u64, _u64, _u64, C.c_uint32, C.c_double, C.c_int, C.c_int, _dp,
-                                   C.POINTER(C.c_int32), C.c_int, C.POINTER(C.c_int), _dp]
+                                 _dp, C.c_double, _dp, _dp, _dp, _dp, C.POINTER(_u64), _dp]
+_lib.dies_oracle_trace.argtypes = [_vp, _u64, _u64, _u64, C.c_uint32, C.c_double, C.c_int, C.c_int, _dp, C.c_double,
+                                   _dp, C.POINTER(C.c_int32), C.c_int, C.POINTER(C.c_int), _dp]
+_lib.dies_oracle_kA_profile.argtypes = [_vp, C.c_double, C.c_double, _dp]
 _lib.dies_oracle_chord_walk.argtypes = [C.c_int, _dp, C.c_int, C.c_double, C.c_double, C.c_int,
                                         C.POINTER(C.c_int), _dp, C.POINTER(C.c_int)]
 _lib.dies_oracle_hg_cos.restype = C.c_double
@@ -132,12 +133,25 @@ class Oracle:
         _lib.dies_oracle_get_tables(self._h, _d(eps), _d(F), _d(mass))
         return eps, F, mass
 
-    def run(self, n_total, seed=1, k_bg=0.5, ffi=0, mode=0, first_id=0, n_run=None, id_stride=1, model_index=0):
+    def kA_profile(self, k_A=1.0, k_A_dilute=0.0):
+        """Per-shell k_A (L130): k_A at the highest density, k_A_dilute at the lowest (0: k_A everywhere)."""
+        k = np.zeros(self.N)
+        _lib.dies_oracle_kA_profile(self._h, float(k_A), float(k_A_dilute), _d(k))
+        return k
+
+    def _weights(self, k_A, k_A_dilute, k_S):
+        if k_A == 1.0 and k_A_dilute == 0.0:
+            return None
+        return self.kA_profile(k_A, k_A_dilute)
+
+    def run(self, n_total, seed=1, k_bg=0.5, ffi=0, mode=0, first_id=0, n_run=None, id_stride=1, model_index=0,
+            k_A=1.0, k_A_dilute=0.0, k_S=1.0):
         """Follow packages first_id..first_id+n_run-1; tallies accumulate until reset()."""
         if n_run is None:
             n_run = n_total * max(self.n_sources, 1) - first_id
+        kw = self._weights(k_A, k_A_dilute, k_S)
         rc = _lib.dies_oracle_run(self._h, n_total, first_id, n_run, id_stride, seed, model_index, k_bg, ffi, mode,
-                                  _d(self.absorbed), _d(self.escaped), _d(self.reemit), _d(self.pathlen),
+                                  _d(kw), float(k_S), _d(self.absorbed), _d(self.escaped), _d(self.reemit), _d(self.pathlen),
                                   self._counters.ctypes.data_as(C.POINTER(_u64)), _d(self._sums))
         if rc != 0:
             raise RuntimeError(f"dies_oracle_run failed: {rc}")
@@ -160,11 +174,13 @@ class Oracle:
         return T
 
     def trace(self, n_total, package_id, seed=1, k_bg=0.5, ffi=0, mode=1, model_index=0, absorbed_state=None,
-              max_events=4096):
+              max_events=4096, k_A=1.0, k_A_dilute=0.0, k_S=1.0):
         ev = np.zeros((max_events, 4), dtype=np.int32)
         n, margin = C.c_int(), C.c_double()
         st = _arr(absorbed_state)
-        rc = _lib.dies_oracle_trace(self._h, n_total, package_id, seed, model_index, k_bg, ffi, mode, _d(st),
+        kw = self._weights(k_A, k_A_dilute, k_S)
+        rc = _lib.dies_oracle_trace(self._h, n_total, package_id, seed, model_index, k_bg, ffi, mode, _d(kw),
+                                    float(k_S), _d(st),
                                     ev.ctypes.data_as(C.POINTER(C.c_int32)), max_events, C.byref(n), C.byref(margin))
         if rc != 0:
             raise RuntimeError(f"dies_oracle_trace failed: {rc}")
