@@ -56,8 +56,10 @@ enum { DIES_EV_LAUNCH = 0, DIES_EV_SCATTER = 1, DIES_EV_ABSORB = 2, DIES_EV_ESCA
 /* indices into the array filled by dies_get_counters */
 enum { DIES_C_PACKAGES = 0, DIES_C_CROSSINGS, DIES_C_FFI_CROSSINGS, DIES_C_SCATTERINGS, DIES_C_ABSORPTIONS,
        DIES_C_ESCAPED, DIES_C_UNINTERACTED, DIES_C_TERMINATED, DIES_C_EXTRA_BLOCKS, DIES_C_CLAMP_HI_SAMPLES,
-       DIES_C_INJECTED_RAW, DIES_C_ESCAPED_RAW, DIES_C_TERMINATED_RAW, DIES_C_T_CLAMP_LO, DIES_C_T_CLAMP_HI,
-       DIES_C_KERNEL_LAUNCHES, DIES_N_COUNTERS };
+       DIES_C_INJECTED_RAW, DIES_C_TERMINATED_RAW, DIES_C_REWEIGHT_RAW, DIES_C_ESCAPED_RAW, DIES_C_T_CLAMP_LO,
+       DIES_C_T_CLAMP_HI, DIES_C_KERNEL_LAUNCHES, DIES_N_COUNTERS };
+/* Raw (fixed-point) bookkeeping, exact in integers: INJECTED_RAW + REWEIGHT_RAW = ESCAPED_RAW + TERMINATED_RAW.
+ * REWEIGHT_RAW is the signed sum (two's complement) of the changes the free-path weights made to package quanta. */
 
 typedef struct {
     double   k_bg;        /* Eq. 5: mu = u^k_bg, W = 2 k_bg mu^(2-1/k_bg); 0.5 = unweighted (Eq. 2)          */
@@ -67,6 +69,13 @@ typedef struct {
     int32_t  fixed_shift; /* S: a package of weight W adds round(W 2^S) to the 64-bit tallies; 0 -> 24      */
     uint64_t n_total;     /* packages per source over the whole (possibly split) run; package energy is
                              L_source / n_total (L51).  0 -> n_packages of this call                        */
+    /* Free-path weighting (section 2.2.2, Eq. 8; R17): the absorption and scattering clocks run
+     * k_A and k_S times faster than the true optical depths, p'(tau) = k e^{-k tau}; the package weight follows
+     * W = e^{tau (k-1)} / k.  0 means 1 (unweighted).  Not combined with ffi (DIES_EINVAL).                        */
+    double   k_A;         /* absorption: everywhere, or at the highest density of the model if k_A_dilute > 0     */
+    double   k_A_dilute;  /* > 0: k_A depends on density (L130, L211): this value at the lowest density, k_A at the
+                             highest, linear in log(rho) between                                                  */
+    double   k_S;         /* scattering                                                                           */
 } dies_run_opts;
 
 /* Bytes of device workspace a model (n_models = 1) or a batch needs. */
@@ -107,7 +116,7 @@ int dies_set_sources_batch(dies_model*, const double* ext_bin_intensity, const d
                            const double* point_bin_weights);
 
 /* Follow n_packages packages per active source (per model) on `cuda_stream` (a cudaStream_t; NULL = default
- * stream).  Asynchronous: returns after the launches.  opts == NULL means {0.5, 0, IRE, 0, 24, n_packages}. */
+ * stream).  Asynchronous: returns after the launches.  opts == NULL means {0.5, 0, IRE, 0, 24, n_packages, 1, 0, 1}. */
 int dies_run(dies_model*, uint64_t n_packages, uint64_t seed, const dies_run_opts* opts, void* cuda_stream);
 int dies_run_batch(dies_model*, uint64_t n_packages_per_model, uint64_t seed, const dies_run_opts* opts,
                    void* cuda_stream);

@@ -17,8 +17,8 @@ LIB_PATH = os.path.join(HERE, "libdies.so")
 DIES_OK, DIES_EINVAL, DIES_ENOMEM, DIES_ECUDA, DIES_ESTATE, DIES_EOVERFLOW = 0, -1, -2, -3, -4, -5
 DIES_MODE_IRE, DIES_MODE_FIXED_T = 0, 1
 COUNTER_NAMES = ("packages", "crossings", "ffi_crossings", "scatterings", "absorptions", "escaped", "uninteracted",
-                 "terminated", "extra_blocks", "clamp_hi_samples", "injected_raw", "escaped_raw", "terminated_raw",
-                 "T_clamp_lo", "T_clamp_hi", "kernel_launches")
+                 "terminated", "extra_blocks", "clamp_hi_samples", "injected_raw", "terminated_raw", "reweight_raw",
+                 "escaped_raw", "T_clamp_lo", "T_clamp_hi", "kernel_launches")
 DIES_N_COUNTERS = len(COUNTER_NAMES)
 EXPORTS = ("dies_workspace_bytes", "dies_create_model", "dies_create_batch", "dies_set_sources",
            "dies_set_sources_batch", "dies_run", "dies_run_batch", "dies_get_temperature", "dies_get_escape_spectrum",
@@ -35,7 +35,8 @@ class DiesError(RuntimeError):
 
 class dies_run_opts(C.Structure):
     _fields_ = [("k_bg", C.c_double), ("ffi", C.c_int32), ("mode", C.c_int32), ("accumulate", C.c_int32),
-                ("fixed_shift", C.c_int32), ("n_total", C.c_uint64)]
+                ("fixed_shift", C.c_int32), ("n_total", C.c_uint64), ("k_A", C.c_double),
+                ("k_A_dilute", C.c_double), ("k_S", C.c_double)]
 
 
 _dp = C.POINTER(C.c_double)
@@ -125,8 +126,10 @@ def dies_test_philox(seed, first_id, block, model_index, n):
     return w, u
 
 
-def _opts(k_bg=0.5, ffi=0, mode=DIES_MODE_IRE, accumulate=0, fixed_shift=24, n_total=0):
-    return dies_run_opts(float(k_bg), int(ffi), int(mode), int(accumulate), int(fixed_shift), int(n_total))
+def _opts(k_bg=0.5, ffi=0, mode=DIES_MODE_IRE, accumulate=0, fixed_shift=24, n_total=0, k_A=1.0, k_A_dilute=0.0,
+          k_S=1.0):
+    return dies_run_opts(float(k_bg), int(ffi), int(mode), int(accumulate), int(fixed_shift), int(n_total),
+                         float(k_A), float(k_A_dilute), float(k_S))
 
 
 class Model:
@@ -222,7 +225,10 @@ class Model:
     def dies_get_counters(self):
         c = np.zeros(DIES_N_COUNTERS, dtype=np.uint64)
         _chk(lib().dies_get_counters(self._h, c.ctypes.data_as(C.POINTER(C.c_uint64)), c.size))
-        return {n: int(v) for n, v in zip(COUNTER_NAMES, c)}
+        d = {n: int(v) for n, v in zip(COUNTER_NAMES, c)}
+        if d["reweight_raw"] >= 1 << 63:                      # signed sum in two's complement
+            d["reweight_raw"] -= 1 << 64
+        return d
 
     def dies_get_tables(self):
         eps = np.zeros(self.nT)

@@ -32,7 +32,7 @@ extern "C" const char* dies_last_error(void) { return g_err; }
 
 // ------------------------------------------------------------------ workspace layout
 struct Layout {
-    size_t emis, eps, Tgrid, epsgrid, F, guideF, guideS, bintab, omega, dustin, rb, rho, mass, stab, cscale, srccdf, srcin, Lsrc, mp,
+    size_t emis, eps, Tgrid, epsgrid, F, guideF, guideS, stabW, bintab, omega, dustin, rb, rho, mass, stab, cscale, srccdf, srcin, Lsrc, mp,
         fixed_row, Tfix, A, esc, next_id, counters, ticket, T_out, Lesc_out, eunit, flags, epsref, total;
 };
 static size_t al(size_t x) { return (x + 255) & ~(size_t)255; }
@@ -49,6 +49,7 @@ static Layout make_layout(int N, int K, int nT, int M)
     L.F = take((size_t)nT * K * 4);
     L.guideF = take((size_t)nT * kGuide * 2);
     L.guideS = take((size_t)M * 2 * kGuide * 2);
+    L.stabW = take((size_t)M * 2 * (ldS + 1) * 16);
     L.bintab = take((size_t)K * 16);
     L.omega = take((size_t)K * 4);
     L.dustin = take((size_t)3 * K * 8);
@@ -90,6 +91,7 @@ struct dies_model {
     cudaStream_t stream;
     int grid_max, blocks_per_sm, n_sms;
     int pool;                             // pool slots per warp of the tracker
+    double kref;                          // opacity unit of the device tables: max_k(kappa_abs + kappa_sca)
     size_t smem_bytes, smem_trace_bytes;
     unsigned long long launches;
 };
@@ -210,6 +212,51 @@ __global__ void k_build_shells(const double* __restrict__ rb, const double* __re
         }
         mass[(size_t)m * ldS + j] = ms;
     }
+}
+
+// Shell table of a run with free-path weighting (Eq. 8; R17): the same unfolded table with 16-byte entries
+// {(r/R)^2, +-rho^, k_A,i rho^, k_A,i}.  k_A,i is k_dense everywhere, or linear in log(rho) between k_dense at the
+// highest density of the model and k_dilute at the lowest (k_dilute > 0).
+__global__ void k_build_wshells(const double* __restrict__ rb, const double* __restrict__ rho, int N, int M, double kref,
+                                double k_dense, double k_dilute, float4* stabW)
+{
+    const int ldS = N + 1, ldT = 2 * ldS + 2;
+    const int idx = blockIdx.x * blockDim.x + threadIdx.x;
+    if (idx >= M * ldT) return;
+    const int m = idx / ldT, x = idx % ldT;
+    const double* r = rb + (size_t)m * (N + 1);
+    const double* d = rho + (size_t)m * N;
+    const double R = r[N];
+    const int cav = r[0] > 0.0 ? 1 : 0;
+    const int Np = N + cav;
+    double lo = 0.0, hi = 0.0; bool any = false;
+    for (int i = 0; i < N; i++) if (d[i] > 0.0) {
+        const double l = log(d[i]);
+        if (!any) { lo = hi = l; any = true; }
+        lo = fmin(lo, l); hi = fmax(hi, l);
+    }
+    auto radius = [&](int b) { return b == 0 ? 0.0 : r[b - cav]; };
+    auto dens = [&](int j) { const int i = j - cav; return (i < 0 || i >= N) ? 0.0 : d[i]; };
+    auto kA = [&](int j) {
+        const double dj = dens(j);
+        if (k_dilute > 0.0 && dj > 0.0 && hi > lo) return k_dense + (k_dilute - k_dense) * (hi - log(dj)) / (hi - lo);
+        return k_dense;
+    };
+    const int c = x - ldS, a = c < 0 ? -c : c;
+    float4 e = make_float4(4.0f, 0.0f, 0.0f, 1.0f);                     // never read
+    if (c <= 0 && a <= Np) {
+        const double rr = radius(a) / R;
+        const float dh = (float)(dens(a) * R * kref);
+        e = make_float4((float)(rr * rr), __int_as_float(__float_as_int(dh) | 0x80000000),
+                        (float)(kA(a) * dens(a) * R * kref), (float)kA(a));
+    } else if (c > 0 && c <= Np) {
+        const double rr = radius(c) / R;
+        e = make_float4((float)(rr * rr), (float)(dens(c - 1) * R * kref), (float)(kA(c - 1) * dens(c - 1) * R * kref),
+                        (float)kA(c - 1));
+    } else if (c == Np + 1) {
+        e = make_float4(-1.0f, 0.0f, 0.0f, 1.0f);                        // sentinel
+    }
+    stabW[(size_t)m * ldT + x] = e;
 }
 
 // source spectrum tables and luminosities: L_ext = 4 pi R^2 * pi * sum_k J_k
@@ -359,16 +406,18 @@ static int pool_slots(bool uniform_q)
     return (uniform_q ? env_int("DIES_POOL_U", 32, kMaxPool, 120) : env_int("DIES_POOL", 32, kMaxPool, 96)) & ~7;
 }
 
-static size_t tracker_smem(int N, int K, int nT, int P, bool trace, bool with_q)
+static size_t tracker_smem(int N, int K, int nT, int P, bool trace, bool with_q, bool wt = false)
 {
     const int ldS = N + 1, ldT = 2 * ldS + 2;
-    return plan_smem(K, nT, ldS, ldT, P, trace, with_q).total;
+    return plan_smem(K, nT, ldS, ldT, P, trace, with_q, wt).total;
 }
 
 template <int MODE, bool TRACE>
 static cudaError_t set_smem(size_t bytes)
 {
-    return cudaFuncSetAttribute(dies_track<MODE, TRACE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
+    cudaError_t e = cudaFuncSetAttribute(dies_track<MODE, TRACE, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
+    if (e != cudaSuccess) return e;
+    return cudaFuncSetAttribute(dies_track<MODE, TRACE, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
 }
 
 extern "C" int dies_workspace_bytes(int n_shells, int n_freq, int n_T, int n_models, size_t* bytes)
@@ -385,7 +434,7 @@ extern "C" int dies_device_info(int* n_sms, int* blocks_per_sm, int* threads_per
     int dev = 0, sms = 0, bps = 0;
     CUDA_TRY(cudaGetDevice(&dev));
     CUDA_TRY(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
-    CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&bps, dies_track<0, false>, kBlock, tracker_smem(100, 200, 1000, pool_slots(true), false, false)));
+    CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&bps, dies_track<0, false, false>, kBlock, tracker_smem(100, 200, 1000, pool_slots(true), false, false)));
     if (n_sms) *n_sms = sms;
     if (blocks_per_sm) *blocks_per_sm = bps;
     if (threads_per_block) *threads_per_block = kBlock;
@@ -431,7 +480,9 @@ extern "C" int dies_create_batch(int n_models, int n_shells, const double* r_bou
     size_t smem = tracker_smem(N, K, nT, pool, false, true);
     const size_t smem_u = tracker_smem(N, K, nT, pool_slots(true), false, false);
     if (smem_u > smem) smem = smem_u;                       // largest of the two launch shapes
-    const size_t smem_trace = tracker_smem(N, K, nT, pool, true, true);
+    const size_t smem_trace = tracker_smem(N, K, nT, pool, true, true, true);
+    const size_t smem_w = tracker_smem(N, K, nT, pool, false, true, true);
+    if (smem_w > smem) smem = smem_w;
     if (smem_trace > 200 * 1024) return fail(DIES_EINVAL, "tables do not fit in shared memory (%zu bytes)", smem_trace);
 
     dies_model* m = new (std::nothrow) dies_model();
@@ -441,12 +492,12 @@ extern "C" int dies_create_batch(int n_models, int n_shells, const double* r_bou
     m->sources_set = m->fixed_set = m->ran = false;
     m->done = m->n_total = 0; m->shift = 24; m->stream = 0; m->launches = 0;
     m->L_ext.assign(M, 0.0); m->L_point.assign(M, 0.0); m->has_ext.assign(M, 0); m->has_point.assign(M, 0);
-    m->smem_bytes = smem; m->smem_trace_bytes = smem_trace; m->pool = pool;
+    m->smem_bytes = smem; m->smem_trace_bytes = smem_trace; m->pool = pool; m->kref = kref;
     DeviceModel& D = m->D;
     D.N = N; D.K = K; D.nT = nT; D.n_models = M; D.ldS = N + 1; D.ldT = 2 * (N + 1) + 2;
     D.bintab = wsp<float4>(m, L.bintab); D.omega = wsp<float>(m, L.omega); D.epsgrid = wsp<float>(m, L.epsgrid);
     D.F = wsp<float>(m, L.F); D.guideF = wsp<unsigned short>(m, L.guideF); D.guideS = wsp<unsigned short>(m, L.guideS);
-    D.stab = wsp<float2>(m, L.stab); D.cscale = wsp<double>(m, L.cscale);
+    D.stab = wsp<float2>(m, L.stab); D.stabW = wsp<float4>(m, L.stabW); D.cscale = wsp<double>(m, L.cscale);
     D.srccdf = wsp<float>(m, L.srccdf); D.mp = wsp<ModelParams>(m, L.mp); D.fixed_row = wsp<int>(m, L.fixed_row);
     D.A = wsp<unsigned long long>(m, L.A); D.esc = wsp<unsigned long long>(m, L.esc);
     D.next_id = wsp<unsigned long long>(m, L.next_id); D.counters = wsp<unsigned long long>(m, L.counters);
@@ -485,7 +536,7 @@ extern "C" int dies_create_batch(int n_models, int n_shells, const double* r_bou
     int dev = 0;
     TRY_OR_FREE(cudaGetDevice(&dev));
     TRY_OR_FREE(cudaDeviceGetAttribute(&m->n_sms, cudaDevAttrMultiProcessorCount, dev));
-    TRY_OR_FREE(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&m->blocks_per_sm, dies_track<0, false>, kBlock, smem));
+    TRY_OR_FREE(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&m->blocks_per_sm, dies_track<0, false, false>, kBlock, smem));
     if (m->blocks_per_sm < 1) { delete m; return fail(DIES_ECUDA, "tracker does not fit on an SM"); }
     m->grid_max = m->n_sms * m->blocks_per_sm;
 #undef TRY_OR_FREE
@@ -583,8 +634,13 @@ extern "C" int dies_set_fixed_temperature(dies_model* m, const double* T, int n)
 static int fill_run_params(dies_model* m, uint64_t n_packages, uint64_t seed, const dies_run_opts* o, RunParams* R,
                            int* mode, int* accumulate, int* shift, uint64_t* n_total)
 {
-    dies_run_opts d = {0.5, 0, DIES_MODE_IRE, 0, 24, 0};
+    dies_run_opts d = {0.5, 0, DIES_MODE_IRE, 0, 24, 0, 1.0, 0.0, 1.0};
     if (o) d = *o;
+    if (d.k_A == 0.0) d.k_A = 1.0;
+    if (d.k_S == 0.0) d.k_S = 1.0;
+    if (!(d.k_A > 0.0) || !(d.k_S > 0.0) || !(d.k_A_dilute >= 0.0)) return fail(DIES_EINVAL, "k_A, k_S must be > 0 and k_A_dilute >= 0");
+    const bool weighted = d.k_A != 1.0 || d.k_S != 1.0 || d.k_A_dilute > 0.0;
+    if (weighted && d.ffi) return fail(DIES_EINVAL, "free-path weighting and forced first interaction are alternatives, not combined");
     if (!(d.k_bg > 0.0) || d.k_bg > 1.0) return fail(DIES_EINVAL, "k_bg must be in (0, 1]");
     if (d.mode != DIES_MODE_IRE && d.mode != DIES_MODE_FIXED_T) return fail(DIES_EINVAL, "bad mode");
     if (d.fixed_shift == 0) d.fixed_shift = 24;
@@ -598,7 +654,9 @@ static int fill_run_params(dies_model* m, uint64_t n_packages, uint64_t seed, co
     R->key0 = (uint32_t)seed; R->key1 = (uint32_t)(seed >> 32);
     for (int r = 0; r < 10; r++) { R->rk[2 * r] = R->key0 + (uint32_t)r * 0x9E3779B9u; R->rk[2 * r + 1] = R->key1 + (uint32_t)r * 0xBB67AE85u; }
     R->k_bg = (float)d.k_bg; R->ffi = d.ffi ? 1 : 0;
-    R->uniform_q = (d.k_bg == 0.5 && !d.ffi && !two) ? 1 : 0;
+    R->uniform_q = (d.k_bg == 0.5 && !d.ffi && !two && !weighted) ? 1 : 0;
+    R->weighted = weighted ? 1 : 0;
+    R->k_S = (float)d.k_S; R->k_A = d.k_A; R->k_A_dilute = d.k_A_dilute;
     R->qscale = (float)(1u << d.fixed_shift);
     R->pool = pool_slots(R->uniform_q != 0);
     R->thr_hi = env_int("DIES_THR_HI", 1, 32, 20);
@@ -631,10 +689,12 @@ extern "C" int dies_run(dies_model* m, uint64_t n_packages, uint64_t seed, const
     m->n_total = n_total; m->shift = shift;
 
     // launch shape: shared memory of this run's pool, persistent blocks (as many as fit on an SM), fewer for tiny runs
-    const size_t smem_launch = tracker_smem(m->N, m->K, m->nT, R.pool, false, !R.uniform_q);
+    const bool wt = R.weighted != 0;
+    const size_t smem_launch = tracker_smem(m->N, m->K, m->nT, R.pool, false, !R.uniform_q, wt);
+    const void* kfun = mode == DIES_MODE_IRE ? (wt ? (const void*)dies_track<0, false, true> : (const void*)dies_track<0, false, false>)
+                                             : (wt ? (const void*)dies_track<1, false, true> : (const void*)dies_track<1, false, false>);
     int bps = 0;
-    if (mode == DIES_MODE_IRE) CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&bps, dies_track<0, false>, kBlock, smem_launch));
-    else CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&bps, dies_track<1, false>, kBlock, smem_launch));
+    CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&bps, kfun, kBlock, smem_launch));
     if (bps < 1) return fail(DIES_ECUDA, "tracker does not fit on an SM");
     const int grid_max = m->n_sms * bps;
     unsigned long long ids = 0;
@@ -651,8 +711,18 @@ extern "C" int dies_run(dies_model* m, uint64_t n_packages, uint64_t seed, const
                                                     wsp<double>(m, m->L.eunit), wsp<ModelParams>(m, m->L.mp),
                                                     (double)n_total, (double)R.qscale, accumulate ? 0 : 1);
     TraceParams tp = {0, 0, 0, nullptr, 0, nullptr, nullptr};
-    if (mode == DIES_MODE_IRE) dies_track<0, false><<<grid, kBlock, smem_launch, st>>>(m->D, R, tp);
-    else dies_track<1, false><<<grid, kBlock, smem_launch, st>>>(m->D, R, tp);
+    if (wt) {
+        // shell table with the weighting factors of this run
+        const int nw = m->M * (2 * m->ldS + 2);
+        k_build_wshells<<<(nw + 127) / 128, 128, 0, st>>>(wsp<double>(m, m->L.rb), wsp<double>(m, m->L.rho), m->N, m->M, m->kref,
+                                                       R.k_A, R.k_A_dilute, wsp<float4>(m, m->L.stabW));
+        m->launches += 1;
+        if (mode == DIES_MODE_IRE) dies_track<0, false, true><<<grid, kBlock, smem_launch, st>>>(m->D, R, tp);
+        else dies_track<1, false, true><<<grid, kBlock, smem_launch, st>>>(m->D, R, tp);
+    } else {
+        if (mode == DIES_MODE_IRE) dies_track<0, false, false><<<grid, kBlock, smem_launch, st>>>(m->D, R, tp);
+        else dies_track<1, false, false><<<grid, kBlock, smem_launch, st>>>(m->D, R, tp);
+    }
     m->launches += 2;
     CUDA_TRY(cudaGetLastError());
     m->done += n_packages;
@@ -672,8 +742,8 @@ static int finalize(dies_model* m)
     const int n = m->M * (m->K > m->N ? m->K : m->N);
     int* flags = wsp<int>(m, m->L.flags);
     CUDA_TRY(cudaMemsetAsync(flags, 0, 16, m->stream));
-    // the derived counters ESCAPED_RAW .. T_CLAMP_HI are recomputed by every finalisation
-    CUDA_TRY(cudaMemsetAsync(m->ws + m->L.counters + DIES_C_ESCAPED_RAW * 8, 0, 4 * 8, m->stream));
+    // the derived counters ESCAPED_RAW, T_CLAMP_LO, T_CLAMP_HI are recomputed by every finalisation
+    CUDA_TRY(cudaMemsetAsync(m->ws + m->L.counters + DIES_C_ESCAPED_RAW * 8, 0, 3 * 8, m->stream));
     k_finalize<<<(n + 255) / 256, 256, 0, m->stream>>>(m->D, wsp<double>(m, m->L.mass), wsp<double>(m, m->L.eunit),
                                                      wsp<double>(m, m->L.eps), wsp<double>(m, m->L.Tgrid),
                                                      wsp<ModelParams>(m, m->L.mp), wsp<double>(m, m->L.T_out),
@@ -788,8 +858,17 @@ extern "C" int dies_trace_packages(dies_model* m, int model_index, uint64_t firs
                       reinterpret_cast<unsigned long long*>(reinterpret_cast<unsigned char*>(d_n) + n_bytes - 8)};
     int grid = (count + kBlock - 1) / kBlock;
     if (grid > m->grid_max) grid = m->grid_max;
-    if (mode == DIES_MODE_IRE) dies_track<0, true><<<grid, kBlock, m->smem_trace_bytes>>>(m->D, R, tp);
-    else dies_track<1, true><<<grid, kBlock, m->smem_trace_bytes>>>(m->D, R, tp);
+    if (R.weighted) {
+        const int nw = m->M * (2 * m->ldS + 2);
+        k_build_wshells<<<(nw + 127) / 128, 128>>>(wsp<double>(m, m->L.rb), wsp<double>(m, m->L.rho), m->N, m->M, m->kref,
+                                                  R.k_A, R.k_A_dilute, wsp<float4>(m, m->L.stabW));
+        m->launches += 1;
+        if (mode == DIES_MODE_IRE) dies_track<0, true, true><<<grid, kBlock, m->smem_trace_bytes>>>(m->D, R, tp);
+        else dies_track<1, true, true><<<grid, kBlock, m->smem_trace_bytes>>>(m->D, R, tp);
+    } else {
+        if (mode == DIES_MODE_IRE) dies_track<0, true, false><<<grid, kBlock, m->smem_trace_bytes>>>(m->D, R, tp);
+        else dies_track<1, true, false><<<grid, kBlock, m->smem_trace_bytes>>>(m->D, R, tp);
+    }
     m->launches += 1;
     cudaError_t e = cudaDeviceSynchronize();
     if (e == cudaSuccess) e = cudaMemcpy(events, d_ev, (size_t)count * max_events * 16, cudaMemcpyDeviceToHost);

@@ -35,7 +35,7 @@ constexpr int kTallyStride = 32;     // 64-bit words between the absorbed-energy
 
 // event counters (same order as DIES_C_* in include/dies.h), accumulated per block in shared memory
 enum { LC_PACKAGES = 0, LC_CROSSINGS, LC_FFI_CROSSINGS, LC_SCATTERINGS, LC_ABSORPTIONS, LC_ESCAPED, LC_UNINTERACTED,
-       LC_TERMINATED, LC_EXTRA_BLOCKS, LC_CLAMP_HI, LC_INJECTED_RAW, LC_N };
+       LC_TERMINATED, LC_EXTRA_BLOCKS, LC_CLAMP_HI, LC_INJECTED_RAW, LC_TERMINATED_RAW, LC_REWEIGHT_RAW, LC_N };
 
 // per-slot flag word: frequency bin | type of the pending event | dry FFI flight | slot holds a package
 constexpr unsigned KF_K = 0xffffu, KF_EVABS = 1u << 16, KF_DRY = 1u << 17, KF_OCC = 1u << 18;
@@ -68,6 +68,7 @@ struct DeviceModel {
     const unsigned short* guideF;    // nT x kGuide: smallest k with F[t][k] > c / kGuide
     const unsigned short* guideS;    // n_models x 2 x kGuide: the same for the source CDFs
     const float2* stab;              // n_models x ldT unfolded shell table
+    const float4* stabW;             // the same for a run with free-path weighting: {r^2, +-rho^, k_A rho^, k_A}
     const double* cscale;            // n_models x ldS: eps^ per raw tally unit
     const float* srccdf;             // n_models x 2 x K: external, point
     const ModelParams* mp;           // n_models
@@ -80,14 +81,16 @@ struct DeviceModel {
 };
 
 // shared-memory plan of a block (byte offsets), used by the kernel and by the host to size the launch
-struct SmemPlan { unsigned bin, cs, tab, eps, omega, row, esc, A, poolA, poolB, poolQ, queues, trace, total; };
-__host__ __device__ inline SmemPlan plan_smem(int K, int nT, int ldS, int ldT, int P, bool trace, bool with_q)
+struct SmemPlan { unsigned bin, cs, tab, eps, omega, row, esc, A, poolA, poolB, poolQ, poolW, queues, trace, total; };
+__host__ __device__ inline SmemPlan plan_smem(int K, int nT, int ldS, int ldT, int P, bool trace, bool with_q,
+                                              bool wt = false)
 {
     SmemPlan p;
     unsigned o = 0;
     p.bin = o;   o += 16u * K;                       // float4 K
     p.cs = o;    o += 8u * ldS;                      // double ldS
-    p.tab = o;   o += 8u * ldT;                      // float2 ldT
+    p.cs = (p.cs + 15u) & ~15u; o = p.cs + 8u * ldS; o = (o + 15u) & ~15u;
+    p.tab = o;   o += (wt ? 16u : 8u) * ldT;         // float2 (float4 with free-path weighting) ldT
     p.eps = o;   o += 4u * nT;
     p.omega = o; o += 4u * K;
     p.row = o;   o += 4u * ldS;
@@ -97,6 +100,8 @@ __host__ __device__ inline SmemPlan plan_smem(int K, int nT, int ldS, int ldT, i
     p.poolA = o; o += 16u * kWarps * P;              // float4 {s, b2, col, pa}
     p.poolB = o; o += 16u * kWarps * P;              // uint4  {id lo, id hi, blk, flags}
     p.poolQ = o; if (with_q) o += 8u * kWarps * P;   // raw quantum of the package (not stored when all are equal)
+    o = (o + 15u) & ~15u;
+    p.poolW = o; if (wt) o += 16u * kWarps * P;      // float4 {colS, colA at the draw, colS at the draw, launch quantum}
     p.queues = o; o += (unsigned)(QT_N * kWarps * P);
     o = (o + 15u) & ~15u;
     p.trace = o; if (trace) o += 12u * kWarps * P;   // pkg, n_ev, crossings so far
@@ -113,6 +118,9 @@ struct RunParams {
     float k_bg;
     int ffi;
     int uniform_q;                   // all packages carry the same raw quantum (no k_bg, no FFI, one source)
+    int weighted;                    // free-path weighting (Eq. 8, R17): two clocks, package weights change in flight
+    float k_S;                       // scattering clock factor
+    double k_A, k_A_dilute;          // absorption clock factor(s) (host side: they go into stabW)
     float qscale;                    // 2^S
     int n_tickets, parts;            // tickets = n_models * parts
     int pool;                        // P: pool slots per warp (multiple of 8, 32 <= P <= kMaxPool)
@@ -194,6 +202,14 @@ __device__ __forceinline__ float2 lds_entry(unsigned a)
     return v;
 }
 
+// one 16-byte entry of the unfolded shell table of a run with free-path weighting
+__device__ __forceinline__ float4 lds_entry4(unsigned a)
+{
+    float4 v;
+    asm("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(a));
+    return v;
+}
+
 // the pool and the queues of a warp are addressed in the shared window directly (32-bit addresses, no generic pointers)
 __device__ __forceinline__ unsigned lds_u8(unsigned a)
 {
@@ -208,6 +224,7 @@ __device__ __forceinline__ unsigned lds_u32(unsigned a)
     asm volatile("ld.shared.u32 %0, [%1];" : "=r"(v) : "r"(a) : "memory");
     return v;
 }
+__device__ __forceinline__ void sts_u32(unsigned a, unsigned v) { asm volatile("st.shared.u32 [%0], %1;" :: "r"(a), "r"(v) : "memory"); }
 __device__ __forceinline__ float4 lds_f4(unsigned a)
 {
     float4 v;
@@ -297,12 +314,15 @@ __device__ __forceinline__ void record(const TraceParams& tp, int pkg, int& n_ev
 // MODE 0: full IRE (returning 64-bit atomics on the global shell tallies, row from eps_old/eps_new)
 // MODE 1: fixed temperature (row from fixed_row; tallies privatised in shared memory)
 // TRACE : replay tp.count packages of one model, tallies read-only, events recorded
-template <int MODE, bool TRACE>
+// WT    : free-path weighting (Eq. 8; R17): absorption and scattering clocks are kept
+//         apart (they run k_A,i and k_S times faster than the true optical depths), the package quantum follows Eq. 8
+template <int MODE, bool TRACE, bool WT>
 __global__ void __launch_bounds__(kBlock, kMinBlocks) dies_track(DeviceModel D, RunParams R, TraceParams tp)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const int K = D.K, nT = D.nT, ldS = D.ldS, ldT = D.ldT, P = R.pool;
-    const SmemPlan sp = plan_smem(K, nT, ldS, ldT, P, TRACE, !R.uniform_q);
+    const SmemPlan sp = plan_smem(K, nT, ldS, ldT, P, TRACE, !R.uniform_q, WT);
+    constexpr unsigned ES = WT ? 16u : 8u;           // bytes per entry of the unfolded shell table
     float4* const s_bin = reinterpret_cast<float4*>(smem_raw + sp.bin);             // K
     double* const s_cs = reinterpret_cast<double*>(smem_raw + sp.cs);               // ldS
     float2* const s_tab = reinterpret_cast<float2*>(smem_raw + sp.tab);             // ldT unfolded shell table
@@ -321,6 +341,7 @@ __global__ void __launch_bounds__(kBlock, kMinBlocks) dies_track(DeviceModel D, 
     const unsigned aA = sbase + sp.poolA + 16u * (unsigned)(wid * P);          // float4 {s, b2, col, pa} per slot
     const unsigned aB = sbase + sp.poolB + 16u * (unsigned)(wid * P);          // uint4 {id lo, id hi, blk, flags}
     const unsigned aQ = sbase + sp.poolQ + 8u * (unsigned)(wid * P);           // raw quantum
+    const unsigned aW = sbase + sp.poolW + 16u * (unsigned)(wid * P);          // WT: second clock and the draw
     const unsigned qA = sbase + sp.queues + (unsigned)(wid * QT_N * P);        // byte queues of pool slots
     const unsigned qS = qA + (unsigned)P, qL = qS + (unsigned)P, qR = qL + (unsigned)P;
     int* const pT = reinterpret_cast<int*>(smem_raw + sp.trace) + wid * 3 * P;      // TRACE only
@@ -348,7 +369,8 @@ __global__ void __launch_bounds__(kBlock, kMinBlocks) dies_track(DeviceModel D, 
         }
         const ModelParams mp = D.mp[m];
         const int Np = mp.Np;
-        for (int x = tid; x < ldT; x += kBlock) s_tab[x] = D.stab[(size_t)m * ldT + x];
+        if (WT) { for (int x = tid; x < ldT; x += kBlock) reinterpret_cast<float4*>(s_tab)[x] = D.stabW[(size_t)m * ldT + x]; }
+        else { for (int x = tid; x < ldT; x += kBlock) s_tab[x] = D.stab[(size_t)m * ldT + x]; }
         for (int x = tid; x < ldS; x += kBlock) {
             s_cs[x] = D.cscale[(size_t)m * ldS + x];
             s_row[x] = (MODE == 1) ? D.fixed_row[(size_t)m * ldS + x] : 0;
@@ -365,8 +387,8 @@ __global__ void __launch_bounds__(kBlock, kMinBlocks) dies_track(DeviceModel D, 
         const unsigned short* const g_srcguide = D.guideS + (size_t)m * 2 * kGuide;
         const unsigned long long n_ids = TRACE ? (unsigned long long)tp.count
                                                : R.n_run * (unsigned long long)(mp.has_ext + mp.has_point);
-        const unsigned tab0 = (unsigned)__cvta_generic_to_shared(s_tab) + 8u * (unsigned)ldS;   // address of entry c = 0
-        const unsigned pa_out = tab0 + 8u * (unsigned)(Np + 1);                     // the sentinel beyond the outer surface
+        const unsigned tab0 = (unsigned)__cvta_generic_to_shared(s_tab) + ES * (unsigned)ldS;   // address of entry c = 0
+        const unsigned pa_out = tab0 + ES * (unsigned)(Np + 1);                     // the sentinel beyond the outer surface
         // raw quantum when every package carries the same one
         const unsigned long long q_uni =
             (unsigned long long)__float2ll_rn((mp.has_ext ? mp.qs_ext : mp.qs_point) * R.qscale);
@@ -419,10 +441,44 @@ __global__ void __launch_bounds__(kBlock, kMinBlocks) dies_track(DeviceModel D, 
                 const bool dryend = issrc && (kf & KF_DRY);      // the dry FFI flight reached the far surface
                 const bool esc = issrc && !dryend && (kf & KF_OCC);
 
+                // (0) free-path weighting (Eq. 8, R17): the quantum the package carries at this event.  Along the
+                //     flight the true survival probability over the biased one is e^{kappa_A (CA - C)} for the
+                //     absorption clock and e^{kappa_S (k_S - 1) C} for the scattering clock (C: column traversed,
+                //     CA: the same weighted with k_A of every shell); the event that ended the flight adds 1/k.
+                float colS = 0.f, cA0 = 0.f, cS0 = 0.f, q0f = 0.f, off = 0.f;
+                if (WT) {
+                    if (type >= 0) { const float4 w4 = lds_f4(aW + 16u * slot); colS = w4.x; cA0 = w4.y; cS0 = w4.z; q0f = w4.w; }
+                    long long dq = 0;
+                    if (isev || esc) {
+                        const float4 bt = s_bin[k];
+                        // col, colS: the columns CA, C consumed up to the committed surface; cA0, cS0: where the clocks end
+                        float CA = col, C = colS, kdiv = 1.f;
+                        if (isev) {
+                            const float4 Ep = lds_entry4(pa - 16u);           // the passage that was committed last
+                            const float rho = fabsf(Ep.y), rhoA = Ep.z;
+                            off = isabs ? (cA0 - col) / rhoA : (cS0 - colS) / rho;   // <= 0: the site lies this far before it
+                            CA = fmaf(rhoA, off, col);
+                            C = fmaf(rho, off, colS);
+                            kdiv = isabs ? Ep.w : R.k_S;
+                        }
+                        const float kapA = bt.x < 3.0e38f ? 1.f / bt.x : 0.f, kapS = bt.y < 3.0e38f ? 1.f / bt.y : 0.f;
+                        const float lnW = fmaf(kapA, CA - C, kapS * (R.k_S - 1.f) * C);
+                        const unsigned long long qn =
+                            (unsigned long long)__double2ll_rn((double)q * (double)(expf(lnW) / kdiv));
+                        dq = (long long)qn - (long long)q;
+                        q = qn;
+                    }
+                    if (__ballot_sync(kFull, dq != 0)) {
+#pragma unroll
+                        for (int o = 16; o > 0; o >>= 1) dq += __shfl_xor_sync(kFull, dq, o);
+                        if (lane == 0) atomicAdd(&s_cnt[LC_REWEIGHT_RAW], (unsigned long long)dq);
+                    }
+                }
+
                 // (1) absorptions first: add the package's quantum to the shell tally, keep the old value (L87).
                 //     The returning atomic is issued here and its result is only needed after the Philox block.
                 // shell of the event: the one traversed on the way to the surface entry before pa, which was not reached
-                const int ci = (int)(pa - tab0) / 8 - 1;
+                const int ci = (int)(pa - tab0) / (int)ES - 1;
                 int j = ci <= 0 ? -ci : ci - 1;
                 const unsigned absmask = __ballot_sync(kFull, isabs);
                 unsigned long long old = 0;
@@ -567,12 +623,13 @@ __global__ void __launch_bounds__(kBlock, kMinBlocks) dies_track(DeviceModel D, 
                         if (launch) {
                             ncross = 0; n_ev = 0;
                             q = (unsigned long long)__float2ll_rn(w * (point ? mp.qs_point : mp.qs_ext) * R.qscale);
+                            q0f = (float)q;
                             record<TRACE>(tp, pkg, n_ev, 0 /*LAUNCH*/, j - mp.cav, k, 0);
                         }
                     } else {
                         // ---- the step is truncated where the column ran out (L85 / L87): the surface passage
                         //      before pa was committed with col < 0, so the site lies col / rho^ before it
-                        const float se = s + col / fabsf(lds_entry(pa - 8u).y);
+                        const float se = WT ? s + off : s + col / fabsf(lds_entry(pa - 8u).y);
                         re2 = fmaf(se, se, b2);
                         re = sqrtf(re2);
                         mu = 2.f * u1 - 1.f;             // re-emission: isotropic (L87)
@@ -615,13 +672,29 @@ __global__ void __launch_bounds__(kBlock, kMinBlocks) dies_track(DeviceModel D, 
                         // L85/L87; R7 tie -> absorption; R15 one column instead of two clocks
                         const float4 bt = s_bin[k];
                         const float cA_ = tauA * bt.x, cS_ = tauS * bt.y;
-                        ev_absorb = (cA_ <= cS_);
-                        col = fminf(cA_, cS_);
+                        if (WT) {
+                            // two clocks counting up from zero: absorption ends at cA0 of k_A-weighted column,
+                            // scattering at cS0 of plain column (its factor k_S sits in cS0)
+                            cA0 = cA_; cS0 = cS_ / R.k_S;
+                            col = 0.f; colS = 0.f;
+                        } else {
+                            ev_absorb = (cA_ <= cS_);
+                            col = fminf(cA_, cS_);
+                        }
+                    }
+                    // L119: a package whose weight fell by ten orders of magnitude is terminated (its quantum may also
+                    // have rounded to nothing at the resolution 2^-S of the tallies, R18)
+                    if (WT && isev && (q == 0ull || (float)q < 1e-10f * q0f)) {
+                        record<TRACE>(tp, pkg, n_ev, 4 /*TERMINATE*/, j - mp.cav, k, ncross);
+                        if (TRACE) tp.n_events[pkg] = n_ev;
+                        atomicAdd(&s_cnt[LC_TERMINATED], 1ull);
+                        if (q) atomicAdd(&s_cnt[LC_TERMINATED_RAW], q);
+                        fly = false; uninter = true;
                     }
                     // ---- next flight: from shell j towards its inner (s < 0) or outer surface
                     s = re * mu;
                     b2 = (atsrc && !point) ? b2src : re2 * (1.f - mu) * (1.f + mu);
-                    pa = tab0 + 8u * (unsigned)((s < 0.f) ? -j : j + 1);
+                    pa = tab0 + ES * (unsigned)((s < 0.f) ? -j : j + 1);
                 }
                 // ---- write the package back; flying packages join the ready queue, a slot whose package ended
                 //      without escaping through the sentinel (FFI, tau0 = 0) is free again; a slot that got no id dies
@@ -631,6 +704,7 @@ __global__ void __launch_bounds__(kBlock, kMinBlocks) dies_track(DeviceModel D, 
                     sts_f4(aA + 16u * slot, s, b2, col, __uint_as_float(pa));
                     sts_u4(aB + 16u * slot, (unsigned)id, (unsigned)(id >> 32), blk, nkf);
                     if (!R.uniform_q) sts_u64(aQ + 8u * slot, q);
+                    if (WT) sts_f4(aW + 16u * slot, colS, cA0, cS0, q0f);
                     if (TRACE) { pT[slot] = pkg; pT[P + slot] = n_ev; pT[2 * P + slot] = (int)ncross; }
                 }
                 if (!R.uniform_q) {
@@ -665,6 +739,113 @@ __global__ void __launch_bounds__(kBlock, kMinBlocks) dies_track(DeviceModel D, 
             // (units of 1/kappa_ref) to the next event, shared-memory address pa of the candidate surface passage
             // (entry E); (pa - pa0) / 8 counts the passages since the package was taken from the pool.
             // =====================================================================================
+            if (WT)
+            {
+                bool has = lane < nR;
+                unsigned slot = 0, pa = tab0;
+                // col: k_A-weighted column consumed (absorption clock, ends at cA0); colS: plain column (ends at cS0)
+                float s = 0.f, b2 = 0.f, col = 1.f, colS = 0.f, cA0 = 0.f, cS0 = 0.f;
+                if (has) {
+                    slot = lds_u8(qR + (nR - 1 - lane));
+                    const float4 a = lds_f4(aA + 16u * slot);
+                    s = a.x; b2 = a.y; col = a.z; pa = __float_as_uint(a.w);
+                    const float4 w4 = lds_f4(aW + 16u * slot);
+                    colS = w4.x; cA0 = w4.y; cS0 = w4.z;
+                }
+                nR -= min(nR, 32);
+                unsigned pa0 = pa;
+                float4 E = lds_entry4(pa);
+                bool alive = has;
+                for (;;) {
+                    const unsigned pb = pa;                      // the table is walked from here with constant offsets
+#pragma unroll
+                    for (int u = 0; u < kUnroll; u++) {
+                        const float d = E.x - b2;
+                        alive = alive && (d >= 0.f);
+                        if (alive) {
+                            // Eq. 4 for both clocks: absorption in k_A rho^, scattering in rho^ (its k_S sits in the draw)
+                            const float sn = __int_as_float(__float_as_int(sqrt_ftz(d)) | (__float_as_int(E.y) & 0x80000000));
+                            const float dl = sn - s;
+                            col = fmaf(E.z, dl, col);
+                            colS = fmaf(fabsf(E.y), dl, colS);
+                            s = sn;
+                            E = lds_entry4(pb + 16u * (u + 1));
+                            pa = pb + 16u * (u + 1);
+                        }
+                        alive = alive && (col <= cA0) && (colS <= cS0);
+                    }
+                    if (!alive && (col <= cA0) && (colS <= cS0)) {
+                        if (__float_as_int(E.y) < 0) {
+                            // the inner surface is not reached (tangent shell): head for the outer one instead
+                            // entry c -> entry 1 - c; the 1 - 2c entries skipped are no passages
+                            const unsigned np = 2u * tab0 + 16u - pa;
+                            pa0 += np - pa;
+                            pa = np;
+                            E = lds_entry4(pa);
+                            alive = true;
+                        } else if (pa != pa_out) {
+                            b2 = E.x;                                // outward, b2 > r^2 by rounding only: graze
+                            alive = true;
+                        }
+                    }
+                    const unsigned am = __ballot_sync(kFull, alive);
+                    const int n_alive = __popc(am);
+                    if (n_alive >= thr_hi) continue;
+                    const bool leave = (nR == 0);
+                    if (leave && n_alive >= thr_lo) continue;
+
+                    // ---- stopped packages (all of them when leaving) go back to the pool and into their queues
+                    const bool out = has && (leave || !alive);
+                    int t = -1;
+                    if (out) {
+                        const bool isev = !alive && ((col > cA0) || (colS > cS0));   // a clock ran out
+                        const unsigned n = ((pa - pa0) >> 4) - (isev ? 1u : 0u);
+                        lc_cross += n;
+                        if (TRACE) pT[2 * P + slot] += (int)n;
+                        sts_f4(aA + 16u * slot, s, b2, col, __uint_as_float(pa));
+                        sts_u32(aW + 16u * slot, __float_as_uint(colS));
+                        t = alive ? QT_READY : QT_SRC;
+                        if (isev) {
+                            // the clock that ran out first along the step decides (R7: a tie is an absorption):
+                            // distances back from the committed surface, (cA0 - col) / (k_A rho^) and (cS0 - colS) / rho^
+                            const float4 Ep = lds_entry4(pa - 16u);
+                            const float fA = col > cA0 ? (cA0 - col) / Ep.z : 3.0e38f;
+                            const float fS = colS > cS0 ? (cS0 - colS) / fabsf(Ep.y) : 3.0e38f;
+                            t = (fA <= fS) ? QT_ABS : QT_SCA;
+                        }
+                    }
+                    {
+                        // one store per leaving package: queue t at position (length of t) + (rank among the lanes of t)
+                        const unsigned mA = __ballot_sync(kFull, t == QT_ABS), mS = __ballot_sync(kFull, t == QT_SCA);
+                        const unsigned mL = __ballot_sync(kFull, t == QT_SRC), mR = __ballot_sync(kFull, t == QT_READY);
+                        const unsigned mine = t == QT_ABS ? mA : t == QT_SCA ? mS : t == QT_SRC ? mL : mR;
+                        const int base = t == QT_ABS ? nA : t == QT_SCA ? P + nS : t == QT_SRC ? 2 * P + nL : 3 * P + nR;
+                        if (out) sts_u8(qA + base + __popc(mine & lt_mask), slot);
+                        nA += __popc(mA); nS += __popc(mS); nL += __popc(mL); nR += __popc(mR);
+                    }
+                    __syncwarp();
+                    if (leave) break;
+                    // ---- idle lanes take the next ready packages
+                    const unsigned fm = ~am;
+                    const int r = __popc(fm & lt_mask);
+                    const bool take = !alive && (r < nR);
+                    if (take) {
+                        slot = lds_u8(qR + (nR - 1 - r));
+                        const float4 a = lds_f4(aA + 16u * slot);
+                        s = a.x; b2 = a.y; col = a.z; pa = __float_as_uint(a.w);
+                        const float4 w4 = lds_f4(aW + 16u * slot);
+                        colS = w4.x; cA0 = w4.y; cS0 = w4.z;
+                        pa0 = pa;
+                        E = lds_entry4(pa);
+                    } else if (!alive) {
+                        col = 1.f; cA0 = 0.f;                    // idle lane: never flies, never looks stopped short
+                    }
+                    has = alive || take;
+                    alive = has;
+                    nR -= min(nR, __popc(fm));
+                }
+            }
+            else
             {
                 bool has = lane < nR;
                 unsigned slot = 0, pa = tab0;

@@ -31,7 +31,8 @@ def test_run_opts_struct_layout():
     assert binding.dies_run_opts.k_bg.offset == 0 and binding.dies_run_opts.ffi.offset == 8
     assert binding.dies_run_opts.n_total.offset == 24
     import ctypes
-    assert ctypes.sizeof(binding.dies_run_opts) == 32
+    assert binding.dies_run_opts.k_A.offset == 32 and binding.dies_run_opts.k_S.offset == 48
+    assert ctypes.sizeof(binding.dies_run_opts) == 56
 
 
 def test_workspace_bytes_and_argument_errors(lib):

@@ -174,7 +174,7 @@ def _ire_stats(orc, p, n, seeds, model_kw=None, **kw):
         m.dies_run(n, seed=s, **kw)
         Tg.append(m.dies_get_temperature())
         c = m.dies_get_counters()
-        assert c["injected_raw"] == c["escaped_raw"] + c["terminated_raw"]      # exact conservation
+        assert c["injected_raw"] + c["reweight_raw"] == c["escaped_raw"] + c["terminated_raw"]   # exact conservation
         n_src = int(p.ext_bin_intensity is not None) + int(p.L_point > 0)
         assert c["packages"] == n * n_src == o.counters["packages"] and c["terminated"] == 0
         m.close()

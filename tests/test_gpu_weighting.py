@@ -1,0 +1,131 @@
+"""GPU parity of the free-path weighting k_A, k_S, k_A(rho) (section 2.2.2, Eq. 8; R17, R18) against
+the oracle, through the C ABI: bit-exact event lists on identical Philox streams, absorbed energy per shell in
+fixed-temperature mode, IRE temperatures over 8 seeds, exact integer bookkeeping, the weight guard (L119)."""
+import numpy as np
+import pytest
+
+from paper_2408_13807_b200 import binding as dies
+from paper_2408_13807_b200 import synth
+from test_gpu_parity import _check_T_parity, _fixed_T
+from test_oracle_pins import toy_problem
+
+pytestmark = pytest.mark.gpu
+
+VARIANTS = [dict(k_A=2.5), dict(k_S=0.6, k_A=1.5), dict(k_A=1.0, k_A_dilute=3.0), dict(k_A=1.2, k_A_dilute=2.0, k_S=1.8, k_bg=0.3)]
+
+
+@pytest.fixture(scope="module")
+def orc():
+    from oracle import dies_oracle as orc
+    return orc
+
+
+def _identity(c):
+    return c["injected_raw"] + c["reweight_raw"] == c["escaped_raw"] + c["terminated_raw"]
+
+
+@pytest.mark.parametrize("kw", VARIANTS)
+@pytest.mark.parametrize("cfg", ["config1", "config2s", "config3s"])
+def test_weighted_trace_bit_exact(orc, cfg, kw):
+    if cfg == "config1":
+        p = synth.config1()
+    elif cfg == "config3s":
+        p = synth.config3(n_shells=40, n_freq=64, tau_V=30.0)
+    else:
+        p = synth.config2(n_shells=50, n_freq=64)
+    n_total, count, max_ev = 100000, 2000, 512
+    o = orc.Oracle(p)
+    o.set_fixed_temperature(_fixed_T(p.n_shells))
+    m = dies.Model(p)
+    m.dies_set_fixed_temperature(_fixed_T(p.n_shells))
+    ev, nev = m.dies_trace_packages(0, count, n_total, seed=5, max_events=max_ev, mode=dies.DIES_MODE_FIXED_T, **kw)
+    safe = same = 0
+    for pid in range(count):
+        ref, nref, margin = o.trace(n_total, pid, seed=5, mode=1, max_events=max_ev, **kw)
+        ok = (nref == nev[pid]) and nref <= max_ev and np.array_equal(ref, ev[pid, :nref])
+        same += ok
+        if margin > 1e-3 and nref <= max_ev:
+            safe += 1
+            assert ok, (pid, margin, ref[:8], ev[pid, :8])
+    assert safe > 0.4 * count
+    assert same >= 0.99 * count, same / count
+    m.close()
+
+
+@pytest.mark.parametrize("kw", VARIANTS)
+def test_weighted_fixed_T_absorbed_energy(orc, kw):
+    """Identical streams, fixed temperatures: absorbed energy per shell within 1e-4 (or a few package quanta)."""
+    p = synth.config2(n_shells=40, n_freq=64, tau_V=3.0)        # centrally peaked density: k_A(rho) varies by shell
+    n = 400_000
+    o = orc.Oracle(p)
+    o.set_fixed_temperature(_fixed_T(p.n_shells))
+    o.run(n, seed=3, mode=1, **kw)
+    m = dies.Model(p)
+    m.dies_set_fixed_temperature(_fixed_T(p.n_shells))
+    m.dies_run(n, seed=3, mode=dies.DIES_MODE_FIXED_T, **kw)
+    raw, unit, energy = m.dies_get_absorbed()
+    c = m.dies_get_counters()
+    e_pkg = o.sums["injected"] / n
+    assert np.all(np.abs(energy - o.absorbed) <= np.maximum(1e-4 * o.absorbed, 5 * e_pkg)), \
+        np.max(np.abs(energy / o.absorbed - 1))
+    assert c["packages"] == n and c["terminated"] == 0 == o.counters["terminated"]
+    for k in ("crossings", "scatterings", "absorptions"):
+        assert abs(c[k] - o.counters[k]) <= 2e-4 * o.counters[k] + 3
+    assert _identity(c)
+    # the same identity in energy against the oracle's own sums
+    esc = m.dies_get_escape_spectrum().sum()
+    assert abs(esc / o.sums["escaped"] - 1) < 1e-4
+    assert abs(c["reweight_raw"] * unit - o.sums["reweight"]) < 2e-3 * abs(o.sums["reweight"]) + 1e-5 * o.sums["injected"]
+    m.close()
+
+
+@pytest.mark.parametrize("kw", [dict(k_A=1.0, k_A_dilute=3.0), dict(k_S=2.0, k_A=0.7)])
+def test_weighted_full_ire_temperature(orc, kw):
+    p = synth.config2(n_shells=40, n_freq=64, tau_V=3.0)
+    _check_T_parity(orc, p, 100_000, **kw)
+
+
+def test_weighted_thin_sphere_matches_the_plain_method(orc):
+    """Config 4 reduced (tau_V = 0.01): k_A(rho) up to 3 against the oracle WITHOUT weighting: same T within noise."""
+    p = synth.config4(n_shells=20)
+    n = 2_000_000
+    m = dies.Model(p)
+    T = []
+    for s in range(1, 5):
+        m.dies_run(n, seed=s, k_A=3.0)
+        T.append(m.dies_get_temperature())
+        assert _identity(m.dies_get_counters())
+    T = np.array(T)
+    To = np.array([orc.Oracle(p).run(400_000, seed=s, ffi=1).temperature() for s in range(1, 5)])
+    se = np.sqrt(T.var(0, ddof=1) / 4 + To.var(0, ddof=1) / 4)
+    assert np.all(np.abs(T.mean(0) - To.mean(0))[4:] < np.maximum(0.01 * To.mean(0), 4 * se)[4:])
+    m.close()
+
+
+def test_weight_guard_and_bookkeeping(orc):
+    p = toy_problem(n_shells=4, tau=20.0, kappa_sca=9.0, g=0.0)
+    n = 20000
+    m = dies.Model(p)
+    m.dies_run(n, seed=2, k_S=10.0)
+    c = m.dies_get_counters()
+    o = orc.Oracle(p).run(n, seed=2, k_S=10.0)
+    assert c["packages"] == n == c["escaped"] + c["terminated"]
+    # the GPU terminates at the tally resolution 2^-24 (R18), the oracle at 1e-10: both terminate most packages
+    assert c["terminated"] > 0.5 * o.counters["terminated"] > 0
+    assert _identity(c)
+    assert c["terminated_raw"] < 1e-6 * c["injected_raw"]
+    m.close()
+
+
+def test_weighting_argument_errors():
+    m = dies.Model(synth.config1())
+    with pytest.raises(dies.DiesError) as e:
+        m.dies_run(100, ffi=1, k_A=2.0)
+    assert e.value.code == dies.DIES_EINVAL
+    with pytest.raises(dies.DiesError) as e:
+        m.dies_run(100, k_S=-1.0)
+    assert e.value.code == dies.DIES_EINVAL
+    m.dies_run(1000, k_A=1.0, k_S=1.0)            # unit factors: the plain kernel
+    c = m.dies_get_counters()
+    assert c["reweight_raw"] == 0 and c["injected_raw"] == c["escaped_raw"]
+    m.close()
