@@ -359,7 +359,16 @@ typedef struct {
     int mode;                /* 0 = full IRE, 1 = fixed temperature */
     const double* kA_w;      /* N or NULL: free-path weighting factor k_A of each shell (Eq. 8; L130: may depend on density) */
     double kS_w;             /* free-path weighting factor k_S (Eq. 8); 1 = unweighted */
+    double g_E;              /* Eq. 6: re-emission directions from a Henyey-Greenstein function; 0 = isotropic (unweighted) */
+    double g_S;              /* Eq. 7: scattering directions from HG(g_S) about the radial reference direction */
+    int use_gS;              /* Eq. 7 is active (g_S = 0 is NOT the plain method, L207) */
 } run_opts;
+
+/* Henyey-Greenstein density of a direction cosine, Eq. 6: p(mu) = (1/2)(1-g^2)/(1+g^2-2 g mu)^{3/2} */
+double dies_oracle_hg_pdf(double g, double mu)
+{
+    return 0.5 * (1.0 - g * g) / pow(1.0 + g * g - 2.0 * g * mu, 1.5);
+}
 
 /* Density-dependent k_A: linear in the logarithm of the density, k_dilute at the lowest
  * density of the model and k_dense at the highest (3.0 and 1.0 in the paper's test); shells without dust get
@@ -525,6 +534,22 @@ static void follow_package(const oracle_model* o, const run_opts* opt, tallies* 
         if (!absorb) {
             /* L85: scatter with the dust scattering function, redraw both free paths */
             draw_block(&s, u);
+            if (opt->use_gS) {
+                /* L112-117, Eq. 7 (garbled as printed; reading R19): the new direction is drawn from HG(g_S) about
+                 * the radial reference direction (towards the centre for the external field, away from it for the
+                 * central source, L109), with a uniform azimuth about that axis; the weight is the ratio of the
+                 * dust's HG density at the true scattering angle to the sampling density */
+                const double mup = dies_oracle_hg_cos(opt->g_S, u[0]);
+                const double phi = 2.0 * PI * u[1];
+                const double mu1 = src_is_point ? mup : -mup;
+                double ct = mu * mu1 + sqrt(fmax(1.0 - mu * mu, 0.0)) * sqrt(fmax(1.0 - mu1 * mu1, 0.0)) * cos(phi);
+                if (ct > 1.0) ct = 1.0;
+                if (ct < -1.0) ct = -1.0;
+                const double W_old = W;
+                W *= dies_oracle_hg_pdf(o->g[k], ct) / dies_oracle_hg_pdf(opt->g_S, mup);
+                ta->sums[D_REWEIGHT] += (W - W_old) * e;
+                mu = mu1;
+            } else {
             double ct = dies_oracle_hg_cos(o->g[k], u[0]);
             double phi = 2.0 * PI * u[1];
             double st = sqrt(fmax(1.0 - ct * ct, 0.0));
@@ -532,6 +557,7 @@ static void follow_package(const oracle_model* o, const run_opts* opt, tallies* 
             mu = mu * ct + sm * st * cos(phi);
             if (mu > 1.0) mu = 1.0;
             if (mu < -1.0) mu = -1.0;
+            }
             tauS = -log(u[2]);
             tauA = -log(u[3]);
             ta->counters[C_SCATTERINGS] += 1;
@@ -560,6 +586,15 @@ static void follow_package(const oracle_model* o, const run_opts* opt, tallies* 
             draw_block(&s, u);
             k = sample_cdf(o->F + (size_t)t * K, K, u[0], rec);
             mu = 2.0 * u[1] - 1.0;
+            if (opt->g_E != 0.0) {
+                /* L105-110, Eq. 6: HG(g_E) instead of isotropic, measured from the direction towards the centre
+                 * (external field) or away from it (central source); weight = isotropic density / HG density */
+                const double mup = dies_oracle_hg_cos(opt->g_E, u[1]);
+                const double W_old = W;
+                W *= 0.5 / dies_oracle_hg_pdf(opt->g_E, mup);
+                ta->sums[D_REWEIGHT] += (W - W_old) * e;
+                mu = src_is_point ? mup : -mup;
+            }
             tauS = -log(u[2]);
             tauA = -log(u[3]);
             if (ta->reemit) ta->reemit[(size_t)i * K + k] += W * e;
@@ -582,7 +617,7 @@ static void follow_package(const oracle_model* o, const run_opts* opt, tallies* 
  * to n_run visits every id once -- used by the order-independence pin). Tallies accumulate. */
 int dies_oracle_run(const oracle_model* o, uint64_t n_total, uint64_t first_id, uint64_t n_run, uint64_t id_stride,
                     uint64_t seed, uint32_t model_index, double k_bg, int ffi, int mode,
-                    const double* kA_w, double kS_w,
+                    const double* kA_w, double kS_w, double g_E, double g_S, int use_gS,
                     double* absorbed, double* escaped, double* reemit, double* pathlen,
                     uint64_t* counters, double* sums)
 {
@@ -590,7 +625,8 @@ int dies_oracle_run(const oracle_model* o, uint64_t n_total, uint64_t first_id, 
     if (!(k_bg > 0.0) || !(kS_w > 0.0)) return -1;
     if (kA_w) for (int i = 0; i < o->N; i++) if (!(kA_w[i] > 0.0)) return -1;
     if (ffi && (kA_w || kS_w != 1.0)) return -1;             /* alternatives in the paper (Fig. 7), not combined */
-    run_opts opt = { n_total, seed, model_index, k_bg, ffi, mode, kA_w, kS_w };
+    if (!(fabs(g_E) < 1.0) || !(fabs(g_S) < 1.0)) return -1;
+    run_opts opt = { n_total, seed, model_index, k_bg, ffi, mode, kA_w, kS_w, g_E, g_S, use_gS };
     tallies ta = { absorbed, escaped, reemit, pathlen, counters, sums };
     for (uint64_t j = 0; j < n_run; j++) {
         uint64_t p = first_id + (uint64_t)(((unsigned __int128)j * id_stride) % n_run);
@@ -602,12 +638,12 @@ int dies_oracle_run(const oracle_model* o, uint64_t n_total, uint64_t first_id, 
 /* Replay one package against the given tallies (not modified) and list its events. */
 int dies_oracle_trace(const oracle_model* o, uint64_t n_total, uint64_t package_id, uint64_t seed,
                       uint32_t model_index, double k_bg, int ffi, int mode, const double* kA_w, double kS_w,
-                      const double* absorbed_state,
+                      double g_E, double g_S, int use_gS, const double* absorbed_state,
                       int32_t* events, int max_events, int* n_events, double* min_margin)
 {
     if (!o || !(o->has_ext || o->has_point) || n_total == 0) return -4;
     if (ffi && (kA_w || kS_w != 1.0)) return -1;
-    run_opts opt = { n_total, seed, model_index, k_bg, ffi, mode, kA_w, kS_w };
+    run_opts opt = { n_total, seed, model_index, k_bg, ffi, mode, kA_w, kS_w, g_E, g_S, use_gS };
     double* absorbed = (double*)calloc(o->N, sizeof(double));
     double* escaped = (double*)calloc(o->K, sizeof(double));
     if (absorbed_state) memcpy(absorbed, absorbed_state, o->N * sizeof(double));

@@ -99,3 +99,60 @@ def test_weight_guard_terminates_trapped_packages():
 def test_ffi_and_free_path_weighting_are_not_combined():
     with pytest.raises(RuntimeError):
         orc.Oracle(synth.config1()).run(100, seed=1, ffi=1, k_A=2.0)
+
+
+# ------------------------------------------------------------------ directional weighting (Eq. 6-7; R19)
+@pytest.mark.parametrize("g", [0.5, -0.4, 0.8])
+def test_hg_density_and_reemission_weight(g):
+    """Eq. 6 integrates to 1 over mu in [-1,1]; sampling mu' from HG(g_E) with the weight (1/2) / p(mu') reproduces
+    the isotropic distribution: mean weight 1 and a flat weighted histogram of mu'."""
+    lib = orc._lib
+    mu = np.linspace(-1, 1, 20001)
+    p = np.array([lib.dies_oracle_hg_pdf(g, x) for x in mu])
+    assert abs(np.sum(0.5 * (p[1:] + p[:-1]) * np.diff(mu)) - 1.0) < 1e-4       # trapezoid rule
+    rng = np.random.default_rng(1)
+    u = rng.random(200000)
+    mup = np.array([lib.dies_oracle_hg_cos(g, x) for x in u])
+    w = 0.5 / np.array([lib.dies_oracle_hg_pdf(g, x) for x in mup])
+    assert abs(w.mean() - 1.0) < 5 * w.std() / math.sqrt(u.size)
+    h, _ = np.histogram(mup, bins=10, range=(-1, 1), weights=w)
+    assert np.max(np.abs(h / h.mean() - 1)) < 0.05
+
+
+def test_scattering_direction_weight_is_unbiased():
+    """Absorbed energy per shell with the dust's own scattering function (g = 0.5) equals the one obtained when the
+    scattering directions are drawn from HG(g_S) about the radial direction and reweighted by Eq. 7."""
+    p = toy_problem(n_shells=6, tau=2.0, kappa_sca=1.0, g=0.5, rho_shape=[4, 3, 2, 1.5, 1, 0.5])
+    n = 300000
+    runs = []
+    for kw in ({}, dict(g_S=0.3), dict(g_S=0.0), dict(g_S=-0.3)):
+        tot = []
+        for seed in range(1, 5):
+            o = orc.Oracle(p).run(n, seed=seed, **kw)
+            tot.append(o.absorbed / o.sums["injected"])
+            s = o.sums
+            assert abs(s["injected"] + s["reweight"] - s["escaped"] - s["terminated"]) < 1e-9 * s["injected"]
+        runs.append(np.array(tot))
+    ref = runs[0]
+    for r in runs[1:]:
+        se = np.sqrt(ref.var(0, ddof=1) / 4 + r.var(0, ddof=1) / 4)
+        assert np.all(np.abs(r.mean(0) - ref.mean(0)) < 5 * se + 1e-4), (r.mean(0) / ref.mean(0))
+    # g_S = 0 is a weighting (isotropic sampling), not the plain run (L207): different realisations
+    assert not np.array_equal(runs[0][0], runs[2][0])
+
+
+def test_reemission_direction_weight_leaves_temperatures_unchanged():
+    """Full IRE on config 1 at tau_V = 3 (re-emitted packages are re-absorbed): T(r) with g_E = 0.5 and -0.5 equals
+    the unweighted T(r) within the combined errors of 6 seeds."""
+    p = synth.config1(tau_V=3.0)
+    n = 60000
+    T = {}
+    for g in (0.0, 0.5, -0.5):
+        T[g] = np.array([orc.Oracle(p).run(n, seed=s, g_E=g).temperature() for s in range(1, 7)])
+    for g in (0.5, -0.5):
+        se = np.sqrt(T[0.0].var(0, ddof=1) / 6 + T[g].var(0, ddof=1) / 6)
+        d = np.abs(T[g].mean(0) - T[0.0].mean(0))
+        assert np.sum(d > np.maximum(0.01 * T[0.0].mean(0), 3.5 * se)) <= 1, d / se
+    a = orc.Oracle(p).run(5000, seed=1)
+    b = orc.Oracle(p).run(5000, seed=1, g_E=0.0)
+    assert np.array_equal(a.absorbed, b.absorbed)         # g_E = 0 is the plain method
