@@ -76,6 +76,15 @@ typedef struct {
     double   k_A_dilute;  /* > 0: k_A depends on density (L130, L211): this value at the lowest density, k_A at the
                              highest, linear in log(rho) between                                                  */
     double   k_S;         /* scattering                                                                           */
+    /* Directional weighting (section 2.2.1, Eq. 6-7; R19).  Angles are measured from the direction
+     * towards the model centre for packages of the external field and away from it for those of the central source.
+     * Not combined with ffi (DIES_EINVAL).                                                                          */
+    double   g_E;         /* re-emission directions from a Henyey-Greenstein function HG(g_E) instead of isotropic,
+                             weight (1/2) / p_HG; 0 = isotropic (the plain method), |g_E| < 1                      */
+    double   g_S;         /* scattering directions from HG(g_S) about that radial direction, weight = dust HG density
+                             at the true scattering angle / p_HG(g_S); only if use_g_S != 0, |g_S| < 1             */
+    int32_t  use_g_S;     /* g_S = 0 is a weighting too (isotropic sampling, L207), hence the switch               */
+    int32_t  reserved;    /* 0                                                                                      */
 } dies_run_opts;
 
 /* Bytes of device workspace a model (n_models = 1) or a batch needs. */
@@ -116,7 +125,7 @@ int dies_set_sources_batch(dies_model*, const double* ext_bin_intensity, const d
                            const double* point_bin_weights);
 
 /* Follow n_packages packages per active source (per model) on `cuda_stream` (a cudaStream_t; NULL = default
- * stream).  Asynchronous: returns after the launches.  opts == NULL means {0.5, 0, IRE, 0, 24, n_packages, 1, 0, 1}. */
+ * stream).  Asynchronous: returns after the launches.  opts == NULL means {0.5, 0, IRE, 0, 24, n_packages, 1, 0, 1, 0, 0, 0, 0}. */
 int dies_run(dies_model*, uint64_t n_packages, uint64_t seed, const dies_run_opts* opts, void* cuda_stream);
 int dies_run_batch(dies_model*, uint64_t n_packages_per_model, uint64_t seed, const dies_run_opts* opts,
                    void* cuda_stream);

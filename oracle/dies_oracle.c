@@ -4,7 +4,7 @@
  * A plain, slow, serial, fp64 CPU implementation of the immediate re-emission (IRE) Monte Carlo
  * of DIES (arXiv 2408.13807) for a 1D spherical cloud of concentric shells, written from the
  * paper (/root/reference/PAPER.md, cited below as PAPER.md:L<line>) and from the readings listed
- * in DESIGN.md ("Readings of the paper", R1..R18).  One photon package is followed to the end
+ * in DESIGN.md ("Readings of the paper", R1..R19).  One photon package is followed to the end
  * before the next one starts.  No blocking, no fusion, no reordering.
  *
  * Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs may
@@ -24,6 +24,7 @@
  *   optically thin limit ..... int kappa J = int kappa B(T) within 0.5 % (north_star check c)
  *   IRE vs iteration ......... agreement with an independent 3-D Cartesian TMC (oracle/tmc_check.c; check d)
  *   k_bg, FFI ................ unbiasedness: same T(r) within errors, E[W] = 1
+ *   directional weighting .... Eq. 6-7 (R19): HG normalisation, E[W] = 1, absorbed energy independent of g_S, T(r) of g_E
  *   free-path weighting ...... Eq. 8 (R17): closed-form first flight under weighting, absorbed energy per shell
  *                              independent of k_A, k_S, k_A(rho); injected + reweight = escaped + terminated; guard (L119)
  * Parity unpinned: absolute T(r) of the optically thick configs 2 and 3 beyond IRE<->TMC agreement

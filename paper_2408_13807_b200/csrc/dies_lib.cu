@@ -634,13 +634,14 @@ extern "C" int dies_set_fixed_temperature(dies_model* m, const double* T, int n)
 static int fill_run_params(dies_model* m, uint64_t n_packages, uint64_t seed, const dies_run_opts* o, RunParams* R,
                            int* mode, int* accumulate, int* shift, uint64_t* n_total)
 {
-    dies_run_opts d = {0.5, 0, DIES_MODE_IRE, 0, 24, 0, 1.0, 0.0, 1.0};
+    dies_run_opts d = {0.5, 0, DIES_MODE_IRE, 0, 24, 0, 1.0, 0.0, 1.0, 0.0, 0.0, 0, 0};
     if (o) d = *o;
     if (d.k_A == 0.0) d.k_A = 1.0;
     if (d.k_S == 0.0) d.k_S = 1.0;
     if (!(d.k_A > 0.0) || !(d.k_S > 0.0) || !(d.k_A_dilute >= 0.0)) return fail(DIES_EINVAL, "k_A, k_S must be > 0 and k_A_dilute >= 0");
-    const bool weighted = d.k_A != 1.0 || d.k_S != 1.0 || d.k_A_dilute > 0.0;
-    if (weighted && d.ffi) return fail(DIES_EINVAL, "free-path weighting and forced first interaction are alternatives, not combined");
+    if (!(fabs(d.g_E) < 1.0) || !(fabs(d.g_S) < 1.0)) return fail(DIES_EINVAL, "|g_E|, |g_S| must be < 1");
+    const bool weighted = d.k_A != 1.0 || d.k_S != 1.0 || d.k_A_dilute > 0.0 || d.g_E != 0.0 || d.use_g_S != 0;
+    if (weighted && d.ffi) return fail(DIES_EINVAL, "free-path / directional weighting and forced first interaction are alternatives, not combined");
     if (!(d.k_bg > 0.0) || d.k_bg > 1.0) return fail(DIES_EINVAL, "k_bg must be in (0, 1]");
     if (d.mode != DIES_MODE_IRE && d.mode != DIES_MODE_FIXED_T) return fail(DIES_EINVAL, "bad mode");
     if (d.fixed_shift == 0) d.fixed_shift = 24;
@@ -657,6 +658,7 @@ static int fill_run_params(dies_model* m, uint64_t n_packages, uint64_t seed, co
     R->uniform_q = (d.k_bg == 0.5 && !d.ffi && !two && !weighted) ? 1 : 0;
     R->weighted = weighted ? 1 : 0;
     R->k_S = (float)d.k_S; R->k_A = d.k_A; R->k_A_dilute = d.k_A_dilute;
+    R->g_E = (float)d.g_E; R->g_S = (float)d.g_S; R->use_gS = d.use_g_S ? 1 : 0;
     R->qscale = (float)(1u << d.fixed_shift);
     R->pool = pool_slots(R->uniform_q != 0);
     R->thr_hi = env_int("DIES_THR_HI", 1, 32, 20);
@@ -830,7 +832,7 @@ extern "C" int dies_trace_packages(dies_model* m, int model_index, uint64_t firs
         return fail(DIES_EINVAL, "bad trace arguments");
     RunParams R;
     int mode, accumulate, shift; uint64_t nt;
-    dies_run_opts o = {0.5, 0, DIES_MODE_FIXED_T, 0, 24, n_total};
+    dies_run_opts o = {0.5, 0, DIES_MODE_FIXED_T, 0, 24, n_total, 1.0, 0.0, 1.0, 0.0, 0.0, 0, 0};
     if (opts) o = *opts;
     o.n_total = n_total;
     int rc = fill_run_params(m, 1, seed, &o, &R, &mode, &accumulate, &shift, &nt);

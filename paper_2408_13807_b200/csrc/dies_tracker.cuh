@@ -121,6 +121,8 @@ struct RunParams {
     int weighted;                    // free-path weighting (Eq. 8, R17): two clocks, package weights change in flight
     float k_S;                       // scattering clock factor
     double k_A, k_A_dilute;          // absorption clock factor(s) (host side: they go into stabW)
+    float g_E, g_S;                  // directional weighting of re-emission (Eq. 6) and scattering (Eq. 7); R19
+    int use_gS;                      // Eq. 7 active (g_S = 0 is a weighting too)
     float qscale;                    // 2^S
     int n_tickets, parts;            // tickets = n_models * parts
     int pool;                        // P: pool slots per warp (multiple of 8, 32 <= P <= kMaxPool)
@@ -599,7 +601,7 @@ __global__ void __launch_bounds__(kBlock, kMinBlocks) dies_track(DeviceModel D, 
                     if (cdf) k = sample_cdf(cdf, guide, u0);          // new frequency bin (launch: L55; re-emission: L87, R4)
 
                     // ---- event site (radius re, re2 = re^2, shell j) and new direction cosine mu w.r.t. the radius
-                    float re, re2, mu, b2src = 0.f;
+                    float re, re2, mu, b2src = 0.f, wdir = 1.f;
                     fly = true;
                     if (atsrc) {
                         // ---- launch
@@ -633,15 +635,39 @@ __global__ void __launch_bounds__(kBlock, kMinBlocks) dies_track(DeviceModel D, 
                         re2 = fmaf(se, se, b2);
                         re = sqrtf(re2);
                         mu = 2.f * u1 - 1.f;             // re-emission: isotropic (L87)
+                        // directional weighting (Eq. 6-7, R19) measures angles from the direction towards the centre
+                        // for packages of the external field and away from it for those of the central source (L109)
+                        const bool ptpkg = mp.has_ext ? ((id - R.id_base) >= R.n_total) : true;
+                        if (WT && isabs && R.g_E != 0.f) {
+                            // Eq. 6: HG(g_E) instead of isotropic; weight = (1/2) / p_HG(mu')
+                            const float mup = hg_cos(R.g_E, u1);
+                            const float x = fmaf(-2.f * R.g_E, mup, 1.f + R.g_E * R.g_E);
+                            wdir = x * sqrtf(x) / (1.f - R.g_E * R.g_E);
+                            mu = ptpkg ? mup : -mup;
+                        }
                         if (issca) {
                             // ---- scattering with the HG phase function (L85, L167)
                             float mu0 = re > 0.f ? se / re : 1.f;
                             mu0 = fminf(1.f, fmaxf(-1.f, mu0));
-                            const float ct = hg_cos(s_bin[k].z, u0);
                             const float sm = sqrtf(fmaxf(1.f - mu0 * mu0, 0.f));
-                            const float sth = sqrtf(fmaxf(1.f - ct * ct, 0.f));
-                            mu = mu0 * ct + sm * sth * cospif(2.f * u1);
-                            mu = fminf(1.f, fmaxf(-1.f, mu));
+                            if (WT && R.use_gS) {
+                                // Eq. 7: direction from HG(g_S) about the radial reference direction, azimuth uniform;
+                                // weight = dust HG density at the true scattering angle / sampling density
+                                const float mup = hg_cos(R.g_S, u0);
+                                const float mu1 = ptpkg ? mup : -mup;
+                                float ct = mu0 * mu1 + sm * sqrtf(fmaxf(1.f - mu1 * mu1, 0.f)) * cospif(2.f * u1);
+                                ct = fminf(1.f, fmaxf(-1.f, ct));
+                                const float g = s_bin[k].z;
+                                const float xa = fmaf(-2.f * g, ct, 1.f + g * g);
+                                const float xb = fmaf(-2.f * R.g_S, mup, 1.f + R.g_S * R.g_S);
+                                wdir = ((1.f - g * g) * xb * sqrtf(xb)) / ((1.f - R.g_S * R.g_S) * xa * sqrtf(xa));
+                                mu = mu1;
+                            } else {
+                                const float ct = hg_cos(s_bin[k].z, u0);
+                                const float sth = sqrtf(fmaxf(1.f - ct * ct, 0.f));
+                                mu = mu0 * ct + sm * sth * cospif(2.f * u1);
+                                mu = fminf(1.f, fmaxf(-1.f, mu));
+                            }
                         }
                         record<TRACE>(tp, pkg, n_ev, issca ? 1 /*SCATTER*/ : 2 /*ABSORB*/, j - mp.cav, k, ncross);
                     }
@@ -681,6 +707,16 @@ __global__ void __launch_bounds__(kBlock, kMinBlocks) dies_track(DeviceModel D, 
                             ev_absorb = (cA_ <= cS_);
                             col = fminf(cA_, cS_);
                         }
+                    }
+                    if (WT && (R.g_E != 0.f || R.use_gS)) {
+                        // the quantum the package carries away from a reweighted direction
+                        long long dq = 0;
+                        if (wdir != 1.f) {
+                            const unsigned long long qn = (unsigned long long)__double2ll_rn((double)q * (double)wdir);
+                            dq = (long long)qn - (long long)q;
+                            q = qn;
+                        }
+                        if (dq != 0) atomicAdd(&s_cnt[LC_REWEIGHT_RAW], (unsigned long long)dq);
                     }
                     // L119: a package whose weight fell by ten orders of magnitude is terminated (its quantum may also
                     // have rounded to nothing at the resolution 2^-S of the tallies, R18)

@@ -32,7 +32,8 @@ def test_run_opts_struct_layout():
     assert binding.dies_run_opts.n_total.offset == 24
     import ctypes
     assert binding.dies_run_opts.k_A.offset == 32 and binding.dies_run_opts.k_S.offset == 48
-    assert ctypes.sizeof(binding.dies_run_opts) == 56
+    assert binding.dies_run_opts.g_E.offset == 56 and binding.dies_run_opts.use_g_S.offset == 72
+    assert ctypes.sizeof(binding.dies_run_opts) == 80
 
 
 def test_workspace_bytes_and_argument_errors(lib):

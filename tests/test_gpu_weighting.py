@@ -129,3 +129,68 @@ def test_weighting_argument_errors():
     c = m.dies_get_counters()
     assert c["reweight_raw"] == 0 and c["injected_raw"] == c["escaped_raw"]
     m.close()
+
+
+# ------------------------------------------------------------------ directional weighting (Eq. 6-7; R19)
+DIR_VARIANTS = [dict(g_E=0.5), dict(g_E=-0.4), dict(g_S=0.3), dict(g_S=0.0), dict(g_S=-0.3, g_E=0.3, k_A=1.5)]
+
+
+@pytest.mark.parametrize("kw", DIR_VARIANTS)
+@pytest.mark.parametrize("cfg", ["config1", "config3s"])
+def test_directional_trace_bit_exact(orc, cfg, kw):
+    p = synth.config1(tau_V=3.0) if cfg == "config1" else synth.config3(n_shells=40, n_freq=64, tau_V=30.0)
+    n_total, count, max_ev = 100000, 2000, 512
+    o = orc.Oracle(p)
+    o.set_fixed_temperature(_fixed_T(p.n_shells))
+    m = dies.Model(p)
+    m.dies_set_fixed_temperature(_fixed_T(p.n_shells))
+    ev, nev = m.dies_trace_packages(0, count, n_total, seed=7, max_events=max_ev, mode=dies.DIES_MODE_FIXED_T, **kw)
+    safe = same = 0
+    for pid in range(count):
+        ref, nref, margin = o.trace(n_total, pid, seed=7, mode=1, max_events=max_ev, **kw)
+        ok = (nref == nev[pid]) and nref <= max_ev and np.array_equal(ref, ev[pid, :nref])
+        same += ok
+        if margin > 1e-3 and nref <= max_ev:
+            safe += 1
+            assert ok, (pid, margin, ref[:8], ev[pid, :8])
+    assert safe > 0.4 * count
+    assert same >= 0.99 * count, same / count
+    m.close()
+
+
+@pytest.mark.parametrize("kw", DIR_VARIANTS)
+def test_directional_fixed_T_absorbed_energy(orc, kw):
+    p = synth.config2(n_shells=40, n_freq=64, tau_V=3.0)
+    n = 400_000
+    o = orc.Oracle(p)
+    o.set_fixed_temperature(_fixed_T(p.n_shells))
+    o.run(n, seed=3, mode=1, **kw)
+    m = dies.Model(p)
+    m.dies_set_fixed_temperature(_fixed_T(p.n_shells))
+    m.dies_run(n, seed=3, mode=dies.DIES_MODE_FIXED_T, **kw)
+    raw, unit, energy = m.dies_get_absorbed()
+    c = m.dies_get_counters()
+    e_pkg = o.sums["injected"] / n
+    assert np.all(np.abs(energy - o.absorbed) <= np.maximum(2e-4 * o.absorbed, 8 * e_pkg)), \
+        np.max(np.abs(energy / o.absorbed - 1))
+    assert c["packages"] == n and c["terminated"] == 0 == o.counters["terminated"]
+    for k in ("crossings", "scatterings", "absorptions"):
+        assert abs(c[k] - o.counters[k]) <= 2e-4 * o.counters[k] + 3
+    assert _identity(c)
+    assert abs(c["reweight_raw"] * unit - o.sums["reweight"]) < 2e-3 * abs(o.sums["reweight"]) + 1e-5 * o.sums["injected"]
+    m.close()
+
+
+@pytest.mark.parametrize("kw", [dict(g_E=0.5), dict(g_S=0.2)])
+def test_directional_full_ire_temperature(orc, kw):
+    p = synth.config2(n_shells=40, n_freq=64, tau_V=3.0)
+    _check_T_parity(orc, p, 100_000, **kw)
+
+
+def test_directional_argument_errors():
+    m = dies.Model(synth.config1())
+    for kw in (dict(g_E=1.0), dict(g_S=-1.5), dict(g_E=0.3, ffi=1)):
+        with pytest.raises(dies.DiesError) as e:
+            m.dies_run(100, **kw)
+        assert e.value.code == dies.DIES_EINVAL
+    m.close()
