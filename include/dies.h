@@ -84,7 +84,8 @@ typedef struct {
     double   g_S;         /* scattering directions from HG(g_S) about that radial direction, weight = dust HG density
                              at the true scattering angle / p_HG(g_S); only if use_g_S != 0, |g_S| < 1             */
     int32_t  use_g_S;     /* g_S = 0 is a weighting too (isotropic sampling, L207), hence the switch               */
-    int32_t  reserved;    /* 0                                                                                      */
+    int32_t  reemit_in_cell; /* L253 (R20): re-emit from a random position of the cell volume (radius uniform in volume
+                             between the shell boundaries) instead of the absorption site; 0 = the IRE method proper */
 } dies_run_opts;
 
 /* Bytes of device workspace a model (n_models = 1) or a batch needs. */

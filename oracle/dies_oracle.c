@@ -4,7 +4,7 @@
  * A plain, slow, serial, fp64 CPU implementation of the immediate re-emission (IRE) Monte Carlo
  * of DIES (arXiv 2408.13807) for a 1D spherical cloud of concentric shells, written from the
  * paper (/root/reference/PAPER.md, cited below as PAPER.md:L<line>) and from the readings listed
- * in DESIGN.md ("Readings of the paper", R1..R19).  One photon package is followed to the end
+ * in DESIGN.md ("Readings of the paper", R1..R20).  One photon package is followed to the end
  * before the next one starts.  No blocking, no fusion, no reordering.
  *
  * Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs may
@@ -363,6 +363,7 @@ typedef struct {
     double g_E;              /* Eq. 6: re-emission directions from a Henyey-Greenstein function; 0 = isotropic (unweighted) */
     double g_S;              /* Eq. 7: scattering directions from HG(g_S) about the radial reference direction */
     int use_gS;              /* Eq. 7 is active (g_S = 0 is NOT the plain method, L207) */
+    int reemit_cell;         /* L253: re-emit from a random position of the cell volume instead of the absorption site */
 } run_opts;
 
 /* Henyey-Greenstein density of a direction cosine, Eq. 6: p(mu) = (1/2)(1-g^2)/(1+g^2-2 g mu)^{3/2} */
@@ -598,6 +599,16 @@ static void follow_package(const oracle_model* o, const run_opts* opt, tallies* 
             }
             tauS = -log(u[2]);
             tauA = -log(u[3]);
+            if (opt->reemit_cell) {
+                /* L253 (reading R20): "the position of re-emission was randomised within the cell volume":
+                 * radius uniform in volume between the boundaries of shell i, one more block for its uniform */
+                double u2[4];
+                draw_block(&s, u2);
+                const double ri = o->rb[i], ro = o->rb[i + 1];
+                r = cbrt(ri * ri * ri + u2[0] * (ro * ro * ro - ri * ri * ri));
+                if (r < ri) r = ri;
+                if (r > ro) r = ro;
+            }
             if (ta->reemit) ta->reemit[(size_t)i * K + k] += W * e;
             ta->counters[C_ABSORPTIONS] += 1;
             rec_event(rec, EV_ABSORB, i, k, crossings);
@@ -618,7 +629,7 @@ static void follow_package(const oracle_model* o, const run_opts* opt, tallies* 
  * to n_run visits every id once -- used by the order-independence pin). Tallies accumulate. */
 int dies_oracle_run(const oracle_model* o, uint64_t n_total, uint64_t first_id, uint64_t n_run, uint64_t id_stride,
                     uint64_t seed, uint32_t model_index, double k_bg, int ffi, int mode,
-                    const double* kA_w, double kS_w, double g_E, double g_S, int use_gS,
+                    const double* kA_w, double kS_w, double g_E, double g_S, int use_gS, int reemit_cell,
                     double* absorbed, double* escaped, double* reemit, double* pathlen,
                     uint64_t* counters, double* sums)
 {
@@ -627,7 +638,7 @@ int dies_oracle_run(const oracle_model* o, uint64_t n_total, uint64_t first_id, 
     if (kA_w) for (int i = 0; i < o->N; i++) if (!(kA_w[i] > 0.0)) return -1;
     if (ffi && (kA_w || kS_w != 1.0)) return -1;             /* alternatives in the paper (Fig. 7), not combined */
     if (!(fabs(g_E) < 1.0) || !(fabs(g_S) < 1.0)) return -1;
-    run_opts opt = { n_total, seed, model_index, k_bg, ffi, mode, kA_w, kS_w, g_E, g_S, use_gS };
+    run_opts opt = { n_total, seed, model_index, k_bg, ffi, mode, kA_w, kS_w, g_E, g_S, use_gS, reemit_cell };
     tallies ta = { absorbed, escaped, reemit, pathlen, counters, sums };
     for (uint64_t j = 0; j < n_run; j++) {
         uint64_t p = first_id + (uint64_t)(((unsigned __int128)j * id_stride) % n_run);
@@ -639,12 +650,12 @@ int dies_oracle_run(const oracle_model* o, uint64_t n_total, uint64_t first_id, 
 /* Replay one package against the given tallies (not modified) and list its events. */
 int dies_oracle_trace(const oracle_model* o, uint64_t n_total, uint64_t package_id, uint64_t seed,
                       uint32_t model_index, double k_bg, int ffi, int mode, const double* kA_w, double kS_w,
-                      double g_E, double g_S, int use_gS, const double* absorbed_state,
+                      double g_E, double g_S, int use_gS, int reemit_cell, const double* absorbed_state,
                       int32_t* events, int max_events, int* n_events, double* min_margin)
 {
     if (!o || !(o->has_ext || o->has_point) || n_total == 0) return -4;
     if (ffi && (kA_w || kS_w != 1.0)) return -1;
-    run_opts opt = { n_total, seed, model_index, k_bg, ffi, mode, kA_w, kS_w, g_E, g_S, use_gS };
+    run_opts opt = { n_total, seed, model_index, k_bg, ffi, mode, kA_w, kS_w, g_E, g_S, use_gS, reemit_cell };
     double* absorbed = (double*)calloc(o->N, sizeof(double));
     double* escaped = (double*)calloc(o->K, sizeof(double));
     if (absorbed_state) memcpy(absorbed, absorbed_state, o->N * sizeof(double));

@@ -37,7 +37,7 @@ class dies_run_opts(C.Structure):
     _fields_ = [("k_bg", C.c_double), ("ffi", C.c_int32), ("mode", C.c_int32), ("accumulate", C.c_int32),
                 ("fixed_shift", C.c_int32), ("n_total", C.c_uint64), ("k_A", C.c_double),
                 ("k_A_dilute", C.c_double), ("k_S", C.c_double), ("g_E", C.c_double), ("g_S", C.c_double),
-                ("use_g_S", C.c_int32), ("reserved", C.c_int32)]
+                ("use_g_S", C.c_int32), ("reemit_in_cell", C.c_int32)]
 
 
 _dp = C.POINTER(C.c_double)
@@ -128,11 +128,11 @@ def dies_test_philox(seed, first_id, block, model_index, n):
 
 
 def _opts(k_bg=0.5, ffi=0, mode=DIES_MODE_IRE, accumulate=0, fixed_shift=24, n_total=0, k_A=1.0, k_A_dilute=0.0,
-          k_S=1.0, g_E=0.0, g_S=None):
+          k_S=1.0, g_E=0.0, g_S=None, reemit_cell=0):
     """g_S=None: scattering directions are not weighted (g_S = 0 is a weighting: isotropic sampling)."""
     return dies_run_opts(float(k_bg), int(ffi), int(mode), int(accumulate), int(fixed_shift), int(n_total),
                          float(k_A), float(k_A_dilute), float(k_S), float(g_E), float(g_S or 0.0),
-                         int(g_S is not None), 0)
+                         int(g_S is not None), int(reemit_cell))
 
 
 class Model:

@@ -640,7 +640,8 @@ static int fill_run_params(dies_model* m, uint64_t n_packages, uint64_t seed, co
     if (d.k_S == 0.0) d.k_S = 1.0;
     if (!(d.k_A > 0.0) || !(d.k_S > 0.0) || !(d.k_A_dilute >= 0.0)) return fail(DIES_EINVAL, "k_A, k_S must be > 0 and k_A_dilute >= 0");
     if (!(fabs(d.g_E) < 1.0) || !(fabs(d.g_S) < 1.0)) return fail(DIES_EINVAL, "|g_E|, |g_S| must be < 1");
-    const bool weighted = d.k_A != 1.0 || d.k_S != 1.0 || d.k_A_dilute > 0.0 || d.g_E != 0.0 || d.use_g_S != 0;
+    const bool weighted = d.k_A != 1.0 || d.k_S != 1.0 || d.k_A_dilute > 0.0 || d.g_E != 0.0 || d.use_g_S != 0 ||
+                          d.reemit_in_cell != 0;
     if (weighted && d.ffi) return fail(DIES_EINVAL, "free-path / directional weighting and forced first interaction are alternatives, not combined");
     if (!(d.k_bg > 0.0) || d.k_bg > 1.0) return fail(DIES_EINVAL, "k_bg must be in (0, 1]");
     if (d.mode != DIES_MODE_IRE && d.mode != DIES_MODE_FIXED_T) return fail(DIES_EINVAL, "bad mode");
@@ -659,6 +660,7 @@ static int fill_run_params(dies_model* m, uint64_t n_packages, uint64_t seed, co
     R->weighted = weighted ? 1 : 0;
     R->k_S = (float)d.k_S; R->k_A = d.k_A; R->k_A_dilute = d.k_A_dilute;
     R->g_E = (float)d.g_E; R->g_S = (float)d.g_S; R->use_gS = d.use_g_S ? 1 : 0;
+    R->reemit_cell = d.reemit_in_cell ? 1 : 0;
     R->qscale = (float)(1u << d.fixed_shift);
     R->pool = pool_slots(R->uniform_q != 0);
     R->thr_hi = env_int("DIES_THR_HI", 1, 32, 20);

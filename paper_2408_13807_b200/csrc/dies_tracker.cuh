@@ -123,6 +123,7 @@ struct RunParams {
     double k_A, k_A_dilute;          // absorption clock factor(s) (host side: they go into stabW)
     float g_E, g_S;                  // directional weighting of re-emission (Eq. 6) and scattering (Eq. 7); R19
     int use_gS;                      // Eq. 7 active (g_S = 0 is a weighting too)
+    int reemit_cell;                 // L253 (R20): re-emit from a random position of the cell volume
     float qscale;                    // 2^S
     int n_tickets, parts;            // tickets = n_models * parts
     int pool;                        // P: pool slots per warp (multiple of 8, 32 <= P <= kMaxPool)
@@ -634,6 +635,18 @@ __global__ void __launch_bounds__(kBlock, kMinBlocks) dies_track(DeviceModel D, 
                         const float se = WT ? s + off : s + col / fabsf(lds_entry(pa - 8u).y);
                         re2 = fmaf(se, se, b2);
                         re = sqrtf(re2);
+                        if (WT && isabs && R.reemit_cell) {
+                            // L253 (R20): the package is re-emitted from a radius uniform in the volume of shell j;
+                            // one more Philox block gives the uniform
+                            uint32_t xr[4];
+                            philox4x32_10_rk(R.rk, (uint32_t)id, (uint32_t)(id >> 32), blk++, (uint32_t)m, xr);
+                            const float ri2 = lds_entry4(tab0 + 16u * (unsigned)j).x, ro2 = lds_entry4(tab0 + 16u * (unsigned)(j + 1)).x;
+                            const float ri = sqrtf(ri2), ro = sqrtf(ro2);
+                            const float ri3 = ri * ri2, ro3 = ro * ro2;
+                            re = cbrtf(fmaf(uniform24(xr[0]), ro3 - ri3, ri3));
+                            re = fminf(ro, fmaxf(ri, re));
+                            re2 = re * re;
+                        }
                         mu = 2.f * u1 - 1.f;             // re-emission: isotropic (L87)
                         // directional weighting (Eq. 6-7, R19) measures angles from the direction towards the centre
                         // for packages of the external field and away from it for those of the central source (L109)

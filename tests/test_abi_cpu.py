@@ -33,6 +33,7 @@ def test_run_opts_struct_layout():
     import ctypes
     assert binding.dies_run_opts.k_A.offset == 32 and binding.dies_run_opts.k_S.offset == 48
     assert binding.dies_run_opts.g_E.offset == 56 and binding.dies_run_opts.use_g_S.offset == 72
+    assert binding.dies_run_opts.reemit_in_cell.offset == 76
     assert ctypes.sizeof(binding.dies_run_opts) == 80
 
 

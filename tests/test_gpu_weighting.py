@@ -194,3 +194,36 @@ def test_directional_argument_errors():
             m.dies_run(100, **kw)
         assert e.value.code == dies.DIES_EINVAL
     m.close()
+
+
+# ------------------------------------------------------------------ re-emission position within the cell (L253; R20)
+def test_reemission_in_cell_trace_and_energy(orc):
+    p = synth.config2(n_shells=40, n_freq=64, tau_V=3.0)
+    Tf = _fixed_T(p.n_shells)
+    o = orc.Oracle(p)
+    o.set_fixed_temperature(Tf)
+    m = dies.Model(p)
+    m.dies_set_fixed_temperature(Tf)
+    n_total, count = 100000, 2000
+    ev, nev = m.dies_trace_packages(0, count, n_total, seed=9, max_events=512, mode=dies.DIES_MODE_FIXED_T, reemit_cell=1)
+    safe = 0
+    for pid in range(count):
+        ref, nref, margin = o.trace(n_total, pid, seed=9, mode=1, max_events=512, reemit_cell=1)
+        ok = (nref == nev[pid]) and nref <= 512 and np.array_equal(ref, ev[pid, :nref])
+        if margin > 1e-3 and nref <= 512:
+            safe += 1
+            assert ok, (pid, margin, ref[:8], ev[pid, :8])
+    assert safe > 0.4 * count
+    n = 400_000
+    o.run(n, seed=3, mode=1, reemit_cell=1)
+    m.dies_run(n, seed=3, mode=dies.DIES_MODE_FIXED_T, reemit_cell=1)
+    raw, unit, energy = m.dies_get_absorbed()
+    e_pkg = o.sums["injected"] / n
+    assert np.all(np.abs(energy - o.absorbed) <= np.maximum(1e-4 * o.absorbed, 5 * e_pkg))
+    c = m.dies_get_counters()
+    assert c["injected_raw"] == c["escaped_raw"] and c["reweight_raw"] == 0
+    m.close()
+
+
+def test_reemission_in_cell_full_ire_temperature(orc):
+    _check_T_parity(orc, synth.config2(n_shells=40, n_freq=64, tau_V=3.0), 100_000, reemit_cell=1)

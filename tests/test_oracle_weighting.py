@@ -156,3 +156,34 @@ def test_reemission_direction_weight_leaves_temperatures_unchanged():
     a = orc.Oracle(p).run(5000, seed=1)
     b = orc.Oracle(p).run(5000, seed=1, g_E=0.0)
     assert np.array_equal(a.absorbed, b.absorbed)         # g_E = 0 is the plain method
+
+
+# ------------------------------------------------------------------ re-emission position within the cell (L253; R20)
+def test_reemission_from_a_random_position_of_the_cell():
+    """One thick shell: packages are absorbed just below the surface and re-emitted in a transparent bin.  From the
+    absorption site (the plain method) the mean way out of an isotropic package is R/2 (surface point: half the
+    directions leave at once, the others cross a chord 2 R cos theta); from a position uniform in the volume it is
+    3R/4.  The path-length tally sees the difference."""
+    p = toy_problem(n_shells=1, tau=200.0)
+    n = 200000
+    res = {}
+    for flag in (0, 1):
+        o = orc.Oracle(p)
+        o.reset(pathlen=True)
+        o.run(n, seed=4, reemit_cell=flag)
+        assert o.counters["absorptions"] > 0.999 * n
+        res[flag] = o.pathlen.sum() / n                                   # mean path per package in units of R = 1
+    assert abs(res[0] - 0.5) < 0.02, res
+    assert abs(res[1] - 0.75) < 0.02, res
+
+
+def test_reemission_position_leaves_temperatures_unchanged():
+    """L253: "No visible differences were observed": T(r) of config 1 (32 shells) agrees within noise."""
+    p = synth.config1(tau_V=3.0)
+    n = 60000
+    a = np.array([orc.Oracle(p).run(n, seed=s).temperature() for s in range(1, 7)])
+    b = np.array([orc.Oracle(p).run(n, seed=s, reemit_cell=1).temperature() for s in range(1, 7)])
+    se = np.sqrt(a.var(0, ddof=1) / 6 + b.var(0, ddof=1) / 6)
+    d = np.abs(a.mean(0) - b.mean(0))
+    assert np.sum(d > np.maximum(0.01 * a.mean(0), 3.5 * se)) <= 1, d / se
+    assert not np.array_equal(a[0], b[0])
