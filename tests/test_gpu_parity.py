@@ -332,3 +332,27 @@ def test_error_codes():
     with pytest.raises(dies.DiesError) as e:
         dies.Model(bad)
     assert e.value.code == dies.DIES_EINVAL
+
+
+def test_large_dimensions(orc):
+    """Many shells (1200: the unfolded table spans several KB of shared memory) and many frequency bins (1000):
+    fixed-temperature parity on identical streams, and the size that no longer fits is refused."""
+    p = synth.config3(n_shells=1200, n_freq=32, tau_V=5.0, n_packages=20000)
+    o, m, raw, unit, energy = _fixed_T_pair(orc, p, 20000)
+    e_pkg = o.sums["injected"] / 20000
+    assert np.all(np.abs(energy - o.absorbed) <= np.maximum(1e-4 * o.absorbed, 3 * e_pkg))
+    c = m.dies_get_counters()
+    assert abs(c["crossings"] - o.counters["crossings"]) <= 2e-4 * o.counters["crossings"] + 3
+    assert c["injected_raw"] == c["escaped_raw"]
+    m.close()
+    p = synth.config1(n_freq=1000, n_packages=50000)
+    o, m, raw, unit, energy = _fixed_T_pair(orc, p, 50000)
+    e_pkg = o.sums["injected"] / 50000
+    assert np.all(np.abs(energy - o.absorbed) <= np.maximum(1e-4 * o.absorbed, 3 * e_pkg))
+    esc = m.dies_get_escape_spectrum()
+    assert abs(esc.sum() / o.sums["escaped"] - 1) < 1e-6
+    assert np.all(np.abs(esc - o.escaped) <= 1e-4 * o.escaped + 3 * e_pkg)
+    m.close()
+    with pytest.raises(dies.DiesError) as e:
+        dies.Model(synth.config3(n_shells=6000, n_freq=16))
+    assert e.value.code == dies.DIES_EINVAL
