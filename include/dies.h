@@ -128,6 +128,10 @@ int dies_set_sources_batch(dies_model*, const double* ext_bin_intensity, const d
 /* Follow n_packages packages per active source (per model) on `cuda_stream` (a cudaStream_t; NULL = default
  * stream).  Asynchronous: returns after the launches.  opts == NULL means {0.5, 0, IRE, 0, 24, n_packages, 1, 0, 1, 0, 0, 0, 0}. */
 int dies_run(dies_model*, uint64_t n_packages, uint64_t seed, const dies_run_opts* opts, void* cuda_stream);
+/* Sharding of fixed-temperature runs over processes / GPUs: the next dies_run that does not
+ * accumulate follows the package ids first_id .. first_id + n_packages - 1 (per source) of a run of opts->n_total
+ * packages instead of starting at 0.  Integer tallies of disjoint id ranges add up to the tallies of the whole run. */
+int dies_seek(dies_model*, uint64_t first_id);
 int dies_run_batch(dies_model*, uint64_t n_packages_per_model, uint64_t seed, const dies_run_opts* opts,
                    void* cuda_stream);
 

@@ -24,7 +24,7 @@ EXPORTS = ("dies_workspace_bytes", "dies_create_model", "dies_create_batch", "di
            "dies_set_sources_batch", "dies_run", "dies_run_batch", "dies_get_temperature", "dies_get_escape_spectrum",
            "dies_set_fixed_temperature", "dies_get_absorbed", "dies_get_counters", "dies_trace_packages",
            "dies_trace_package", "dies_test_philox", "dies_get_tables", "dies_destroy", "dies_last_error",
-           "dies_device_info", "dies_bench_atomics")
+           "dies_device_info", "dies_bench_atomics", "dies_seek")
 
 
 class DiesError(RuntimeError):
@@ -63,6 +63,7 @@ def lib():
     L.dies_set_sources_batch.argtypes = [vp, _dp, _dp, _dp]
     L.dies_run.argtypes = [vp, u64, u64, C.POINTER(dies_run_opts), vp]
     L.dies_run_batch.argtypes = [vp, u64, u64, C.POINTER(dies_run_opts), vp]
+    L.dies_seek.argtypes = [vp, u64]
     L.dies_get_temperature.argtypes = [vp, _dp, C.c_int]
     L.dies_get_escape_spectrum.argtypes = [vp, _dp, C.c_int]
     L.dies_set_fixed_temperature.argtypes = [vp, _dp, C.c_int]
@@ -199,6 +200,9 @@ class Model:
         _chk(lib().dies_run(self._h, int(n_packages), int(seed), C.byref(o), C.c_void_p(s)))
 
     dies_run_batch = dies_run
+
+    def dies_seek(self, first_id):
+        _chk(lib().dies_seek(self._h, int(first_id)))
 
     def dies_get_temperature(self):
         T = np.zeros(self.n_models * self.N)

@@ -87,6 +87,7 @@ struct dies_model {
     std::vector<double> L_ext, L_point;   // per model
     std::vector<int> has_ext, has_point;
     unsigned long long done, n_total;     // packages per source already followed / planned
+    unsigned long long next_first;        // dies_seek: first package id (per source) of the next fresh run
     int shift;
     cudaStream_t stream;
     int grid_max, blocks_per_sm, n_sms;
@@ -490,7 +491,7 @@ extern "C" int dies_create_batch(int n_models, int n_shells, const double* r_bou
     m->N = N; m->K = K; m->nT = nT; m->M = M; m->ldS = N + 1;
     m->L = L; m->ws = (unsigned char*)workspace_dev;
     m->sources_set = m->fixed_set = m->ran = false;
-    m->done = m->n_total = 0; m->shift = 24; m->stream = 0; m->launches = 0;
+    m->done = m->n_total = 0; m->next_first = 0; m->shift = 24; m->stream = 0; m->launches = 0;
     m->L_ext.assign(M, 0.0); m->L_point.assign(M, 0.0); m->has_ext.assign(M, 0); m->has_point.assign(M, 0);
     m->smem_bytes = smem; m->smem_trace_bytes = smem_trace; m->pool = pool; m->kref = kref;
     DeviceModel& D = m->D;
@@ -683,8 +684,9 @@ extern "C" int dies_run(dies_model* m, uint64_t n_packages, uint64_t seed, const
         if (n_total != m->n_total || shift != m->shift) return fail(DIES_ESTATE, "accumulate needs the same n_total and fixed_shift");
     } else {
         accumulate = 0;
-        m->done = 0;
+        m->done = m->next_first;
     }
+    m->next_first = 0;
     if (m->done + n_packages > n_total) return fail(DIES_EINVAL, "more packages than n_total");
     R.id_base = m->done;
     cudaStream_t st = (cudaStream_t)cuda_stream;
@@ -731,6 +733,13 @@ extern "C" int dies_run(dies_model* m, uint64_t n_packages, uint64_t seed, const
     CUDA_TRY(cudaGetLastError());
     m->done += n_packages;
     m->ran = true;
+    return DIES_OK;
+}
+
+extern "C" int dies_seek(dies_model* m, uint64_t first_id)
+{
+    if (!m) return fail(DIES_EINVAL, "model is NULL");
+    m->next_first = first_id;
     return DIES_OK;
 }
 

@@ -57,3 +57,25 @@ def max_over_ranks(ms: float, device) -> float:
     if dist.is_available() and dist.is_initialized() and dist.get_world_size() > 1:
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
     return float(t.item())
+
+
+def run_fixed_T_shard(model, n_total: int, seed: int, rank: int, world: int, **opts):
+    """Fixed-temperature tracking of this rank's share of an n_total-package run on `model` (a binding.Model whose
+    fixed temperatures are set): follows the rank's package-id range, then sums the integer tallies over the ranks.
+    Returns (absorbed raw units per shell summed over the ranks, this rank's escaped energy per bin, this rank's
+    counters)."""
+    import numpy as np
+    from . import binding
+
+    first, count = package_range(n_total, rank, world)
+    model.dies_seek(first)
+    if count > 0:
+        model.dies_run(count, seed=seed, mode=binding.DIES_MODE_FIXED_T, n_total=n_total, **opts)
+        raw, unit, _ = model.dies_get_absorbed()
+        esc = model.dies_get_escape_spectrum()
+        counters = model.dies_get_counters()
+    else:
+        raw, unit, esc, counters = np.zeros(model.N, dtype=np.int64), 0.0, np.zeros(model.K), {}
+    dev = model.device if dist.is_available() and dist.is_initialized() and dist.get_backend() == "nccl" else "cpu"
+    (raw_sum,) = allreduce_tallies(torch.as_tensor(np.ascontiguousarray(raw), dtype=torch.int64, device=dev))
+    return raw_sum.cpu().numpy(), esc, counters

@@ -356,3 +356,31 @@ def test_large_dimensions(orc):
     with pytest.raises(dies.DiesError) as e:
         dies.Model(synth.config3(n_shells=6000, n_freq=16))
     assert e.value.code == dies.DIES_EINVAL
+
+
+def test_fixed_T_shards_add_up_bit_exactly():
+    """disjoint package-id ranges followed by different handles (the ranks of a sharded run, here
+    one after the other on one GPU) give integer tallies whose sum is the single run's, bit for bit."""
+    from paper_2408_13807_b200 import sharding
+    p = synth.config1()
+    n, seed = 100_001, 8
+    whole = dies.Model(p)
+    whole.dies_set_fixed_temperature(_fixed_T(p.n_shells))
+    whole.dies_run(n, seed=seed, mode=dies.DIES_MODE_FIXED_T)
+    raw_w, _, _ = whole.dies_get_absorbed()
+    c_w = whole.dies_get_counters()
+    world = 3
+    tot = np.zeros_like(raw_w)
+    cross = 0
+    for rank in range(world):
+        m = dies.Model(p)
+        m.dies_set_fixed_temperature(_fixed_T(p.n_shells))
+        raw, esc, c = sharding.run_fixed_T_shard(m, n, seed, rank, world)
+        first, count = sharding.package_range(n, rank, world)
+        assert c["packages"] == count
+        tot += raw
+        cross += c["crossings"]
+        m.close()
+    assert np.array_equal(tot, raw_w)
+    assert cross == c_w["crossings"]
+    whole.close()
