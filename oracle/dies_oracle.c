@@ -364,6 +364,7 @@ typedef struct {
     double g_S;              /* Eq. 7: scattering directions from HG(g_S) about the radial reference direction */
     int use_gS;              /* Eq. 7 is active (g_S = 0 is NOT the plain method, L207) */
     int reemit_cell;         /* L253: re-emit from a random position of the cell volume instead of the absorption site */
+    int fp32_tallies;        /* negative control (L155, L179-181): keep the absorbed energy of a cell in single precision */
 } run_opts;
 
 /* Henyey-Greenstein density of a direction cosine, Eq. 6: p(mu) = (1/2)(1-g^2)/(1+g^2-2 g mu)^{3/2} */
@@ -570,6 +571,9 @@ static void follow_package(const oracle_model* o, const run_opts* opt, tallies* 
              * the emission spectra at the new and old temperatures */
             double old = ta->absorbed[i];
             double new_ = old + W * e;
+            /* L155: "the limited precision of floating point operations" -- the paper's fp32 counters stop growing
+             * once an update is below half a unit in the last place of the sum (from ~1e8 packages on, L179) */
+            if (opt->fp32_tallies) new_ = (double)(float)((float)old + (float)(W * e));
             ta->absorbed[i] = new_;
             int t;
             if (opt->mode == 1) t = o->fixed_row[i];
@@ -629,7 +633,7 @@ static void follow_package(const oracle_model* o, const run_opts* opt, tallies* 
  * to n_run visits every id once -- used by the order-independence pin). Tallies accumulate. */
 int dies_oracle_run(const oracle_model* o, uint64_t n_total, uint64_t first_id, uint64_t n_run, uint64_t id_stride,
                     uint64_t seed, uint32_t model_index, double k_bg, int ffi, int mode,
-                    const double* kA_w, double kS_w, double g_E, double g_S, int use_gS, int reemit_cell,
+                    const double* kA_w, double kS_w, double g_E, double g_S, int use_gS, int reemit_cell, int fp32_tallies,
                     double* absorbed, double* escaped, double* reemit, double* pathlen,
                     uint64_t* counters, double* sums)
 {
@@ -638,7 +642,7 @@ int dies_oracle_run(const oracle_model* o, uint64_t n_total, uint64_t first_id, 
     if (kA_w) for (int i = 0; i < o->N; i++) if (!(kA_w[i] > 0.0)) return -1;
     if (ffi && (kA_w || kS_w != 1.0)) return -1;             /* alternatives in the paper (Fig. 7), not combined */
     if (!(fabs(g_E) < 1.0) || !(fabs(g_S) < 1.0)) return -1;
-    run_opts opt = { n_total, seed, model_index, k_bg, ffi, mode, kA_w, kS_w, g_E, g_S, use_gS, reemit_cell };
+    run_opts opt = { n_total, seed, model_index, k_bg, ffi, mode, kA_w, kS_w, g_E, g_S, use_gS, reemit_cell, fp32_tallies };
     tallies ta = { absorbed, escaped, reemit, pathlen, counters, sums };
     for (uint64_t j = 0; j < n_run; j++) {
         uint64_t p = first_id + (uint64_t)(((unsigned __int128)j * id_stride) % n_run);
@@ -655,7 +659,7 @@ int dies_oracle_trace(const oracle_model* o, uint64_t n_total, uint64_t package_
 {
     if (!o || !(o->has_ext || o->has_point) || n_total == 0) return -4;
     if (ffi && (kA_w || kS_w != 1.0)) return -1;
-    run_opts opt = { n_total, seed, model_index, k_bg, ffi, mode, kA_w, kS_w, g_E, g_S, use_gS, reemit_cell };
+    run_opts opt = { n_total, seed, model_index, k_bg, ffi, mode, kA_w, kS_w, g_E, g_S, use_gS, reemit_cell, 0 };
     double* absorbed = (double*)calloc(o->N, sizeof(double));
     double* escaped = (double*)calloc(o->K, sizeof(double));
     if (absorbed_state) memcpy(absorbed, absorbed_state, o->N * sizeof(double));

@@ -31,7 +31,7 @@ _lib.dies_oracle_set_fixed_temperature.argtypes = [_vp, _dp]
 _lib.dies_oracle_temperature.argtypes = [_vp, _dp, _dp, C.POINTER(C.c_int), C.POINTER(C.c_int)]
 _lib.dies_oracle_get_tables.argtypes = [_vp, _dp, _dp, _dp]
 _lib.dies_oracle_run.argtypes = [_vp, _u64, _u64, _u64, _u64, _u64, C.c_uint32, C.c_double, C.c_int, C.c_int,
-                                 _dp, C.c_double, C.c_double, C.c_double, C.c_int, C.c_int, _dp, _dp, _dp, _dp,
+                                 _dp, C.c_double, C.c_double, C.c_double, C.c_int, C.c_int, C.c_int, _dp, _dp, _dp, _dp,
                                  C.POINTER(_u64), _dp]
 _lib.dies_oracle_trace.argtypes = [_vp, _u64, _u64, _u64, C.c_uint32, C.c_double, C.c_int, C.c_int, _dp, C.c_double,
                                    C.c_double, C.c_double, C.c_int, C.c_int,
@@ -149,7 +149,7 @@ class Oracle:
         return self.kA_profile(k_A, k_A_dilute)
 
     def run(self, n_total, seed=1, k_bg=0.5, ffi=0, mode=0, first_id=0, n_run=None, id_stride=1, model_index=0,
-            k_A=1.0, k_A_dilute=0.0, k_S=1.0, g_E=0.0, g_S=None, reemit_cell=0):
+            k_A=1.0, k_A_dilute=0.0, k_S=1.0, g_E=0.0, g_S=None, reemit_cell=0, fp32_tallies=0):
         """Follow packages first_id..first_id+n_run-1; tallies accumulate until reset().  g_S=None: scattering
         directions are not weighted (g_S = 0 is a weighting: isotropic sampling, L207)."""
         if n_run is None:
@@ -157,7 +157,7 @@ class Oracle:
         kw = self._weights(k_A, k_A_dilute, k_S)
         rc = _lib.dies_oracle_run(self._h, n_total, first_id, n_run, id_stride, seed, model_index, k_bg, ffi, mode,
                                   _d(kw), float(k_S), float(g_E), float(g_S or 0.0), int(g_S is not None),
-                                  int(reemit_cell), _d(self.absorbed), _d(self.escaped), _d(self.reemit), _d(self.pathlen),
+                                  int(reemit_cell), int(fp32_tallies), _d(self.absorbed), _d(self.escaped), _d(self.reemit), _d(self.pathlen),
                                   self._counters.ctypes.data_as(C.POINTER(_u64)), _d(self._sums))
         if rc != 0:
             raise RuntimeError(f"dies_oracle_run failed: {rc}")

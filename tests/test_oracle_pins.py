@@ -436,3 +436,19 @@ def test_trace_is_a_replay_of_run():
         assert np.all(np.diff(ev[:, 3]) >= 0)
     c = o.counters
     assert (tot["scatter"], tot["absorb"], tot["cross"]) == (c["scatterings"], c["absorptions"], c["crossings"])
+
+
+def test_fp32_counters_lose_energy_where_int64_design_cannot():
+    """Negative control for PAPER.md L155 / L179-181: with single-precision absorption counters a cell that receives
+    more than 2^24 equal updates no longer sums them (the paper's reason for N_B batches); the fp64 oracle -- and the GPU's
+    64-bit fixed-point tallies -- keep every update.  One thick shell: every package is absorbed once."""
+    p = toy_problem(n_shells=1, tau=200.0)
+    n = 20_000_000
+    good = orc.Oracle(p).run(n, seed=1)
+    bad = orc.Oracle(p).run(n, seed=1, fp32_tallies=1)
+    e_pkg = good.sums["injected"] / n
+    assert good.counters["absorptions"] == bad.counters["absorptions"] > 0.999 * n
+    assert abs(good.absorbed[0] / (good.counters["absorptions"] * e_pkg) - 1) < 1e-9
+    # beyond 2^24 updates an update is about half a unit in the last place of the fp32 sum: it is rounded to a whole
+    # unit or to nothing, and the total drifts by tens of per cent (up or down, depending on the binade)
+    assert abs(bad.absorbed[0] / good.absorbed[0] - 1) > 0.05
