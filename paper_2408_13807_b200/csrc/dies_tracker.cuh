@@ -29,7 +29,7 @@ constexpr unsigned kFull = 0xffffffffu;
 constexpr unsigned kChunk = 128;     // package ids a warp takes from the global counter at a time
 constexpr int kUnroll = 12;           // crossings per vote in the crossing loop
 constexpr int kMaxPool = 248;        // pool slots per warp (queue entries are bytes)
-constexpr int kGuide = 256;          // cut-points per CDF row of the guide tables
+constexpr int kGuide = 1024;         // cut-points per CDF row of the guide tables
 constexpr int kTallyStride = 32;     // 64-bit words between the absorbed-energy tallies of two shells: one tally per
                                      // 256 bytes, because the L2 atomic unit serialises updates of the same line
 
