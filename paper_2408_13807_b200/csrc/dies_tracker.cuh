@@ -485,16 +485,19 @@ __global__ void __launch_bounds__(kBlock, kMinBlocks) dies_track(DeviceModel D, 
                 int j = ci <= 0 ? -ci : ci - 1;
                 const unsigned absmask = __ballot_sync(kFull, isabs);
                 unsigned long long old = 0;
+                unsigned peers = 0;
+                int leader = 0;
                 if (absmask) {
                     if (TRACE) {
                         if (isabs && MODE == 0) old = gA[j * kTallyStride];
                     } else if (MODE == 1) {
                         if (isabs) smem_add64(&s_A[j], &s_A[ldS + j], q);
                     } else if (R.uniform_q) {
-                        const unsigned peers = __match_any_sync(kFull, isabs ? j : -1 - lane);
-                        const int leader = __ffs(peers) - 1;
+                        // the leader's atomic is issued now; its value is broadcast only where the rows are needed, after
+                        // the Philox block, so that nothing waits for L2 here
+                        peers = __match_any_sync(kFull, isabs ? j : -1 - lane);
+                        leader = __ffs(peers) - 1;
                         if (isabs && lane == leader) old = atomicAdd(&gA[j * kTallyStride], q * (unsigned long long)__popc(peers));
-                        old = __shfl_sync(kFull, old, leader) + q * (unsigned long long)__popc(peers & lt_mask);
                     } else if (isabs) {
                         old = atomicAdd(&gA[j * kTallyStride], q);
                     }
@@ -571,12 +574,15 @@ __global__ void __launch_bounds__(kBlock, kMinBlocks) dies_track(DeviceModel D, 
                         if (MODE == 1) {
                             row = s_row[j];
                         } else {
+                            const int hint = s_row[j];
+                            if (!TRACE && R.uniform_q)
+                                old = __shfl_sync(absmask, old, leader) + q * (unsigned long long)__popc(peers & lt_mask);
                             // emitted power per mass before and after this absorption; rows of the table (R4)
                             const double cs = s_cs[j];
                             const float eps_old = (float)((double)old * cs);
                             const float eps_new = (float)((double)(old + q) * cs);
-                            const int hint = s_row[j];
                             row = row_from(s_eps, nT, hint, eps_old);
+
                             if (row > hint) atomicMax(&s_row[j], row);
                             const bool same = (row == nT - 1) || (eps_new < s_eps[row]);
                             if (eps_new >= s_eps[nT - 1]) atomicAdd(&s_cnt[LC_CLAMP_HI], 1ull);
@@ -599,7 +605,8 @@ __global__ void __launch_bounds__(kBlock, kMinBlocks) dies_track(DeviceModel D, 
                     const float u0 = uniform24(xw[0]), u1 = uniform24(xw[1]);
                     const float tauS = neg_log(uniform24(xw[2]));       // Eq. 1
                     const float tauA = neg_log(uniform24(xw[3]));
-                    if (cdf) k = sample_cdf(cdf, guide, u0);          // new frequency bin (launch: L55; re-emission: L87, R4)
+                    // new frequency bin (launch: L55; re-emission: L87, R4)
+                    if (cdf) k = sample_cdf(cdf, guide, u0);
 
                     // ---- event site (radius re, re2 = re^2, shell j) and new direction cosine mu w.r.t. the radius
                     float re, re2, mu, b2src = 0.f, wdir = 1.f;
