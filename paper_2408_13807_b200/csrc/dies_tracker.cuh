@@ -913,35 +913,38 @@ __global__ void __launch_bounds__(kBlock, kMinBlocks) dies_track(DeviceModel D, 
                 }
                 nR -= min(nR, 32);
                 unsigned pa0 = pa;
-                float2 E = lds_entry(pa);
                 bool alive = has;
                 for (;;) {
-                    const unsigned pb = pa;                      // the table is walked from here with constant offsets
+                    // the table is walked from pb with constant offsets; the entries are read two steps ahead of their
+                    // use and unconditionally (a lane that has stopped reads on harmlessly, at most 13 entries past its
+                    // own, inside the block's shared memory), so that no crossing waits for a shared-memory load
+                    const unsigned pb = pa;
+                    float2 T0 = lds_entry(pb), T1 = lds_entry(pb + 8u);
 #pragma unroll
                     for (int u = 0; u < kUnroll; u++) {
-                        const float d = E.x - b2;
+                        const float2 T2 = lds_entry(pb + 8u * (u + 2));
+                        const float d = T0.x - b2;
                         alive = alive && (d >= 0.f);
                         if (alive) {
                             // col -= rho^ (sn - s) as (col + rho^ s) - rho^ sn: the first half does not wait for the sqrt
-                            const float t = fmaf(fabsf(E.y), s, col);
-                            s = __int_as_float(__float_as_int(sqrt_ftz(d)) | (__float_as_int(E.y) & 0x80000000));
-                            col = fmaf(-fabsf(E.y), s, t);
-                            E = lds_entry(pb + 8u * (u + 1));
+                            const float t = fmaf(fabsf(T0.y), s, col);
+                            s = __int_as_float(__float_as_int(sqrt_ftz(d)) | (__float_as_int(T0.y) & 0x80000000));
+                            col = fmaf(-fabsf(T0.y), s, t);
                             pa = pb + 8u * (u + 1);
                         }
                         alive = alive && (col >= 0.f);
+                        T0 = T1; T1 = T2;
                     }
                     if (!alive && (col >= 0.f)) {
-                        if (__float_as_int(E.y) < 0) {
-                            // the inner surface is not reached (tangent shell): head for the outer one instead
-                            // entry c -> entry 1 - c; the 1 - 2c entries skipped are no passages
+                        if (pa <= tab0) {
+                            // an inward entry (c <= 0) whose surface is not reached (tangent shell): head for the outer
+                            // one instead, entry c -> entry 1 - c; the 1 - 2c entries skipped are no passages
                             const unsigned np = 2u * tab0 + 8u - pa;
                             pa0 += np - pa;
                             pa = np;
-                            E = lds_entry(pa);
                             alive = true;
                         } else if (pa != pa_out) {
-                            b2 = E.x;                                // outward, b2 > r^2 by rounding only: graze
+                            b2 = lds_entry(pa).x;                    // outward, b2 > r^2 by rounding only: graze
                             alive = true;
                         }
                     }
@@ -984,7 +987,6 @@ __global__ void __launch_bounds__(kBlock, kMinBlocks) dies_track(DeviceModel D, 
                         const float4 a = lds_f4(aA + 16u * slot);
                         s = a.x; b2 = a.y; col = a.z; pa = __float_as_uint(a.w);
                         pa0 = pa;
-                        E = lds_entry(pa);
                     } else if (!alive) {
                         col = -1.f;                              // idle lane: never flies, never looks stopped short
                     }
