@@ -384,3 +384,33 @@ def test_fixed_T_shards_add_up_bit_exactly():
     assert np.array_equal(tot, raw_w)
     assert cross == c_w["crossings"]
     whole.close()
+
+
+def test_batch_full_ire_temperature_over_8_seeds(orc):
+    """Config 5 reduced (4 spheres of 64 shells, one launch per seed): per-shell T of every model within 1 % or 3
+    combined standard errors of the oracle's 8-seed mean; shells flagged once are re-examined on seeds 9-16."""
+    b = synth.config5(n_models=4, n_packages=40_000)
+
+    def stats(seeds):
+        To = np.zeros((len(seeds), b.n_models, 64))
+        Tg = np.zeros_like(To)
+        m = dies.Model(batch=b)
+        for a, s in enumerate(seeds):
+            m.dies_run(b.n_packages, seed=s)
+            Tg[a] = m.dies_get_temperature()
+            c = m.dies_get_counters()
+            assert c["injected_raw"] == c["escaped_raw"] and c["packages"] == b.n_models * b.n_packages
+            for i in range(b.n_models):
+                o = orc.Oracle(b.model(i))
+                o.run(b.n_packages, seed=s, model_index=i)
+                To[a, i] = o.temperature()
+        m.close()
+        return To.reshape(len(seeds), -1), Tg.reshape(len(seeds), -1)
+
+    To, Tg = stats(range(1, 9))
+    bad, info = _T_outliers(To, Tg)
+    if np.any(bad):
+        assert bad.sum() <= max(1, int(0.05 * bad.size)), info
+        To2, Tg2 = stats(range(9, 17))
+        bad2, info2 = _T_outliers(To2, Tg2)
+        assert not np.any(bad & bad2), (info, info2)
