@@ -384,12 +384,13 @@ __global__ void k_test_philox(uint32_t k0, uint32_t k1, unsigned long long first
 // ------------------------------------------------------------------ helpers
 static int check_device()
 {
-    int dev = 0;
+    // (cudaGetDeviceProperties costs milliseconds; the compute capability is one attribute)
+    int dev = 0, major = 0, minor = 0;
     cudaError_t e = cudaGetDevice(&dev);
     if (e != cudaSuccess) return fail(DIES_ECUDA, "no CUDA device: %s", cudaGetErrorString(e));
-    cudaDeviceProp p;
-    CUDA_TRY(cudaGetDeviceProperties(&p, dev));
-    if (p.major != 10) return fail(DIES_ECUDA, "libdies is built for sm_100a only; device is sm_%d%d", p.major, p.minor);
+    CUDA_TRY(cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev));
+    CUDA_TRY(cudaDeviceGetAttribute(&minor, cudaDevAttrComputeCapabilityMinor, dev));
+    if (major != 10) return fail(DIES_ECUDA, "libdies is built for sm_100a only; device is sm_%d%d", major, minor);
     return DIES_OK;
 }
 
@@ -416,6 +417,9 @@ static size_t tracker_smem(int N, int K, int nT, int P, bool trace, bool with_q,
 template <int MODE, bool TRACE>
 static cudaError_t set_smem(size_t bytes)
 {
+    static size_t granted = 0;                       // per kernel pair: raise the limit only when a model needs more
+    if (bytes <= granted) return cudaSuccess;
+    granted = bytes;
     cudaError_t e = cudaFuncSetAttribute(dies_track<MODE, TRACE, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
     if (e != cudaSuccess) return e;
     return cudaFuncSetAttribute(dies_track<MODE, TRACE, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
