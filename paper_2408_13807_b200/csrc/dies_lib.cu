@@ -84,6 +84,7 @@ struct dies_model {
     unsigned char* ws;
     DeviceModel D;
     bool sources_set, fixed_set, ran;
+    bool finalized;                       // T_out / Lesc_out / derived counters are those of the last run
     std::vector<double> L_ext, L_point;   // per model
     std::vector<int> has_ext, has_point;
     unsigned long long done, n_total;     // packages per source already followed / planned
@@ -494,7 +495,7 @@ extern "C" int dies_create_batch(int n_models, int n_shells, const double* r_bou
     if (!m) return fail(DIES_ENOMEM, "host allocation failed");
     m->N = N; m->K = K; m->nT = nT; m->M = M; m->ldS = N + 1;
     m->L = L; m->ws = (unsigned char*)workspace_dev;
-    m->sources_set = m->fixed_set = m->ran = false;
+    m->sources_set = m->fixed_set = m->ran = m->finalized = false;
     m->done = m->n_total = 0; m->next_first = 0; m->shift = 24; m->stream = 0; m->launches = 0;
     m->L_ext.assign(M, 0.0); m->L_point.assign(M, 0.0); m->has_ext.assign(M, 0); m->has_point.assign(M, 0);
     m->smem_bytes = smem; m->smem_trace_bytes = smem_trace; m->pool = pool; m->kref = kref;
@@ -737,6 +738,7 @@ extern "C" int dies_run(dies_model* m, uint64_t n_packages, uint64_t seed, const
     CUDA_TRY(cudaGetLastError());
     m->done += n_packages;
     m->ran = true;
+    m->finalized = false;
     return DIES_OK;
 }
 
@@ -756,6 +758,7 @@ extern "C" int dies_run_batch(dies_model* m, uint64_t n, uint64_t seed, const di
 static int finalize(dies_model* m)
 {
     if (!m->ran) return fail(DIES_ESTATE, "no run yet");
+    if (m->finalized) return DIES_OK;            // nothing ran since the last read-out
     const int n = m->M * (m->K > m->N ? m->K : m->N);
     int* flags = wsp<int>(m, m->L.flags);
     CUDA_TRY(cudaMemsetAsync(flags, 0, 16, m->stream));
@@ -772,6 +775,7 @@ static int finalize(dies_model* m)
     CUDA_TRY(cudaStreamSynchronize(m->stream));
     CUDA_TRY(cudaGetLastError());
     if (hf[1]) return fail(DIES_EOVERFLOW, "a tally exceeded 2^62");
+    m->finalized = true;
     return DIES_OK;
 }
 
