@@ -106,27 +106,36 @@ static T* wsp(dies_model* m, size_t off) { return reinterpret_cast<T*>(m->ws + o
 __global__ void k_build_tables(const double* __restrict__ emis, int nT, int K, double* __restrict__ eps,
                                float* __restrict__ F, int* flags)
 {
-    const int t = blockIdx.x * blockDim.x + threadIdx.x;
+    // one warp per temperature row: lane l owns the bins [l c, (l+1) c), c = ceil(K / 32)
+    const int t = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
     if (t >= nT) return;
     const double* row = emis + (size_t)t * K;
     const double* prev = t > 0 ? row - K : nullptr;
-    double s = 0.0, tot = 0.0;
+    const int c = (K + 31) / 32, k0 = min(lane * c, K), k1 = min(k0 + c, K);
+    double s = 0.0, part = 0.0;
     bool bad = false;
-    for (int k = 0; k < K; k++) {
+    for (int k = k0; k < k1; k++) {
         const double d = row[k] - (prev ? prev[k] : 0.0);
         if (!(d >= 0.0)) bad = true;
         s += row[k];
-        tot += d;
+        part += d;
     }
-    eps[t] = s;
-    if (bad || !(tot > 0.0)) atomicOr(flags, 1);
-    double c = 0.0;
+    // totals and the exclusive prefix of the partial sums of the increments
+    double tot = part, ssum = s, pre = part;
+    for (int o = 1; o < 32; o <<= 1) {
+        const double v = __shfl_up_sync(0xffffffffu, pre, o);
+        if (lane >= o) pre += v;
+    }
+    for (int o = 16; o > 0; o >>= 1) { tot += __shfl_xor_sync(0xffffffffu, tot, o); ssum += __shfl_xor_sync(0xffffffffu, ssum, o); }
+    pre -= part;
+    if (__any_sync(0xffffffffu, bad) || !(tot > 0.0)) { if (lane == 0) atomicOr(flags, 1); }
+    if (lane == 0) eps[t] = ssum;
     float* f = F + (size_t)t * K;
-    for (int k = 0; k < K; k++) {
-        c += row[k] - (prev ? prev[k] : 0.0);
-        f[k] = (float)(c / tot);
+    double cum = pre;
+    for (int k = k0; k < k1; k++) {
+        cum += row[k] - (prev ? prev[k] : 0.0);
+        f[k] = (k == K - 1) ? 1.0f : (float)(cum / tot);
     }
-    f[K - 1] = 1.0f;
 }
 
 // guide tables of the cut-point sampler: guide[row][c] = smallest k with cdf[row][k] > c / kGuide
@@ -523,7 +532,7 @@ extern "C" int dies_create_batch(int n_models, int n_shells, const double* r_bou
     TRY_OR_FREE(cudaMemcpyAsync(m->ws + L.rb, r_bounds, (size_t)M * (N + 1) * 8, cudaMemcpyHostToDevice, 0));
     TRY_OR_FREE(cudaMemcpyAsync(m->ws + L.rho, rho, (size_t)M * N * 8, cudaMemcpyHostToDevice, 0));
     int* flags = wsp<int>(m, L.flags);
-    k_build_tables<<<(nT + 127) / 128, 128>>>(wsp<double>(m, L.emis), nT, K, wsp<double>(m, L.eps), wsp<float>(m, L.F), flags);
+    k_build_tables<<<(nT * 32 + 127) / 128, 128>>>(wsp<double>(m, L.emis), nT, K, wsp<double>(m, L.eps), wsp<float>(m, L.F), flags);
     k_build_guide<<<(nT * kGuide + 255) / 256, 256>>>(wsp<float>(m, L.F), nT, K, wsp<unsigned short>(m, L.guideF));
     k_build_epsgrid<<<(nT + 127) / 128, 128>>>(wsp<double>(m, L.eps), nT, wsp<float>(m, L.epsgrid), wsp<double>(m, L.epsref), flags);
     k_build_dust<<<(K + 127) / 128, 128>>>(wsp<double>(m, L.dustin), K, kref, wsp<float4>(m, L.bintab), wsp<float>(m, L.omega));
