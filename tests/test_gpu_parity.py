@@ -414,3 +414,29 @@ def test_batch_full_ire_temperature_over_8_seeds(orc):
         To2, Tg2 = stats(range(9, 17))
         bad2, info2 = _T_outliers(To2, Tg2)
         assert not np.any(bad & bad2), (info, info2)
+
+
+def test_smallest_dimensions(orc):
+    """One shell, two temperatures, two frequency bins (one of them transparent, zero scattering, g = 0), and a
+    three-shell model with a cavity and scattering: fixed-temperature parity and exact conservation."""
+    from test_oracle_pins import toy_problem
+    for p in (toy_problem(n_shells=1, tau=1.5), toy_problem(n_shells=3, tau=2.0, kappa_sca=0.7, g=0.0, r_in=0.2)):
+        n = 30000
+        Tfix = np.full(p.n_shells, 25.0)
+        o = orc.Oracle(p)
+        o.set_fixed_temperature(Tfix)
+        o.run(n, seed=6, mode=1)
+        m = dies.Model(p)
+        m.dies_set_fixed_temperature(Tfix)
+        m.dies_run(n, seed=6, mode=dies.DIES_MODE_FIXED_T)
+        raw, unit, energy = m.dies_get_absorbed()
+        e_pkg = o.sums["injected"] / n
+        assert np.all(np.abs(energy - o.absorbed) <= np.maximum(1e-4 * o.absorbed, 3 * e_pkg))
+        c = m.dies_get_counters()
+        assert c["packages"] == n == c["escaped"] and c["injected_raw"] == c["escaped_raw"]
+        for k in ("crossings", "scatterings", "absorptions"):
+            assert abs(c[k] - o.counters[k]) <= 2e-4 * o.counters[k] + 3
+        m.dies_run(n, seed=6)                      # full IRE on the same tiny model
+        T = m.dies_get_temperature()
+        assert np.all(np.isfinite(T)) and m.dies_get_counters()["injected_raw"] == m.dies_get_counters()["escaped_raw"]
+        m.close()
