@@ -11,7 +11,9 @@ LIB = os.path.join(HERE, "libdies.so")
 SOURCES = [os.path.join(CSRC, "dies_lib.cu")]
 DEPS = SOURCES + [os.path.join(CSRC, "dies_tracker.cuh"), os.path.join(HERE, "..", "include", "dies.h")]
 NVCC_FLAGS = ["-O3", "-std=c++17", "-lineinfo", "-gencode", "arch=compute_100a,code=sm_100a", "-shared",
-              "-Xcompiler", "-fPIC", "-Xptxas", "-v"]
+              "-Xcompiler", "-fPIC", "-Xptxas", "-v",
+              # single-precision division and square root of the event arithmetic at 2 ulp (R14b)
+              "-prec-div=false", "-prec-sqrt=false"]
 
 
 def build(force: bool = False, verbose: bool = False) -> str:
