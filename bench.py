@@ -32,7 +32,7 @@ from paper_2408_13807_b200 import sharding, synth  # noqa: E402
 # crossing = SASS instructions of one predicated crossing step; scattering / absorption / package = predicated-on
 # thread-instructions executed on the unit's own source lines (shared event stream + its own branch) per unit,
 # from the ncu source page of the same workload.  Queue handling, swaps, votes, fix-ups and idle lanes are NOT work.
-INSTR = dict(crossing=9, scattering=297, absorption=351, package=268)
+INSTR = dict(crossing=8, scattering=297, absorption=351, package=268)
 # dram__bytes_read.sum + dram__bytes_write.sum of one dies_track launch (ncu --set full, profiles/r1n_ncu_full.md)
 TRAFFIC_BYTES_PER_LAUNCH = 737536
 SM_COUNT, SCHEDULERS, LANES = 148, 4, 32

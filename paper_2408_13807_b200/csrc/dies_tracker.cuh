@@ -914,6 +914,10 @@ __global__ void __launch_bounds__(kBlock, kMinBlocks) dies_track(DeviceModel D, 
                 nR -= min(nR, 32);
                 unsigned pa0 = pa;
                 bool alive = has;
+                // the along-ray coordinate is kept as a = +-s, positive along the direction of the entry the package
+                // heads for (inward entries: a = -s), so that a new surface is a = sqrt(d) without a sign operation
+                // and the signed density of the entry (negative: inward) does the rest
+                float a = (pa <= tab0) ? -s : s;
                 for (;;) {
                     // the table is walked from pb with constant offsets; the entries are read two steps ahead of their
                     // use and unconditionally (a lane that has stopped reads on harmlessly, at most 13 entries past its
@@ -926,10 +930,10 @@ __global__ void __launch_bounds__(kBlock, kMinBlocks) dies_track(DeviceModel D, 
                         const float d = T0.x - b2;
                         alive = alive && (d >= 0.f);
                         if (alive) {
-                            // col -= rho^ (sn - s) as (col + rho^ s) - rho^ sn: the first half does not wait for the sqrt
-                            const float t = fmaf(fabsf(T0.y), s, col);
-                            s = __int_as_float(__float_as_int(sqrt_ftz(d)) | (__float_as_int(T0.y) & 0x80000000));
-                            col = fmaf(-fabsf(T0.y), s, t);
+                            // col -= rho^ (sn - s) as (col + rho^ s) - rho^ sn with s = +-a, sn = +-sqrt(d), T0.y = +-rho^
+                            const float t = fmaf(T0.y, a, col);
+                            a = sqrt_ftz(d);
+                            col = fmaf(-T0.y, a, t);
                             pa = pb + 8u * (u + 1);
                         }
                         alive = alive && (col >= 0.f);
@@ -942,6 +946,7 @@ __global__ void __launch_bounds__(kBlock, kMinBlocks) dies_track(DeviceModel D, 
                             const unsigned np = 2u * tab0 + 8u - pa;
                             pa0 += np - pa;
                             pa = np;
+                            a = -a;                                  // the coordinate now runs along an outward entry
                             alive = true;
                         } else if (pa != pa_out) {
                             b2 = lds_entry(pa).x;                    // outward, b2 > r^2 by rounding only: graze
@@ -963,6 +968,8 @@ __global__ void __launch_bounds__(kBlock, kMinBlocks) dies_track(DeviceModel D, 
                         const unsigned n = ((pa - pa0) >> 3) - (isev ? 1u : 0u);
                         if (kf & KF_DRY) lc_ffi += n;
                         else { lc_cross += n; if (TRACE) pT[2 * P + slot] += (int)n; }
+                        // signed coordinate: a runs along the entry ahead (flying) or the one just committed (event)
+                        s = ((alive ? pa : pa - 8u) <= tab0) ? -a : a;
                         sts_f4(aA + 16u * slot, s, b2, col, __uint_as_float(pa));
                         // stopped on the sentinel: left the model (escape, or the end of a dry FFI flight)
                         t = alive ? QT_READY : (isev ? ((kf & KF_EVABS) ? QT_ABS : QT_SCA) : QT_SRC);
@@ -984,8 +991,9 @@ __global__ void __launch_bounds__(kBlock, kMinBlocks) dies_track(DeviceModel D, 
                     const bool take = !alive && (r < nR);
                     if (take) {
                         slot = lds_u8(qR + (nR - 1 - r));
-                        const float4 a = lds_f4(aA + 16u * slot);
-                        s = a.x; b2 = a.y; col = a.z; pa = __float_as_uint(a.w);
+                        const float4 a4 = lds_f4(aA + 16u * slot);
+                        s = a4.x; b2 = a4.y; col = a4.z; pa = __float_as_uint(a4.w);
+                        a = (pa <= tab0) ? -s : s;
                         pa0 = pa;
                     } else if (!alive) {
                         col = -1.f;                              // idle lane: never flies, never looks stopped short
