@@ -2,7 +2,7 @@
 //
 // Every warp owns a POOL of P photon packages whose state lives in shared memory (40 bytes per package) and four
 // small queues of pool slots: packages ready to fly, and packages waiting for an absorption, a scattering, or a
-// source event (escape tally + launch of the next package id, or the end of a dry FFI flight).  The warp alternates
+// source event (escape tally + launch of the next package id).  The warp alternates
 // between
 //   (1) a CROSSING phase: 32 flying packages in registers run the shell-crossing loop (Eq. 4) with
 //       no random numbers, no global memory and no branches (every crossing is predicated on the lane still flying).
@@ -37,7 +37,7 @@ constexpr int kTallyStride = 32;     // 64-bit words between the absorbed-energy
 enum { LC_PACKAGES = 0, LC_CROSSINGS, LC_FFI_CROSSINGS, LC_SCATTERINGS, LC_ABSORPTIONS, LC_ESCAPED, LC_UNINTERACTED,
        LC_TERMINATED, LC_EXTRA_BLOCKS, LC_CLAMP_HI, LC_INJECTED_RAW, LC_TERMINATED_RAW, LC_REWEIGHT_RAW, LC_N };
 
-// per-slot flag word: frequency bin | type of the pending event | dry FFI flight | slot holds a package
+// per-slot flag word: frequency bin | type of the pending event | (unused) | slot holds a package
 constexpr unsigned KF_K = 0xffffu, KF_EVABS = 1u << 16, KF_DRY = 1u << 17, KF_OCC = 1u << 18;
 // the queues of a warp
 enum { QT_ABS = 0, QT_SCA, QT_SRC, QT_READY, QT_N };
@@ -48,7 +48,7 @@ struct ModelParams {
     int has_ext, has_point;
     float r0hat;       // r_bounds[0] / R
     float qs_ext, qs_point;   // e_src / e_ref (<= 1): raw units per unit-weight package / 2^S
-    float colmax;      // a column (units of 1/kappa_ref) larger than that of any chord: start of a dry FFI flight
+    float colmax;      // a column (units of 1/kappa_ref) larger than that of any chord: start value of the FFI chord sum
 };
 
 // The shell table of one model is "unfolded" along a chord: entry c in [-ldS, ldS+1] (stored at c + ldS)
@@ -441,7 +441,7 @@ __global__ void __launch_bounds__(kBlock, kMinBlocks) dies_track(DeviceModel D, 
                     if (TRACE) { pkg = pT[slot]; n_ev = pT[P + slot]; ncross = (unsigned)pT[2 * P + slot]; }
                 }
                 int k = (int)(kf & KF_K);
-                const bool dryend = issrc && (kf & KF_DRY);      // the dry FFI flight reached the far surface
+                constexpr bool dryend = false;                   // (FFI sums its chord inside the launch event: no dry flights)
                 const bool esc = issrc && !dryend && (kf & KF_OCC);
 
                 // (0) free-path weighting (Eq. 8, R17): the quantum the package carries at this event.  Along the
@@ -557,15 +557,15 @@ __global__ void __launch_bounds__(kBlock, kMinBlocks) dies_track(DeviceModel D, 
                     wc_pkg += __popc(__ballot_sync(kFull, launch));
                 }
 
-                // (4) events: launch / scatter / absorb + re-emit / end of a dry FFI flight; one Philox block each
+                // (4) events: launch / scatter / absorb + re-emit; one Philox block each
                 //     (DESIGN.md RNG contract), one instruction stream for all of them
                 bool fly = false, ev_absorb = false, dry = false, uninter = false;
+                unsigned long long q_inj = 0;
                 if (launch || isev || dryend) {
                     uint32_t xw[4];
                     const bool atsrc = launch || dryend;                            // the event site is the source
                     const bool point = atsrc && (mp.has_ext ? ((id - R.id_base) >= R.n_total) : true);
-                    // block 0 belongs to the launch; with FFI the end of the dry flight draws it again
-                    unsigned b = dryend ? 0u : blk;
+                    unsigned b = blk;
                     philox4x32_10_rk(R.rk, (uint32_t)id, (uint32_t)(id >> 32), b, (uint32_t)m, xw);
                     const float* cdf = nullptr;      // table the new frequency bin is drawn from (launch, re-emission)
                     const unsigned short* guide = nullptr;
@@ -601,7 +601,7 @@ __global__ void __launch_bounds__(kBlock, kMinBlocks) dies_track(DeviceModel D, 
                         cdf = g_src + (point ? K : 0);                              // L55 source spectrum table
                         guide = g_srcguide + (point ? kGuide : 0);
                     }
-                    blk = (launch && R.ffi) ? 0u : b + 1u;
+                    blk = b + 1u;
                     const float u0 = uniform24(xw[0]), u1 = uniform24(xw[1]);
                     const float tauS = neg_log(uniform24(xw[2]));       // Eq. 1
                     const float tauA = neg_log(uniform24(xw[3]));
@@ -634,6 +634,7 @@ __global__ void __launch_bounds__(kBlock, kMinBlocks) dies_track(DeviceModel D, 
                             ncross = 0; n_ev = 0;
                             q = (unsigned long long)__float2ll_rn(w * (point ? mp.qs_point : mp.qs_ext) * R.qscale);
                             q0f = (float)q;
+                            q_inj = q;                           // (FFI splits the quantum below)
                             record<TRACE>(tp, pkg, n_ev, 0 /*LAUNCH*/, j - mp.cav, k, 0);
                         }
                     } else {
@@ -693,12 +694,39 @@ __global__ void __launch_bounds__(kBlock, kMinBlocks) dies_track(DeviceModel D, 
                     }
                     // ---- column (in units of 1/kappa_ref) to the next event and its type
                     if (R.ffi && atsrc) {
-                        if (!dryend) {
-                            // forced first interaction (Eq. 9-12, R11): a dry flight along the whole chord first
-                            col = mp.colmax; dry = true;
-                        } else {
+                        // forced first interaction (Eq. 9-12, R11).  The optical depth tau0 of the whole launch chord is
+                        // summed here, in the launch batch (all lanes walk their chords together: no exchange, no vote,
+                        // no second event for the package), with the arithmetic of the crossing step
+                        float cdry = mp.colmax;
+                        if (!WT) {
+                            const float sw = re * mu;
+                            float b2w = point ? re2 * (1.f - mu) * (1.f + mu) : b2src;
+                            unsigned pw = tab0 + 8u * (unsigned)((sw < 0.f) ? -j : j + 1);
+                            float aw = (pw <= tab0) ? -sw : sw;
+                            unsigned nff = 0;
+                            for (;;) {
+                                const float2 T = lds_entry(pw);
+                                const float d = T.x - b2w;
+                                if (d >= 0.f) {
+                                    const float t = fmaf(T.y, aw, cdry);
+                                    aw = sqrt_ftz(d);
+                                    cdry = fmaf(-T.y, aw, t);
+                                    pw += 8u;
+                                    nff++;
+                                } else if (pw <= tab0) {
+                                    pw = 2u * tab0 + 8u - pw;        // tangent shell: on to the mirrored outward entry
+                                    aw = -aw;
+                                } else if (pw != pa_out) {
+                                    b2w = T.x;                       // graze
+                                } else {
+                                    break;                           // the sentinel: the chord has left the model
+                                }
+                            }
+                            lc_ffi += nff;
+                        }
+                        {
                             const float kext = s_bin[k].w;
-                            const float tau0 = kext * (mp.colmax - col);           // Eq. 9
+                            const float tau0 = kext * (mp.colmax - cdry);          // Eq. 9
                             const float Pint = -expm1f(-tau0);                     // Eq. 12
                             const unsigned long long q_un = min(q, (unsigned long long)__float2ll_rn((float)q * expf(-tau0)));
                             if (!TRACE && q_un) smem_add64(&s_esc[k], &s_esc[K + k], q_un);   // un-interacted share escapes in bin k
@@ -765,7 +793,7 @@ __global__ void __launch_bounds__(kBlock, kMinBlocks) dies_track(DeviceModel D, 
                 }
                 if (!R.uniform_q) {
                     // raw units injected by the launches of this batch
-                    unsigned long long inj = launch ? q : 0ull;
+                    unsigned long long inj = launch ? q_inj : 0ull;
                     const unsigned lm = __ballot_sync(kFull, launch);
                     if (lm) {
 #pragma unroll
@@ -971,7 +999,7 @@ __global__ void __launch_bounds__(kBlock, kMinBlocks) dies_track(DeviceModel D, 
                         // signed coordinate: a runs along the entry ahead (flying) or the one just committed (event)
                         s = ((alive ? pa : pa - 8u) <= tab0) ? -a : a;
                         sts_f4(aA + 16u * slot, s, b2, col, __uint_as_float(pa));
-                        // stopped on the sentinel: left the model (escape, or the end of a dry FFI flight)
+                        // stopped on the sentinel: left the model
                         t = alive ? QT_READY : (isev ? ((kf & KF_EVABS) ? QT_ABS : QT_SCA) : QT_SRC);
                     }
                     {
