@@ -85,7 +85,7 @@ struct dies_model {
     DeviceModel D;
     bool sources_set, fixed_set, ran;
     bool finalized;                       // T_out / Lesc_out / derived counters are those of the last run
-    std::vector<double> L_ext, L_point;   // per model
+    std::vector<double> L_point;          // per model
     std::vector<int> has_ext, has_point;
     unsigned long long done, n_total;     // packages per source already followed / planned
     unsigned long long next_first;        // dies_seek: first package id (per source) of the next fresh run
@@ -272,7 +272,7 @@ __global__ void k_build_wshells(const double* __restrict__ rb, const double* __r
 
 // source spectrum tables and luminosities: L_ext = 4 pi R^2 * pi * sum_k J_k
 __global__ void k_build_sources(const double* __restrict__ srcin, const double* __restrict__ rb, int N, int K, int M,
-                                float* srccdf, double* Lsrc)
+                                float* srccdf, double* Lsrc, ModelParams* mp)
 {
     const int idx = blockIdx.x * blockDim.x + threadIdx.x;
     if (idx >= 2 * M) return;
@@ -285,6 +285,9 @@ __global__ void k_build_sources(const double* __restrict__ srcin, const double* 
         const double pi = 3.14159265358979323846;
         const double R = rb[(size_t)m * (N + 1) + N];
         Lsrc[2 * m] = 4.0 * pi * R * R * pi * tot;
+        mp[m].has_ext = tot > 0.0 ? 1 : 0;                       // which sources of the model are active (R2)
+    } else {
+        mp[m].has_point = (Lsrc[2 * m + 1] > 0.0 && tot > 0.0) ? 1 : 0;
     }
     double c = 0.0;
     for (int k = 0; k < K; k++) {
@@ -506,7 +509,7 @@ extern "C" int dies_create_batch(int n_models, int n_shells, const double* r_bou
     m->L = L; m->ws = (unsigned char*)workspace_dev;
     m->sources_set = m->fixed_set = m->ran = m->finalized = false;
     m->done = m->n_total = 0; m->next_first = 0; m->shift = 24; m->stream = 0; m->launches = 0;
-    m->L_ext.assign(M, 0.0); m->L_point.assign(M, 0.0); m->has_ext.assign(M, 0); m->has_point.assign(M, 0);
+    m->L_point.assign(M, 0.0); m->has_ext.assign(M, 0); m->has_point.assign(M, 0);
     m->smem_bytes = smem; m->smem_trace_bytes = smem_trace; m->pool = pool; m->kref = kref;
     DeviceModel& D = m->D;
     D.N = N; D.K = K; D.nT = nT; D.n_models = M; D.ldS = N + 1; D.ldT = 2 * (N + 1) + 2;
@@ -582,9 +585,7 @@ extern "C" int dies_set_sources_batch(dies_model* m, const double* ext, const do
     if (!m) return fail(DIES_EINVAL, "model is NULL");
     const int K = m->K, M = m->M, N = m->N;
     std::vector<double> in((size_t)M * 2 * K, 0.0);
-    std::vector<ModelParams> mp(M);
     CUDA_TRY(cudaStreamSynchronize(m->stream));
-    CUDA_TRY(cudaMemcpy(mp.data(), m->ws + m->L.mp, (size_t)M * sizeof(ModelParams), cudaMemcpyDeviceToHost));
     bool any = false;
     for (int i = 0; i < M; i++) {
         double J = 0.0, P = 0.0;
@@ -602,22 +603,19 @@ extern "C" int dies_set_sources_batch(dies_model* m, const double* ext, const do
         if (Lp < 0.0) return fail(DIES_EINVAL, "model %d: L_point < 0", i);
         m->has_ext[i] = J > 0.0; m->has_point[i] = (Lp > 0.0 && P > 0.0);
         m->L_point[i] = m->has_point[i] ? Lp : 0.0;
-        mp[i].has_ext = m->has_ext[i]; mp[i].has_point = m->has_point[i];
         any = any || m->has_ext[i] || m->has_point[i];
     }
     std::vector<double> Ls((size_t)2 * M, 0.0);
     for (int i = 0; i < M; i++) Ls[2 * i + 1] = m->L_point[i];
     CUDA_TRY(cudaMemcpy(m->ws + m->L.srcin, in.data(), in.size() * 8, cudaMemcpyHostToDevice));
     CUDA_TRY(cudaMemcpy(m->ws + m->L.Lsrc, Ls.data(), Ls.size() * 8, cudaMemcpyHostToDevice));
-    CUDA_TRY(cudaMemcpy(m->ws + m->L.mp, mp.data(), (size_t)M * sizeof(ModelParams), cudaMemcpyHostToDevice));
     k_build_sources<<<(2 * M + 127) / 128, 128>>>(wsp<double>(m, m->L.srcin), wsp<double>(m, m->L.rb), N, K, M,
-                                                  wsp<float>(m, m->L.srccdf), wsp<double>(m, m->L.Lsrc));
+                                                  wsp<float>(m, m->L.srccdf), wsp<double>(m, m->L.Lsrc),
+                                                  wsp<ModelParams>(m, m->L.mp));
     k_build_guide<<<(2 * M * kGuide + 255) / 256, 256>>>(wsp<float>(m, m->L.srccdf), 2 * M, K,
                                                         wsp<unsigned short>(m, m->L.guideS));
     m->launches += 2;
-    CUDA_TRY(cudaMemcpy(Ls.data(), m->ws + m->L.Lsrc, Ls.size() * 8, cudaMemcpyDeviceToHost));
     CUDA_TRY(cudaGetLastError());
-    for (int i = 0; i < M; i++) m->L_ext[i] = m->has_ext[i] ? Ls[2 * i] : 0.0;
     m->sources_set = any;
     m->ran = false; m->done = 0;
     return DIES_OK;
