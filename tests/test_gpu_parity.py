@@ -440,3 +440,16 @@ def test_smallest_dimensions(orc):
         T = m.dies_get_temperature()
         assert np.all(np.isfinite(T)) and m.dies_get_counters()["injected_raw"] == m.dies_get_counters()["escaped_raw"]
         m.close()
+
+
+def test_atomic_microbenchmark_runs():
+    """dies_bench_atomics (measurement support of bench.py): sane figures, merged draws issue fewer atomics."""
+    r1 = dies.dies_bench_atomics(1, None, 1, iters=200)
+    r0 = dies.dies_bench_atomics(1, None, 0, iters=200)
+    assert r1["lane_ops_per_s"] > 5 * r0["lane_ops_per_s"] > 0       # one address: a warp merges 32 draws into one
+    assert abs(r1["atomics_per_s"] / r1["lane_ops_per_s"] - 1 / 32) < 1e-6
+    w = np.arange(1, 101, dtype=float)
+    rw = dies.dies_bench_atomics(100, w, 1, iters=200)
+    assert 0 < rw["atomics_per_s"] <= rw["lane_ops_per_s"]
+    with pytest.raises(dies.DiesError):
+        dies.dies_bench_atomics(100, -w, 1)
