@@ -3,8 +3,9 @@
  *
  * Monte Carlo propagation of photon packages through a 1D spherically symmetric dust cloud of
  * concentric shells with the immediate re-emission (IRE) method (section 2.1),
- * with initial-direction weighting k_bg (Eq. 5) and forced first interaction (Eq. 9-12,
- * L132-149).  Citations are lines of /root/reference/PAPER.md; "R<n>" are the readings of
+ * with the weighted sampling schemes of the paper's Table 1 -- initial direction k_bg (Eq. 5),
+ * re-emission and scattering directions g_E, g_S (Eq. 6-7), absorption and scattering free paths k_A,
+ * k_S, also density dependent (Eq. 8) -- and forced first interaction (Eq. 9-12).  Citations are lines of /root/reference/PAPER.md; "R<n>" are the readings of
  * DESIGN.md.  Every step of the path runs in hand-written sm_100a CUDA kernels; there is no CPU
  * fallback: every entry point that needs the device returns DIES_ECUDA when it is missing.
  *
