@@ -453,3 +453,35 @@ def test_atomic_microbenchmark_runs():
     assert 0 < rw["atomics_per_s"] <= rw["lane_ops_per_s"]
     with pytest.raises(dies.DiesError):
         dies.dies_bench_atomics(100, -w, 1)
+
+
+def test_ire_mode_trace_against_run_tallies(orc):
+    """Full IRE decisions (table rows from the cell energy before / after the absorption, the extra Philox block when
+    they differ) replayed package by package: after a GPU IRE run, packages traced in IRE mode against the run's
+    tallies give the oracle's event lists computed from the same tallies."""
+    p = synth.config1()
+    n = p.n_packages
+    m = dies.Model(p)
+    m.dies_run(n, seed=12)
+    raw, unit, energy = m.dies_get_absorbed()
+    o = orc.Oracle(p)
+    count, max_ev = 1500, 512
+    ev, nev = m.dies_trace_packages(0, count, n, seed=77, max_events=max_ev, mode=dies.DIES_MODE_IRE)
+    safe = same = 0
+    for pid in range(count):
+        ref, nref, margin = o.trace(n, pid, seed=77, mode=0, max_events=max_ev, absorbed_state=energy)
+        ok = (nref == nev[pid]) and nref <= max_ev and np.array_equal(ref, ev[pid, :nref])
+        same += ok
+        safe += (margin > 1e-3)
+    assert safe > 0.4 * count
+    assert same >= 0.985 * count, same / count
+    # early in a run the cells are cold and an absorption spans many table rows: replay against a young state too
+    m.dies_run(2000, seed=13, n_total=n)
+    raw, unit, energy = m.dies_get_absorbed()
+    ev, nev = m.dies_trace_packages(5000, 500, n, seed=78, max_events=max_ev, mode=dies.DIES_MODE_IRE)
+    same = 0
+    for x in range(500):
+        ref, nref, margin = o.trace(n, 5000 + x, seed=78, mode=0, max_events=max_ev, absorbed_state=energy)
+        same += (nref == nev[x]) and nref <= max_ev and np.array_equal(ref, ev[x, :nref])
+    assert same >= 0.97 * 500, same / 500
+    m.close()
