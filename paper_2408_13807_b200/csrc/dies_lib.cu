@@ -718,7 +718,8 @@ extern "C" int dies_run(dies_model* m, uint64_t n_packages, uint64_t seed, const
     unsigned long long ids = 0;
     for (int i = 0; i < m->M; i++) ids += n_packages * (unsigned long long)(m->has_ext[i] + m->has_point[i]);
     const unsigned long long per_block = (unsigned long long)kWarps * R.pool;    // packages a block keeps in flight
-    unsigned long long want = (ids + 2ull * per_block - 1) / (2ull * per_block);
+    const unsigned long long per_b = (unsigned long long)env_int("DIES_PKG_PER_BLOCK", 32, 1 << 20, (int)per_block);   // small runs: one pool filling per warp
+    unsigned long long want = (ids + per_b - 1) / per_b;
     int grid = (int)(want < 1 ? 1 : (want > (unsigned long long)grid_max ? grid_max : want));
     if (m->M == 1) { R.parts = grid; R.n_tickets = grid; }
     else { R.parts = (8 * grid + m->M - 1) / m->M; if (R.parts < 1) R.parts = 1; R.n_tickets = m->M * R.parts; }
