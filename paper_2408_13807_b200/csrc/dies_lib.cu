@@ -717,10 +717,14 @@ extern "C" int dies_run(dies_model* m, uint64_t n_packages, uint64_t seed, const
     const int grid_max = m->n_sms * bps;
     unsigned long long ids = 0;
     for (int i = 0; i < m->M; i++) ids += n_packages * (unsigned long long)(m->has_ext[i] + m->has_point[i]);
-    const unsigned long long per_block = (unsigned long long)kWarps * R.pool;    // packages a block keeps in flight
-    const unsigned long long per_b = (unsigned long long)env_int("DIES_PKG_PER_BLOCK", 32, 1 << 20, (int)per_block);   // small runs: one pool filling per warp
+    // small runs: 32 packages per warp and chunks to match, so that every SM takes part; large runs: the whole grid
+    const unsigned long long per_b = (unsigned long long)env_int("DIES_PKG_PER_BLOCK", 32, 1 << 20, kWarps * 32);
     unsigned long long want = (ids + per_b - 1) / per_b;
     int grid = (int)(want < 1 ? 1 : (want > (unsigned long long)grid_max ? grid_max : want));
+    {
+        const unsigned long long per_warp = ids / ((unsigned long long)grid * kWarps * (unsigned long long)m->M) ;
+        R.chunk = (unsigned)(per_warp < 32 ? 32 : (per_warp > kChunk ? kChunk : per_warp));
+    }
     if (m->M == 1) { R.parts = grid; R.n_tickets = grid; }
     else { R.parts = (8 * grid + m->M - 1) / m->M; if (R.parts < 1) R.parts = 1; R.n_tickets = m->M * R.parts; }
 
@@ -877,6 +881,7 @@ extern "C" int dies_trace_packages(dies_model* m, int model_index, uint64_t firs
     }
     R.n_run = nt; R.id_base = 0;
     R.uniform_q = 0; R.pool = m->pool;                     // the trace kernels keep the quantum per package
+    R.chunk = 32;
     int32_t *d_ev = nullptr, *d_n = nullptr;
     CUDA_TRY(cudaMalloc(&d_ev, (size_t)count * max_events * 16));
     // n_events (count ints) followed by the 64-bit counter the traced package indices are taken from

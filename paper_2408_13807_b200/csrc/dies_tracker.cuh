@@ -26,7 +26,7 @@ constexpr int kBlock = 256;          // threads per block
 constexpr int kWarps = kBlock / 32;
 constexpr int kMinBlocks = 4;        // resident blocks per SM asked from the compiler (64 registers)
 constexpr unsigned kFull = 0xffffffffu;
-constexpr unsigned kChunk = 128;     // package ids a warp takes from the global counter at a time
+constexpr unsigned kChunk = 128;     // package ids a warp takes from the global counter at a time (large runs)
 constexpr int kUnroll = 12;           // crossings per vote in the crossing loop
 constexpr int kMaxPool = 248;        // pool slots per warp (queue entries are bytes)
 constexpr int kGuide = 1024;         // cut-points per CDF row of the guide tables
@@ -126,6 +126,7 @@ struct RunParams {
     int reemit_cell;                 // L253 (R20): re-emit from a random position of the cell volume
     float qscale;                    // 2^S
     int n_tickets, parts;            // tickets = n_models * parts
+    unsigned chunk;                  // package ids a warp takes at a time: kChunk, fewer (>= 32) when a run is small
     int pool;                        // P: pool slots per warp (multiple of 8, 32 <= P <= kMaxPool)
     int thr_hi;                      // crossing phase: swap stopped lanes for ready packages when fewer fly
     int thr_lo;                      // crossing phase: with no ready package left, leave when fewer fly
@@ -529,9 +530,9 @@ __global__ void __launch_bounds__(kBlock, kMinBlocks) dies_track(DeviceModel D, 
                         ch_next += cnt;
                     } else {
                         unsigned long long base = 0;
-                        if (lane == 0) base = atomicAdd(g_next, (unsigned long long)kChunk);
+                        if (lane == 0) base = atomicAdd(g_next, (unsigned long long)R.chunk);
                         base = __shfl_sync(kFull, base, 0);
-                        unsigned long long nend = base + kChunk;
+                        unsigned long long nend = base + R.chunk;
                         if (nend > n_ids) nend = n_ids;
                         if (base >= n_ids) { exhausted = true; nend = base; }
                         if (need && rank >= avail) {
