@@ -723,7 +723,8 @@ extern "C" int dies_run(dies_model* m, uint64_t n_packages, uint64_t seed, const
     int grid = (int)(want < 1 ? 1 : (want > (unsigned long long)grid_max ? grid_max : want));
     {
         const unsigned long long per_warp = ids / ((unsigned long long)grid * kWarps * (unsigned long long)m->M) ;
-        R.chunk = (unsigned)(per_warp < 32 ? 32 : (per_warp > kChunk ? kChunk : per_warp));
+        const unsigned long long cmax = (unsigned long long)env_int("DIES_CHUNK", 32, 4096, (int)kChunk);
+        R.chunk = (unsigned)(per_warp < 32 ? 32 : (per_warp > cmax ? cmax : per_warp));
     }
     if (m->M == 1) { R.parts = grid; R.n_tickets = grid; }
     else { R.parts = (8 * grid + m->M - 1) / m->M; if (R.parts < 1) R.parts = 1; R.n_tickets = m->M * R.parts; }
