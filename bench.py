@@ -28,13 +28,13 @@ if ROOT not in sys.path:
 
 from paper_2408_13807_b200 import sharding, synth  # noqa: E402
 
-# Algorithmic thread-instructions per unit of work in the shipped tracker (profiles/r1p_ncu_full.md):
+# Algorithmic thread-instructions per unit of work in the shipped tracker (profiles/r1q_ncu_full.md):
 # crossing = SASS instructions of one predicated crossing step; scattering / absorption / package = predicated-on
 # thread-instructions executed on the unit's own source lines (shared event stream + its own branch) per unit,
 # from the ncu source page of the same workload.  Queue handling, swaps, votes, fix-ups and idle lanes are NOT work.
-INSTR = dict(crossing=8, scattering=240, absorption=326, package=258)
-# dram__bytes_read.sum + dram__bytes_write.sum of one dies_track launch (ncu --set full, profiles/r1p_ncu_full.md)
-TRAFFIC_BYTES_PER_LAUNCH = 730368
+INSTR = dict(crossing=8, scattering=231, absorption=332, package=252)
+# dram__bytes_read.sum + dram__bytes_write.sum of one dies_track launch (ncu --set full, profiles/r1q_ncu_full.md)
+TRAFFIC_BYTES_PER_LAUNCH = 732160
 SM_COUNT, SCHEDULERS, LANES = 148, 4, 32
 
 
@@ -291,7 +291,7 @@ def run_ours(args, rank, world, local_rank):
                                           frac=c1["absorptions"] / (step_ms * 1e-3) / atom["lane_ops_per_s"],
                                           peak_source=f"dies_bench_atomics({n_shells * min(n_models, 64)} tallies, the run's shell histogram, warp-merged={int(uniform_q)}) on this GPU"),
                               peak_source=f"148 SMs x 4 schedulers x 32 lanes x {sm_max:.0f} MHz ({peak_src})",
-                              instr_per_unit=INSTR, kernel="dies_track<0,false>", kernel_ms=step_ms),
+                              instr_per_unit=INSTR, kernel="dies_track<0,false,false>", kernel_ms=step_ms),
                 wall_s=t_wall)
     # ---- the oracle timed beside it on this box's host cores (rank 0, N = 1 only)
     if world == 1 and not args.no_cpu_baseline:
