@@ -28,6 +28,10 @@ def _problem(name):
         return synth.config3(tau_V=1000.0), {}
     if name == "config4":
         return synth.config4(), dict(ffi=1)
+    if name == "config4_kA":                          # free-path weighting, the comparator of FFI in Fig. 7 (Eq. 8)
+        return synth.config4(ffi=0), dict(k_A=3.0, k_S=2.0)
+    if name == "config3_dir":                         # directional weighting (Eq. 6-7) with sub-cell re-emission (L253)
+        return synth.config3(), dict(g_E=0.5, g_S=0.2, reemit_cell=1)
     raise KeyError(name)
 
 
@@ -38,7 +42,7 @@ def _L_injected(p):
     return L + float(p.L_point)
 
 
-@pytest.mark.parametrize("name", ["config2", "config2_kbg", "config3", "config4"])
+@pytest.mark.parametrize("name", ["config2", "config2_kbg", "config3", "config4", "config4_kA", "config3_dir"])
 def test_sampled_packages_at_full_size(orc, name):
     """64 packages at each of 12 places of the full id range [0, n_packages): identical event lists (type, shell,
     bin, crossings so far) for every package whose decisions sit > 1e-3 from their thresholds in the oracle."""
@@ -126,6 +130,34 @@ def test_full_size_batch_properties(orc):
         o.run(100_000, seed=3, model_index=i)
         To = o.temperature()
         assert np.max(np.abs(T[i][24:] / To[24:] - 1)) < 0.04, i
+    m.close()
+
+
+def test_sampled_packages_of_the_full_size_batch(orc):
+    """Config 5 (1024 spheres x 1e6 packages): 48 packages at 4 places of the id range of models 0, 511 and 1023,
+    followed one by one by the oracle of that sphere (the model index is the fourth word of the Philox counter)."""
+    b = synth.config5()
+    m = dies.Model(batch=b)
+    n_total, max_ev = b.n_packages, 1024
+    Tfix = np.tile(np.linspace(10.0, 40.0, b.rho.shape[1]), (b.n_models, 1))
+    m.dies_set_fixed_temperature(Tfix)
+    safe = same = total = 0
+    for i in (0, 511, 1023):
+        o = orc.Oracle(b.model(i))
+        o.set_fixed_temperature(Tfix[i])
+        for first in np.linspace(0, n_total - 48, 4).astype(np.int64):
+            ev, nev = m.dies_trace_packages(int(first), 48, n_total, seed=13, model_index=i, max_events=max_ev,
+                                            mode=dies.DIES_MODE_FIXED_T)
+            for x in range(48):
+                ref, nref, margin = o.trace(n_total, int(first) + x, seed=13, mode=1, model_index=i, max_events=max_ev)
+                ok = (nref == nev[x]) and nref <= max_ev and np.array_equal(ref, ev[x, :nref])
+                total += 1
+                same += ok
+                if margin > 1e-3 and nref <= max_ev:
+                    safe += 1
+                    assert ok, (i, int(first) + x, margin, ref[:6], ev[x, :6])
+    assert safe > 0.4 * total
+    assert same >= 0.99 * total, same / total
     m.close()
 
 
