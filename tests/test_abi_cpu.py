@@ -83,3 +83,22 @@ def test_synthetic_configs_have_the_stated_shapes():
     b = synth.config5(n_models=16, n_packages=1000)
     assert b.rho.shape == (16, 64) and b.ext_bin_intensity.shape == (16, 100)
     assert 0.1 <= b.meta["tau_V"].min() and b.meta["tau_V"].max() <= 100
+
+
+def test_c_example_compiles_and_links_against_the_library(tmp_path):
+    """examples/c_abi_sphere.c uses include/dies.h from plain C: it must compile without warnings about the
+    declarations and link against libdies.so (it is run on the GPU by tests/test_gpu_c_example.py)."""
+    import os
+    import shutil
+    import subprocess
+    from paper_2408_13807_b200 import build
+    build.build()
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    cuda = os.environ.get("CUDA_HOME", "/usr/local/cuda")
+    pkg = os.path.join(root, "paper_2408_13807_b200")
+    cc = shutil.which("gcc") or shutil.which("cc")
+    r = subprocess.run([cc, "-std=c99", "-Wall", "-Werror", "-O1", "-I" + os.path.join(root, "include"),
+                        "-I" + os.path.join(cuda, "include"), os.path.join(root, "examples", "c_abi_sphere.c"),
+                        "-o", str(tmp_path / "c_abi_sphere"), "-L" + pkg, "-ldies", "-L" + os.path.join(cuda, "lib64"),
+                        "-lcudart", "-lm", "-Wl,-rpath," + pkg], capture_output=True, text=True)
+    assert r.returncode == 0, r.stderr
