@@ -37,8 +37,8 @@ constexpr int kTallyStride = 32;     // 64-bit words between the absorbed-energy
 enum { LC_PACKAGES = 0, LC_CROSSINGS, LC_FFI_CROSSINGS, LC_SCATTERINGS, LC_ABSORPTIONS, LC_ESCAPED, LC_UNINTERACTED,
        LC_TERMINATED, LC_EXTRA_BLOCKS, LC_CLAMP_HI, LC_INJECTED_RAW, LC_TERMINATED_RAW, LC_REWEIGHT_RAW, LC_N };
 
-// per-slot flag word: frequency bin | type of the pending event | (unused) | slot holds a package
-constexpr unsigned KF_K = 0xffffu, KF_EVABS = 1u << 16, KF_DRY = 1u << 17, KF_OCC = 1u << 18;
+// per-slot flag word: frequency bin | type of the pending event | slot holds a package
+constexpr unsigned KF_K = 0xffffu, KF_EVABS = 1u << 16, KF_OCC = 1u << 18;
 // the queues of a warp
 enum { QT_ABS = 0, QT_SCA, QT_SRC, QT_READY, QT_N };
 
@@ -442,8 +442,7 @@ __global__ void __launch_bounds__(kBlock, kMinBlocks) dies_track(DeviceModel D, 
                     if (TRACE) { pkg = pT[slot]; n_ev = pT[P + slot]; ncross = (unsigned)pT[2 * P + slot]; }
                 }
                 int k = (int)(kf & KF_K);
-                constexpr bool dryend = false;                   // (FFI sums its chord inside the launch event: no dry flights)
-                const bool esc = issrc && !dryend && (kf & KF_OCC);
+                const bool esc = issrc && (kf & KF_OCC);
 
                 // (0) free-path weighting (Eq. 8, R17): the quantum the package carries at this event.  Along the
                 //     flight the true survival probability over the biased one is e^{kappa_A (CA - C)} for the
@@ -518,7 +517,7 @@ __global__ void __launch_bounds__(kBlock, kMinBlocks) dies_track(DeviceModel D, 
                 }
                 // (3) free slots take the next package id from the global counter
                 bool launch = false;
-                const bool need = issrc && !dryend;
+                const bool need = issrc;
                 const unsigned needmask = __ballot_sync(kFull, need);
                 if (needmask && !exhausted) {
                     const unsigned cnt = __popc(needmask);
@@ -560,11 +559,11 @@ __global__ void __launch_bounds__(kBlock, kMinBlocks) dies_track(DeviceModel D, 
 
                 // (4) events: launch / scatter / absorb + re-emit; one Philox block each
                 //     (DESIGN.md RNG contract), one instruction stream for all of them
-                bool fly = false, ev_absorb = false, dry = false, uninter = false;
+                bool fly = false, ev_absorb = false, uninter = false;
                 unsigned long long q_inj = 0;
-                if (launch || isev || dryend) {
+                if (launch || isev) {
                     uint32_t xw[4];
-                    const bool atsrc = launch || dryend;                            // the event site is the source
+                    const bool atsrc = launch;                                      // the event site is the source
                     const bool point = atsrc && (mp.has_ext ? ((id - R.id_base) >= R.n_total) : true);
                     unsigned b = blk;
                     philox4x32_10_rk(R.rk, (uint32_t)id, (uint32_t)(id >> 32), b, (uint32_t)m, xw);
@@ -785,7 +784,7 @@ __global__ void __launch_bounds__(kBlock, kMinBlocks) dies_track(DeviceModel D, 
                 //      without escaping through the sentinel (FFI, tau0 = 0) is free again; a slot that got no id dies
                 if (fly || uninter) {
                     const unsigned nkf = uninter ? 0u
-                        : ((unsigned)k | (ev_absorb ? KF_EVABS : 0u) | (dry ? KF_DRY : 0u) | KF_OCC);
+                        : ((unsigned)k | (ev_absorb ? KF_EVABS : 0u) | KF_OCC);
                     sts_f4(aA + 16u * slot, s, b2, col, __uint_as_float(pa));
                     sts_u4(aB + 16u * slot, (unsigned)id, (unsigned)(id >> 32), blk, nkf);
                     if (!R.uniform_q) sts_u64(aQ + 8u * slot, q);
@@ -995,8 +994,8 @@ __global__ void __launch_bounds__(kBlock, kMinBlocks) dies_track(DeviceModel D, 
                         const unsigned kf = lds_u32(aB + 16u * slot + 12u);
                         const bool isev = !alive && (col < 0.f);         // the column ran out: scattering or absorption
                         const unsigned n = ((pa - pa0) >> 3) - (isev ? 1u : 0u);
-                        if (kf & KF_DRY) lc_ffi += n;
-                        else { lc_cross += n; if (TRACE) pT[2 * P + slot] += (int)n; }
+                        lc_cross += n;
+                        if (TRACE) pT[2 * P + slot] += (int)n;
                         // signed coordinate: a runs along the entry ahead (flying) or the one just committed (event)
                         s = ((alive ? pa : pa - 8u) <= tab0) ? -a : a;
                         sts_f4(aA + 16u * slot, s, b2, col, __uint_as_float(pa));
