@@ -2,7 +2,7 @@
  * isotropic external field (PAPER.md L49-55 sources, L87 immediate re-emission), 1e6 packages, full IRE.
  *
  * Build (from the repository root, after `python __graft_entry__.py` has built libdies.so):
- *   gcc -O2 -Iinclude -I/usr/local/cuda/include examples/c_abi_sphere.c -o /tmp/c_abi_sphere \
+ *   gcc -O2 -Iinclude -I/usr/local/cuda/include tests/c_abi/c_abi_sphere.c -o /tmp/c_abi_sphere \
  *       -Lpaper_2408_13807_b200 -ldies -L/usr/local/cuda/lib64 -lcudart -lm \
  *       -Wl,-rpath,$PWD/paper_2408_13807_b200 -Wl,-rpath,/usr/local/cuda/lib64
  * Exit code 0: the run conserved energy (escaping luminosity = injected luminosity, exact integer bookkeeping) and

@@ -86,7 +86,7 @@ def test_synthetic_configs_have_the_stated_shapes():
 
 
 def test_c_example_compiles_and_links_against_the_library(tmp_path):
-    """examples/c_abi_sphere.c uses include/dies.h from plain C: it must compile without warnings about the
+    """tests/c_abi/c_abi_sphere.c uses include/dies.h from plain C: it must compile without warnings about the
     declarations and link against libdies.so (it is run on the GPU by tests/test_gpu_c_example.py)."""
     import os
     import shutil
@@ -98,7 +98,7 @@ def test_c_example_compiles_and_links_against_the_library(tmp_path):
     pkg = os.path.join(root, "paper_2408_13807_b200")
     cc = shutil.which("gcc") or shutil.which("cc")
     r = subprocess.run([cc, "-std=c99", "-Wall", "-Werror", "-O1", "-I" + os.path.join(root, "include"),
-                        "-I" + os.path.join(cuda, "include"), os.path.join(root, "examples", "c_abi_sphere.c"),
+                        "-I" + os.path.join(cuda, "include"), os.path.join(root, "tests", "c_abi", "c_abi_sphere.c"),
                         "-o", str(tmp_path / "c_abi_sphere"), "-L" + pkg, "-ldies", "-L" + os.path.join(cuda, "lib64"),
                         "-lcudart", "-lm", "-Wl,-rpath," + pkg], capture_output=True, text=True)
     assert r.returncode == 0, r.stderr

@@ -1,4 +1,4 @@
-"""The boundary is a C ABI: examples/c_abi_sphere.c (plain C, cudaMalloc + the dies_* calls of include/dies.h, no
+"""The boundary is a C ABI: tests/c_abi/c_abi_sphere.c (plain C, cudaMalloc + the dies_* calls of include/dies.h, no
 Python and no torch in the process) is built with gcc against libdies.so and run on the GPU; the same problem is then
 followed by the oracle and the temperatures compared."""
 import os
@@ -22,7 +22,7 @@ def test_c_program_runs_the_hot_path_through_the_c_abi(tmp_path):
     cc = shutil.which("gcc") or shutil.which("cc")
     assert cc, "no C compiler on this box"
     subprocess.run([cc, "-O2", "-I" + os.path.join(ROOT, "include"), "-I" + os.path.join(CUDA, "include"),
-                    os.path.join(ROOT, "examples", "c_abi_sphere.c"), "-o", exe, "-L" + pkg, "-ldies",
+                    os.path.join(ROOT, "tests", "c_abi", "c_abi_sphere.c"), "-o", exe, "-L" + pkg, "-ldies",
                     "-L" + os.path.join(CUDA, "lib64"), "-lcudart", "-lm", "-Wl,-rpath," + pkg,
                     "-Wl,-rpath," + os.path.join(CUDA, "lib64")], check=True)
     r = subprocess.run([exe], capture_output=True, text=True, timeout=120)
