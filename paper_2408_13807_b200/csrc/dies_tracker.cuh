@@ -501,9 +501,9 @@ __global__ void __launch_bounds__(kBlock, kMinBlocks) dies_track(DeviceModel D, 
                     } else if (isabs) {
                         old = atomicAdd(&gA[j * kTallyStride], q);
                     }
-                    wc_abs += __popc(absmask);
+                    wc_abs += (unsigned)cA;
                 }
-                wc_sca += __popc(__ballot_sync(kFull, issca));
+                wc_sca += (unsigned)cS;
 
                 // (2) escapes (PAPER.md L87 last sentence)
                 const unsigned escmask = __ballot_sync(kFull, esc);
@@ -1005,7 +1005,7 @@ __global__ void __launch_bounds__(kBlock, kMinBlocks) dies_track(DeviceModel D, 
                     {
                         // one store per leaving package: queue t at position (length of t) + (rank among the lanes of t)
                         const unsigned mA = __ballot_sync(kFull, t == QT_ABS), mS = __ballot_sync(kFull, t == QT_SCA);
-                        const unsigned mL = __ballot_sync(kFull, t == QT_SRC), mR = __ballot_sync(kFull, t == QT_READY);
+                        const unsigned mL = __ballot_sync(kFull, t == QT_SRC), mR = leave ? am : 0u;   // flying lanes leave only at the end
                         const unsigned mine = t == QT_ABS ? mA : t == QT_SCA ? mS : t == QT_SRC ? mL : mR;
                         const int base = t == QT_ABS ? nA : t == QT_SCA ? P + nS : t == QT_SRC ? 2 * P + nL : 3 * P + nR;
                         if (out) sts_u8(qA + base + __popc(mine & lt_mask), slot);
