@@ -967,19 +967,20 @@ __global__ void __launch_bounds__(kBlock, kMinBlocks) dies_track(DeviceModel D, 
                         alive = alive && (col >= 0.f);
                         T0 = T1; T1 = T2;
                     }
-                    if (!alive && (col >= 0.f)) {
-                        if (pa <= tab0) {
-                            // an inward entry (c <= 0) whose surface is not reached (tangent shell): head for the outer
-                            // one instead, entry c -> entry 1 - c; the 1 - 2c entries skipped are no passages
-                            const unsigned np = 2u * tab0 + 8u - pa;
-                            pa0 += np - pa;
-                            pa = np;
-                            a = -a;                                  // the coordinate now runs along an outward entry
-                            alive = true;
-                        } else if (pa != pa_out) {
-                            b2 = lds_entry(pa).x;                    // outward, b2 > r^2 by rounding only: graze
-                            alive = true;
-                        }
+                    {
+                        // stopped short of a surface with column left (branch-free: nearly every block has such lanes).
+                        // tang: an inward entry (c <= 0) whose surface is not reached (tangent shell): head for the outer
+                        // one instead, entry c -> entry 1 - c; the 1 - 2c entries skipped are no passages and the
+                        // coordinate now runs along an outward entry.  graze: outward, b2 > r^2 by rounding only.
+                        const bool stop = !alive && (col >= 0.f);
+                        const bool tang = stop && (pa <= tab0);
+                        const bool graze = stop && (pa > tab0) && (pa != pa_out);
+                        const unsigned np = tang ? (2u * tab0 + 8u - pa) : pa;
+                        pa0 += np - pa;
+                        pa = np;
+                        a = tang ? -a : a;
+                        if (graze) b2 = lds_entry(pa).x;
+                        alive = alive || tang || graze;
                     }
                     const unsigned am = __ballot_sync(kFull, alive);
                     const int n_alive = __popc(am);
