@@ -858,19 +858,20 @@ __global__ void __launch_bounds__(kBlock, kMinBlocks) dies_track(DeviceModel D, 
                         }
                         alive = alive && (col <= cA0) && (colS <= cS0);
                     }
-                    if (!alive && (col <= cA0) && (colS <= cS0)) {
-                        if (__float_as_int(E.y) < 0) {
-                            // the inner surface is not reached (tangent shell): head for the outer one instead
-                            // entry c -> entry 1 - c; the 1 - 2c entries skipped are no passages
-                            const unsigned np = 2u * tab0 + 16u - pa;
-                            pa0 += np - pa;
-                            pa = np;
-                            E = lds_entry4(pa);
-                            alive = true;
-                        } else if (pa != pa_out) {
-                            b2 = E.x;                                // outward, b2 > r^2 by rounding only: graze
-                            alive = true;
-                        }
+                    {
+                        // stopped short of a surface with both clocks still running (branch-free, as in the plain block).
+                        // tang: the inner surface is not reached (tangent shell): head for the outer one instead, entry
+                        // c -> entry 1 - c; the 1 - 2c entries skipped are no passages.  graze: outward, b2 > r^2 by
+                        // rounding only.
+                        const bool stop = !alive && (col <= cA0) && (colS <= cS0);
+                        const bool tang = stop && (__float_as_int(E.y) < 0);
+                        const bool graze = stop && !tang && (pa != pa_out);
+                        const unsigned np = tang ? (2u * tab0 + 16u - pa) : pa;
+                        pa0 += np - pa;
+                        pa = np;
+                        if (tang) E = lds_entry4(pa);
+                        if (graze) b2 = E.x;
+                        alive = alive || tang || graze;
                     }
                     const unsigned am = __ballot_sync(kFull, alive);
                     const int n_alive = __popc(am);
