@@ -28,13 +28,14 @@ if ROOT not in sys.path:
 
 from paper_2408_13807_b200 import sharding, synth  # noqa: E402
 
-# Algorithmic thread-instructions per unit of work in the shipped tracker (profiles/r1q_ncu_full.md):
+# Algorithmic thread-instructions per unit of work in the shipped tracker (profiles/r1q_ncu_full.md and
+# r1r_ncu_full.md):
 # crossing = SASS instructions of one predicated crossing step; scattering / absorption / package = predicated-on
 # thread-instructions executed on the unit's own source lines (shared event stream + its own branch) per unit,
 # from the ncu source page of the same workload.  Queue handling, swaps, votes, fix-ups and idle lanes are NOT work.
 INSTR = dict(crossing=8, scattering=231, absorption=332, package=252)
-# dram__bytes_read.sum + dram__bytes_write.sum of one dies_track launch (ncu --set full, profiles/r1q_ncu_full.md)
-TRAFFIC_BYTES_PER_LAUNCH = 732160
+# dram__bytes_read.sum + dram__bytes_write.sum of one dies_track launch (ncu --set full, profiles/r1r_ncu_full.md)
+TRAFFIC_BYTES_PER_LAUNCH = 734464
 SM_COUNT, SCHEDULERS, LANES = 148, 4, 32
 
 
