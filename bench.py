@@ -313,6 +313,35 @@ def run_ours(args, rank, world, local_rank):
     m.close()
 
 
+def run_noise_study(args):
+    """Config 4 (BASELINE.json: "noise per shell vs packages reported"; section 3.2): standard deviation
+    of the shell temperatures over 8 seeds against the number of packages, forced first interaction on and off.
+    One JSON line; every run goes through the C ABI (dies_run + dies_get_temperature), nothing is timed here."""
+    import torch
+    from paper_2408_13807_b200 import binding as dies
+    dev = torch.device("cuda", 0)
+    torch.cuda.set_device(dev)
+    seeds = list(range(1, 9))
+    rows = []
+    for ffi in (0, 1):
+        p = synth.config4(ffi=ffi)
+        m = dies.Model(p, device=str(dev))
+        for n in (10**5, 10**6, 10**7, 10**8):
+            T = []
+            for sd in seeds:
+                m.dies_run(n, seed=sd, k_bg=0.5, ffi=ffi)
+                T.append(m.dies_get_temperature())
+            T = np.array(T)
+            rel = T.std(0, ddof=1) / T.mean(0)
+            h = p.n_shells // 2
+            rows.append(dict(ffi=ffi, packages=n, rel_sigma_T_mean=float(rel.mean()), rel_sigma_T_max=float(rel.max()),
+                             rel_sigma_T_inner_half=float(rel[:h].mean()), rel_sigma_T_outer_half=float(rel[h:].mean()),
+                             T_mean_K=float(T.mean())))
+        m.close()
+    print(json.dumps(dict(study="config4 noise per shell vs packages", seeds=len(seeds), n_shells=p.n_shells,
+                          data="synthetic", rows=rows)))
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -327,11 +356,15 @@ def main():
     ap.add_argument("--ref-total", type=int, default=20_000_000)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--cpu-all-cores", action="store_true", help="also time the oracle on all host cores (one process each)")
+    ap.add_argument("--noise-study", action="store_true", help="config 4: sigma_T per shell over 8 seeds vs packages, FFI on / off")
     args = ap.parse_args()
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
-    if args.impl == "reference":
+    if args.noise_study:
+        if rank == 0:
+            run_noise_study(args)
+    elif args.impl == "reference":
         run_reference(args, rank, world)
     else:
         if args.warmup < 3:
