@@ -191,6 +191,8 @@ def run_ours(args, rank, world, local_rank):
     torch.cuda.set_device(dev)
     if world > 1:
         dist.init_process_group("nccl", device_id=dev)
+    if args.tune:
+        dies.dies_set_tuning(**{k: int(v) for k, v in (kv.split("=") for kv in args.tune.split(","))})
     p = make_problem(args.workload, args.packages)
     batch = isinstance(p, synth.BatchProblem)
     n_models = p.n_models if batch else 1
@@ -355,6 +357,7 @@ def main():
     ap.add_argument("--ref-sample", type=int, default=1_000_000)
     ap.add_argument("--ref-total", type=int, default=20_000_000)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--tune", default="", help="launch tuning for dies_set_tuning, e.g. visit=2,slots_uniform=5 (include/dies.h: dies_tuning)")
     ap.add_argument("--cpu-all-cores", action="store_true", help="also time the oracle on all host cores (one process each)")
     ap.add_argument("--noise-study", action="store_true", help="config 4: sigma_T per shell over 8 seeds vs packages, FFI on / off")
     args = ap.parse_args()

@@ -171,6 +171,26 @@ int dies_get_tables(dies_model*, double* eps, float* F);
 int dies_bench_atomics(int n_addr, const double* weights, int aggregate, int iters, double* lane_ops_per_s,
                        double* atomics_per_s);
 
+/* Launch tuning of the trackers (process-wide; the defaults are the measured optimum on config 2).
+ * It is not part of the method: integer tallies of fixed-temperature runs do not depend on it at all, full-IRE results
+ * only through the order of absorptions (within noise).  Fields that are 0 keep their current value;
+ * dies_set_tuning(NULL) restores the defaults; out-of-range values give DIES_EINVAL and change nothing. */
+typedef struct {
+    int32_t slots_uniform;  /* dies_fly: pool slots per lane when all packages carry one quantum, 1..8 (default 5)   */
+    int32_t slots;          /* dies_fly: the same with per-package quanta (k_bg, FFI, two sources), 1..8 (4)         */
+    int32_t visit;          /* dies_fly: crossing blocks between two event phases, 1..64 (3)                         */
+    int32_t thr_idle;       /* dies_fly: partial event batches while at least this many lanes starve, 1..32 (4)      */
+    int32_t chunk;          /* package ids a warp takes from the global counter at a time, 32..4096 (128)            */
+    int32_t pkg_per_block;  /* grid sizing of small runs: packages per block, 32..2^20 (256)                         */
+    int32_t w_pool;         /* dies_track (weighted runs): pool slots per warp, 32..248 (96)                         */
+    int32_t w_thr_hi;       /* dies_track: swap stopped lanes for ready packages when fewer fly, 1..32 (20)          */
+    int32_t w_thr_lo;       /* dies_track: with no ready package left, leave when fewer fly, 1..32 (16)              */
+    int32_t w_min_ready;    /* dies_track: mixed event batches only while fewer packages are ready, 1..248 (32)      */
+    int32_t atom_stride;    /* dies_bench_atomics: 64-bit words between two tallies, 1..64 (32)                      */
+} dies_tuning;
+int dies_set_tuning(const dies_tuning* t);
+int dies_get_tuning(dies_tuning* t);
+
 int dies_destroy(dies_model*);
 const char* dies_last_error(void);
 /* "sm_100a" build tag, number of SMs and resident blocks per SM of the tracker (for the bench log). */

@@ -24,7 +24,7 @@ EXPORTS = ("dies_workspace_bytes", "dies_create_model", "dies_create_batch", "di
            "dies_set_sources_batch", "dies_run", "dies_run_batch", "dies_get_temperature", "dies_get_escape_spectrum",
            "dies_set_fixed_temperature", "dies_get_absorbed", "dies_get_counters", "dies_trace_packages",
            "dies_trace_package", "dies_test_philox", "dies_get_tables", "dies_destroy", "dies_last_error",
-           "dies_device_info", "dies_bench_atomics", "dies_seek")
+           "dies_device_info", "dies_bench_atomics", "dies_seek", "dies_set_tuning", "dies_get_tuning")
 
 
 class DiesError(RuntimeError):
@@ -38,6 +38,11 @@ class dies_run_opts(C.Structure):
                 ("fixed_shift", C.c_int32), ("n_total", C.c_uint64), ("k_A", C.c_double),
                 ("k_A_dilute", C.c_double), ("k_S", C.c_double), ("g_E", C.c_double), ("g_S", C.c_double),
                 ("use_g_S", C.c_int32), ("reemit_in_cell", C.c_int32)]
+
+
+class dies_tuning(C.Structure):
+    _fields_ = [(n, C.c_int32) for n in ("slots_uniform", "slots", "visit", "thr_idle", "chunk", "pkg_per_block",
+                                         "w_pool", "w_thr_hi", "w_thr_lo", "w_min_ready", "atom_stride")]
 
 
 _dp = C.POINTER(C.c_double)
@@ -78,6 +83,8 @@ def lib():
     L.dies_last_error.restype = C.c_char_p
     L.dies_device_info.argtypes = [C.POINTER(C.c_int)] * 3
     L.dies_bench_atomics.argtypes = [C.c_int, _dp, C.c_int, C.c_int, _dp, _dp]
+    L.dies_set_tuning.argtypes = [C.POINTER(dies_tuning)]
+    L.dies_get_tuning.argtypes = [C.POINTER(dies_tuning)]
     _lib = L
     return L
 
@@ -105,6 +112,21 @@ def dies_device_info():
     a, b, c = C.c_int(), C.c_int(), C.c_int()
     _chk(lib().dies_device_info(C.byref(a), C.byref(b), C.byref(c)))
     return dict(n_sms=a.value, blocks_per_sm=b.value, threads_per_block=c.value)
+
+
+def dies_set_tuning(**fields):
+    """Launch tuning of the trackers (include/dies.h: dies_tuning); no fields restores the defaults."""
+    if not fields:
+        _chk(lib().dies_set_tuning(None))
+        return
+    t = dies_tuning(**{k: int(v) for k, v in fields.items()})
+    _chk(lib().dies_set_tuning(C.byref(t)))
+
+
+def dies_get_tuning():
+    t = dies_tuning()
+    _chk(lib().dies_get_tuning(C.byref(t)))
+    return {n: getattr(t, n) for n, _ in dies_tuning._fields_}
 
 
 def dies_bench_atomics(n_addr, weights=None, aggregate=1, iters=2000):

@@ -1,14 +1,17 @@
 // dies_lib.cu -- C ABI of libdies (include/dies.h): host argument checking, device table construction,
-// launches of the tracker (dies_tracker.cuh) and read-back.  Compiled for sm_100a only; no CPU fallback.
+// launches of the trackers (dies_fly.cuh: runs with weights fixed at launch; dies_tracker.cuh: runs with free-path or
+// directional weighting) and read-back.  Compiled for sm_100a only; no CPU fallback.
 #include <cmath>
 #include <cstdarg>
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <mutex>
 #include <vector>
 
 #include "../../include/dies.h"
 #include "dies_tracker.cuh"
+#include "dies_fly.cuh"
 
 using namespace dies;
 
@@ -407,35 +410,124 @@ static int check_device()
     return DIES_OK;
 }
 
-static int env_int(const char* name, int lo, int hi, int dflt)
+// ------------------------------------------------------------------ launch tuning (include/dies.h: dies_tuning)
+static const dies_tuning kTuningDefaults = {5, 4, 6, 8, (int32_t)kChunk, kFlyWarps * 32, 96, 20, 16, 32, kTallyStride};
+static dies_tuning g_tuning = kTuningDefaults;
+static std::mutex g_tuning_mutex;
+
+static dies_tuning tuning()
 {
-    const char* e = getenv(name);
-    if (e) { int v = atoi(e); if (v >= lo && v <= hi) return v; }
-    return dflt;
+    std::lock_guard<std::mutex> lock(g_tuning_mutex);
+    return g_tuning;
 }
 
-// pool slots per warp: a multiple of 8 in [32, kMaxPool]
+extern "C" int dies_set_tuning(const dies_tuning* t)
+{
+    std::lock_guard<std::mutex> lock(g_tuning_mutex);
+    if (!t) { g_tuning = kTuningDefaults; return DIES_OK; }
+    dies_tuning n = g_tuning;
+    struct { int32_t dies_tuning::*f; int lo, hi; const char* name; } spec[] = {
+        {&dies_tuning::slots_uniform, 1, kMaxSlots, "slots_uniform"}, {&dies_tuning::slots, 1, kMaxSlots, "slots"},
+        {&dies_tuning::visit, 1, 64, "visit"}, {&dies_tuning::thr_idle, 1, 32, "thr_idle"},
+        {&dies_tuning::chunk, 32, 4096, "chunk"}, {&dies_tuning::pkg_per_block, 32, 1 << 20, "pkg_per_block"},
+        {&dies_tuning::w_pool, 32, kMaxPool, "w_pool"}, {&dies_tuning::w_thr_hi, 1, 32, "w_thr_hi"},
+        {&dies_tuning::w_thr_lo, 1, 32, "w_thr_lo"}, {&dies_tuning::w_min_ready, 1, kMaxPool, "w_min_ready"},
+        {&dies_tuning::atom_stride, 1, 64, "atom_stride"}};
+    for (auto& sp : spec) {
+        const int v = t->*(sp.f);
+        if (v == 0) continue;
+        if (v < sp.lo || v > sp.hi) return fail(DIES_EINVAL, "dies_set_tuning: %s must be in [%d, %d]", sp.name, sp.lo, sp.hi);
+        n.*(sp.f) = v;
+    }
+    n.w_pool &= ~7;
+    g_tuning = n;
+    return DIES_OK;
+}
+
+extern "C" int dies_get_tuning(dies_tuning* t)
+{
+    if (!t) return fail(DIES_EINVAL, "NULL argument");
+    *t = tuning();
+    return DIES_OK;
+}
+
+// pool slots per lane of dies_fly
 // (with per-package quanta | with one quantum for all packages: 8 bytes less per slot, so a deeper pool fits)
-static int pool_slots(bool uniform_q)
+static int fly_slots(bool uniform_q) { const dies_tuning t = tuning(); return uniform_q ? t.slots_uniform : t.slots; }
+
+static size_t fly_smem(int N, int K, int nT, int M, bool trace, bool with_q, int logc)
 {
-    return (uniform_q ? env_int("DIES_POOL_U", 32, kMaxPool, 120) : env_int("DIES_POOL", 32, kMaxPool, 96)) & ~7;
+    const int ldS = N + 1, ldT = 2 * ldS + 2;
+    return plan_fly(K, nT, ldS, ldT, M, trace, with_q, logc).total;
 }
 
+// Launch shape of dies_fly for a model: 16 interleaved copies of the shell table when they fit beside a pool of at
+// least 3 slots per lane, else one copy; the pool as deep as asked for, or as fits.
+constexpr size_t kFlySmemMax = 227 * 1024;
+static bool fly_shape(int N, int K, int nT, int want_slots, bool trace, bool with_q, int* logc, int* slots)
+{
+    for (int lc = 4; lc >= 0; lc -= 4) {
+        const int least = lc ? (want_slots < 3 ? want_slots : 3) : 1;
+        for (int M = want_slots; M >= least; M--)
+            if (fly_smem(N, K, nT, M, trace, with_q, lc) <= kFlySmemMax) { *logc = lc; *slots = M; return true; }
+    }
+    return false;
+}
+
+// shared memory of dies_track (weighted runs)
 static size_t tracker_smem(int N, int K, int nT, int P, bool trace, bool with_q, bool wt = false)
 {
     const int ldS = N + 1, ldT = 2 * ldS + 2;
     return plan_smem(K, nT, ldS, ldT, P, trace, with_q, wt).total;
 }
 
-template <int MODE, bool TRACE>
-static cudaError_t set_smem(size_t bytes)
+// Dynamic shared memory a kernel may be launched with: raised per device and only upwards (a model that needs less
+// must not lower it under a model that needs more), under a mutex (handles of different threads are independent).
+enum { KF_FLY = 0 /* + mode + 2 trace + 4 (one table copy) */, KF_TRK0 = 8, KF_TRK1, KF_TRK0T, KF_TRK1T, KF_N };
+static int fly_kernel(int mode, bool trace, int logc) { return KF_FLY + (mode == DIES_MODE_IRE ? 0 : 1) + (trace ? 2 : 0) + (logc ? 0 : 4); }
+static const void* kernel_fn(int which)
 {
-    static size_t granted = 0;                       // per kernel pair: raise the limit only when a model needs more
-    if (bytes <= granted) return cudaSuccess;
-    granted = bytes;
-    cudaError_t e = cudaFuncSetAttribute(dies_track<MODE, TRACE, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
+    switch (which) {
+    case 0: return (const void*)dies_fly<0, false, 4>;
+    case 1: return (const void*)dies_fly<1, false, 4>;
+    case 2: return (const void*)dies_fly<0, true, 4>;
+    case 3: return (const void*)dies_fly<1, true, 4>;
+    case 4: return (const void*)dies_fly<0, false, 0>;
+    case 5: return (const void*)dies_fly<1, false, 0>;
+    case 6: return (const void*)dies_fly<0, true, 0>;
+    case 7: return (const void*)dies_fly<1, true, 0>;
+    case KF_TRK0: return (const void*)dies_track<0, false, true>;
+    case KF_TRK1: return (const void*)dies_track<1, false, true>;
+    case KF_TRK0T: return (const void*)dies_track<0, true, true>;
+    default: return (const void*)dies_track<1, true, true>;
+    }
+}
+static void launch_fly(int which, int grid, size_t smem, cudaStream_t st, const DeviceModel& D, const RunParams& R,
+                       const TraceParams& tp, const FlyPlan& fp)
+{
+    switch (which) {
+    case 0: dies_fly<0, false, 4><<<grid, kFlyBlock, smem, st>>>(D, R, tp, fp); break;
+    case 1: dies_fly<1, false, 4><<<grid, kFlyBlock, smem, st>>>(D, R, tp, fp); break;
+    case 2: dies_fly<0, true, 4><<<grid, kFlyBlock, smem, st>>>(D, R, tp, fp); break;
+    case 3: dies_fly<1, true, 4><<<grid, kFlyBlock, smem, st>>>(D, R, tp, fp); break;
+    case 4: dies_fly<0, false, 0><<<grid, kFlyBlock, smem, st>>>(D, R, tp, fp); break;
+    case 5: dies_fly<1, false, 0><<<grid, kFlyBlock, smem, st>>>(D, R, tp, fp); break;
+    case 6: dies_fly<0, true, 0><<<grid, kFlyBlock, smem, st>>>(D, R, tp, fp); break;
+    default: dies_fly<1, true, 0><<<grid, kFlyBlock, smem, st>>>(D, R, tp, fp); break;
+    }
+}
+static cudaError_t grant_smem(int which, size_t bytes)
+{
+    static std::mutex mu;
+    static size_t granted[64][KF_N] = {};
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
     if (e != cudaSuccess) return e;
-    return cudaFuncSetAttribute(dies_track<MODE, TRACE, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
+    std::lock_guard<std::mutex> lock(mu);
+    if (dev >= 0 && dev < 64 && bytes <= granted[dev][which]) return cudaSuccess;
+    e = cudaFuncSetAttribute(kernel_fn(which), cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
+    if (e == cudaSuccess && dev >= 0 && dev < 64) granted[dev][which] = bytes;
+    return e;
 }
 
 extern "C" int dies_workspace_bytes(int n_shells, int n_freq, int n_T, int n_models, size_t* bytes)
@@ -452,10 +544,10 @@ extern "C" int dies_device_info(int* n_sms, int* blocks_per_sm, int* threads_per
     int dev = 0, sms = 0, bps = 0;
     CUDA_TRY(cudaGetDevice(&dev));
     CUDA_TRY(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
-    CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&bps, dies_track<0, false, false>, kBlock, tracker_smem(100, 200, 1000, pool_slots(true), false, false)));
+    bps = 1;                                     // dies_fly: one block of kFlyBlock threads per SM
     if (n_sms) *n_sms = sms;
     if (blocks_per_sm) *blocks_per_sm = bps;
-    if (threads_per_block) *threads_per_block = kBlock;
+    if (threads_per_block) *threads_per_block = kFlyBlock;
     return DIES_OK;
 }
 
@@ -494,14 +586,12 @@ extern "C" int dies_create_batch(int n_models, int n_shells, const double* r_bou
     if (rc) return rc;
     const Layout L = make_layout(N, K, nT, M);
     if (workspace_bytes < L.total) return fail(DIES_ENOMEM, "workspace too small: %zu < %zu", workspace_bytes, L.total);
-    const int pool = pool_slots(false);
-    size_t smem = tracker_smem(N, K, nT, pool, false, true);
-    const size_t smem_u = tracker_smem(N, K, nT, pool_slots(true), false, false);
-    if (smem_u > smem) smem = smem_u;                       // largest of the two launch shapes
-    const size_t smem_trace = tracker_smem(N, K, nT, pool, true, true, true);
-    const size_t smem_w = tracker_smem(N, K, nT, pool, false, true, true);
-    if (smem_w > smem) smem = smem_w;
-    if (smem_trace > 200 * 1024) return fail(DIES_EINVAL, "tables do not fit in shared memory (%zu bytes)", smem_trace);
+    // the smallest launch shapes of the two trackers must fit (the shapes of a run are chosen in dies_run)
+    const int pool = tuning().w_pool;
+    const size_t smem = fly_smem(N, K, nT, 1, false, true, 0);
+    const size_t smem_trace = tracker_smem(N, K, nT, 32, true, true, true);
+    if (smem_trace > 200 * 1024 || fly_smem(N, K, nT, 1, true, true, 0) > kFlySmemMax)
+        return fail(DIES_EINVAL, "tables do not fit in shared memory (%zu bytes)", smem_trace);
 
     dies_model* m = new (std::nothrow) dies_model();
     if (!m) return fail(DIES_ENOMEM, "host allocation failed");
@@ -547,15 +637,10 @@ extern "C" int dies_create_batch(int n_models, int n_shells, const double* r_bou
     TRY_OR_FREE(cudaGetLastError());
     if (hflags[0] & 1) { delete m; return fail(DIES_EINVAL, "emis must be >= 0 and non-decreasing with T in every bin"); }
     if (hflags[0] & 2) { delete m; return fail(DIES_EINVAL, "row sums of emis must strictly increase with T"); }
-    TRY_OR_FREE((set_smem<0, false>(smem)));
-    TRY_OR_FREE((set_smem<1, false>(smem)));
-    TRY_OR_FREE((set_smem<0, true>(smem_trace)));
-    TRY_OR_FREE((set_smem<1, true>(smem_trace)));
     int dev = 0;
     TRY_OR_FREE(cudaGetDevice(&dev));
     TRY_OR_FREE(cudaDeviceGetAttribute(&m->n_sms, cudaDevAttrMultiProcessorCount, dev));
-    TRY_OR_FREE(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&m->blocks_per_sm, dies_track<0, false, false>, kBlock, smem));
-    if (m->blocks_per_sm < 1) { delete m; return fail(DIES_ECUDA, "tracker does not fit on an SM"); }
+    m->blocks_per_sm = 1;
     m->grid_max = m->n_sms * m->blocks_per_sm;
 #undef TRY_OR_FREE
     *out = m;
@@ -616,6 +701,8 @@ extern "C" int dies_set_sources_batch(dies_model* m, const double* ext, const do
                                                         wsp<unsigned short>(m, m->L.guideS));
     m->launches += 2;
     CUDA_TRY(cudaGetLastError());
+    // the tables are built on the legacy default stream; dies_run may use any stream (also a non-blocking one)
+    CUDA_TRY(cudaDeviceSynchronize());
     m->sources_set = any;
     m->ran = false; m->done = 0;
     return DIES_OK;
@@ -675,10 +762,11 @@ static int fill_run_params(dies_model* m, uint64_t n_packages, uint64_t seed, co
     R->g_E = (float)d.g_E; R->g_S = (float)d.g_S; R->use_gS = d.use_g_S ? 1 : 0;
     R->reemit_cell = d.reemit_in_cell ? 1 : 0;
     R->qscale = (float)(1u << d.fixed_shift);
-    R->pool = pool_slots(R->uniform_q != 0);
-    R->thr_hi = env_int("DIES_THR_HI", 1, 32, 20);
-    R->thr_lo = env_int("DIES_THR_LO", 1, 32, 16);
-    R->min_ready = env_int("DIES_MIN_READY", 1, kMaxPool, 32);
+    const dies_tuning tn = tuning();
+    R->pool = tn.w_pool;
+    R->thr_hi = tn.w_thr_hi; R->thr_lo = tn.w_thr_lo; R->min_ready = tn.w_min_ready;
+    R->slots = fly_slots(R->uniform_q != 0);
+    R->visit = tn.visit; R->thr_idle = tn.thr_idle;
     R->n_tickets = 0; R->parts = 1;
     return DIES_OK;
 }
@@ -708,22 +796,28 @@ extern "C" int dies_run(dies_model* m, uint64_t n_packages, uint64_t seed, const
 
     // launch shape: shared memory of this run's pool, persistent blocks (as many as fit on an SM), fewer for tiny runs
     const bool wt = R.weighted != 0;
-    const size_t smem_launch = tracker_smem(m->N, m->K, m->nT, R.pool, false, !R.uniform_q, wt);
-    const void* kfun = mode == DIES_MODE_IRE ? (wt ? (const void*)dies_track<0, false, true> : (const void*)dies_track<0, false, false>)
-                                             : (wt ? (const void*)dies_track<1, false, true> : (const void*)dies_track<1, false, false>);
+    const dies_tuning tn = tuning();
+    int logc = 0;
+    if (!wt && !fly_shape(m->N, m->K, m->nT, R.slots, false, !R.uniform_q, &logc, &R.slots))
+        return fail(DIES_ECUDA, "tracker does not fit on an SM");
+    const int kf = wt ? (mode == DIES_MODE_IRE ? KF_TRK0 : KF_TRK1) : fly_kernel(mode, false, logc);
+    const FlyPlan fp = plan_fly(m->K, m->nT, m->ldS, m->D.ldT, R.slots, false, !R.uniform_q, logc);
+    const size_t smem_launch = wt ? tracker_smem(m->N, m->K, m->nT, R.pool, false, !R.uniform_q, true) : fp.total;
+    const int threads = wt ? kBlock : kFlyBlock, warps = threads / 32;
+    CUDA_TRY(grant_smem(kf, smem_launch));
     int bps = 0;
-    CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&bps, kfun, kBlock, smem_launch));
+    CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&bps, kernel_fn(kf), threads, smem_launch));
     if (bps < 1) return fail(DIES_ECUDA, "tracker does not fit on an SM");
     const int grid_max = m->n_sms * bps;
     unsigned long long ids = 0;
     for (int i = 0; i < m->M; i++) ids += n_packages * (unsigned long long)(m->has_ext[i] + m->has_point[i]);
     // small runs: 32 packages per warp and chunks to match, so that every SM takes part; large runs: the whole grid
-    const unsigned long long per_b = (unsigned long long)env_int("DIES_PKG_PER_BLOCK", 32, 1 << 20, kWarps * 32);
+    const unsigned long long per_b = wt ? (unsigned long long)(kWarps * 32) : (unsigned long long)tn.pkg_per_block;
     unsigned long long want = (ids + per_b - 1) / per_b;
     int grid = (int)(want < 1 ? 1 : (want > (unsigned long long)grid_max ? grid_max : want));
     {
-        const unsigned long long per_warp = ids / ((unsigned long long)grid * kWarps * (unsigned long long)m->M) ;
-        const unsigned long long cmax = (unsigned long long)env_int("DIES_CHUNK", 32, 4096, (int)kChunk);
+        const unsigned long long per_warp = ids / ((unsigned long long)grid * warps * (unsigned long long)m->M) ;
+        const unsigned long long cmax = (unsigned long long)tn.chunk;
         R.chunk = (unsigned)(per_warp < 32 ? 32 : (per_warp > cmax ? cmax : per_warp));
     }
     if (m->M == 1) { R.parts = grid; R.n_tickets = grid; }
@@ -744,8 +838,7 @@ extern "C" int dies_run(dies_model* m, uint64_t n_packages, uint64_t seed, const
         if (mode == DIES_MODE_IRE) dies_track<0, false, true><<<grid, kBlock, smem_launch, st>>>(m->D, R, tp);
         else dies_track<1, false, true><<<grid, kBlock, smem_launch, st>>>(m->D, R, tp);
     } else {
-        if (mode == DIES_MODE_IRE) dies_track<0, false, false><<<grid, kBlock, smem_launch, st>>>(m->D, R, tp);
-        else dies_track<1, false, false><<<grid, kBlock, smem_launch, st>>>(m->D, R, tp);
+        launch_fly(kf, grid, smem_launch, st, m->D, R, tp, fp);
     }
     m->launches += 2;
     CUDA_TRY(cudaGetLastError());
@@ -881,7 +974,8 @@ extern "C" int dies_trace_packages(dies_model* m, int model_index, uint64_t firs
         m->launches += 1;
     }
     R.n_run = nt; R.id_base = 0;
-    R.uniform_q = 0; R.pool = m->pool;                     // the trace kernels keep the quantum per package
+    R.uniform_q = 0;                                       // the trace kernels keep the quantum per package
+    R.slots = fly_slots(false);
     R.chunk = 32;
     int32_t *d_ev = nullptr, *d_n = nullptr;
     CUDA_TRY(cudaMalloc(&d_ev, (size_t)count * max_events * 16));
@@ -891,19 +985,34 @@ extern "C" int dies_trace_packages(dies_model* m, int model_index, uint64_t firs
     cudaMemset(d_n, 0, n_bytes);
     TraceParams tp = {model_index, first_id, count, d_ev, max_events, d_n,
                       reinterpret_cast<unsigned long long*>(reinterpret_cast<unsigned char*>(d_n) + n_bytes - 8)};
-    int grid = (count + kBlock - 1) / kBlock;
-    if (grid > m->grid_max) grid = m->grid_max;
+    cudaError_t ge = cudaSuccess;
     if (R.weighted) {
+        int grid = (count + kBlock - 1) / kBlock;
+        if (grid > 4 * m->n_sms) grid = 4 * m->n_sms;
         const int nw = m->M * (2 * m->ldS + 2);
         k_build_wshells<<<(nw + 127) / 128, 128>>>(wsp<double>(m, m->L.rb), wsp<double>(m, m->L.rho), m->N, m->M, m->kref,
                                                   R.k_A, R.k_A_dilute, wsp<float4>(m, m->L.stabW));
         m->launches += 1;
-        if (mode == DIES_MODE_IRE) dies_track<0, true, true><<<grid, kBlock, m->smem_trace_bytes>>>(m->D, R, tp);
-        else dies_track<1, true, true><<<grid, kBlock, m->smem_trace_bytes>>>(m->D, R, tp);
+        const size_t sm = tracker_smem(m->N, m->K, m->nT, R.pool, true, true, true);
+        ge = grant_smem(mode == DIES_MODE_IRE ? KF_TRK0T : KF_TRK1T, sm);
+        if (ge == cudaSuccess) {
+            if (mode == DIES_MODE_IRE) dies_track<0, true, true><<<grid, kBlock, sm>>>(m->D, R, tp);
+            else dies_track<1, true, true><<<grid, kBlock, sm>>>(m->D, R, tp);
+        }
     } else {
-        if (mode == DIES_MODE_IRE) dies_track<0, true, false><<<grid, kBlock, m->smem_trace_bytes>>>(m->D, R, tp);
-        else dies_track<1, true, false><<<grid, kBlock, m->smem_trace_bytes>>>(m->D, R, tp);
+        int grid = (count + kFlyBlock - 1) / kFlyBlock;
+        if (grid > m->grid_max) grid = m->grid_max;
+        int logc = 0;
+        if (!fly_shape(m->N, m->K, m->nT, R.slots, true, true, &logc, &R.slots)) {
+            cudaFree(d_ev); cudaFree(d_n);
+            return fail(DIES_ECUDA, "tracker does not fit on an SM");
+        }
+        const FlyPlan fp = plan_fly(m->K, m->nT, m->ldS, m->D.ldT, R.slots, true, true, logc);
+        const int kf = fly_kernel(mode, true, logc);
+        ge = grant_smem(kf, fp.total);
+        if (ge == cudaSuccess) launch_fly(kf, grid, fp.total, 0, m->D, R, tp, fp);
     }
+    if (ge != cudaSuccess) { cudaFree(d_ev); cudaFree(d_n); return fail(DIES_ECUDA, "trace: %s", cudaGetErrorString(ge)); }
     m->launches += 1;
     cudaError_t e = cudaDeviceSynchronize();
     if (e == cudaSuccess) e = cudaMemcpy(events, d_ev, (size_t)count * max_events * 16, cudaMemcpyDeviceToHost);
@@ -972,7 +1081,7 @@ __global__ void k_bench_atomics(unsigned long long* tallies, int n_addr, int str
 extern "C" int dies_bench_atomics(int n_addr, const double* weights, int aggregate, int iters, double* lane_ops_per_s,
                                   double* atomics_per_s)
 {
-    const int stride = env_int("DIES_ATOM_STRIDE", 1, 64, kTallyStride);     // 64-bit words between two tallies
+    const int stride = tuning().atom_stride;     // 64-bit words between two tallies
     if (n_addr < 1 || n_addr > 65535 || iters < 1 || !lane_ops_per_s || !atomics_per_s)
         return fail(DIES_EINVAL, "bad arguments");
     // look-up table of the histogram: entry e holds the tally whose cumulative weight covers (e + 0.5) / 4096

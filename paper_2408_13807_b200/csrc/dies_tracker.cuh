@@ -131,6 +131,9 @@ struct RunParams {
     int thr_hi;                      // crossing phase: swap stopped lanes for ready packages when fewer fly
     int thr_lo;                      // crossing phase: with no ready package left, leave when fewer fly
     int min_ready;                   // event phase: mixed batches only while fewer packages are ready
+    int slots;                       // dies_fly: pool slots per lane (1 <= slots <= kMaxSlots)
+    int visit;                       // dies_fly: crossing blocks between two event phases
+    int thr_idle;                    // dies_fly: partial event batches while at least this many lanes starve
 };
 
 struct TraceParams {
@@ -267,11 +270,14 @@ __device__ __forceinline__ int sample_cdf(const float* __restrict__ cdf, const u
     return k;
 }
 
-// t(eps) = #{j : grid[j] <= eps} clamped to n-1, given a lower bound t0 <= t(eps): the table row of a cell
-// emitting eps (R4).  Rows only move up during a run, so the scan from the block's last known row is short.
+// t(eps) = #{j : grid[j] <= eps} clamped to n-1, from a hint t0 near t(eps): the table row of a cell emitting eps
+// (R4).  Rows only move up during a run, so the scan from the block's last known row is short.  The hint is shared by
+// the warps of a block: a warp whose atomic returned an older (smaller) tally than the one the hint was raised for
+// first steps down to its own row.
 __device__ __forceinline__ int row_from(const float* grid, int n, int t0, float eps)
 {
     int t = t0;
+    while (t > 0 && grid[t - 1] > eps) t--;
     if (grid[min(t + 8, n - 1)] <= eps) {          // far away (first touch of a shell): bisect (t+8, n]
         int lo = min(t + 8, n - 1) + 1, hi = n;
         while (lo < hi) {
