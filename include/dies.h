@@ -178,8 +178,8 @@ int dies_bench_atomics(int n_addr, const double* weights, int aggregate, int ite
 typedef struct {
     int32_t slots_uniform;  /* dies_fly: pool slots per lane when all packages carry one quantum, 1..8 (default 5)   */
     int32_t slots;          /* dies_fly: the same with per-package quanta (k_bg, FFI, two sources), 1..8 (4)         */
-    int32_t visit;          /* dies_fly: crossing blocks between two event phases, 1..64 (3)                         */
-    int32_t thr_idle;       /* dies_fly: partial event batches while at least this many lanes starve, 1..32 (4)      */
+    int32_t visit;          /* dies_fly: crossing blocks between two event phases, 1..64 (8)                         */
+    int32_t min_ready;      /* dies_fly: partial event batches only while fewer packages are ready, 1..256 (32)      */
     int32_t chunk;          /* package ids a warp takes from the global counter at a time, 32..4096 (128)            */
     int32_t pkg_per_block;  /* grid sizing of small runs: packages per block, 32..2^20 (256)                         */
     int32_t w_pool;         /* dies_track (weighted runs): pool slots per warp, 32..248 (96)                         */

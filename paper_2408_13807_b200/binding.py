@@ -41,7 +41,7 @@ class dies_run_opts(C.Structure):
 
 
 class dies_tuning(C.Structure):
-    _fields_ = [(n, C.c_int32) for n in ("slots_uniform", "slots", "visit", "thr_idle", "chunk", "pkg_per_block",
+    _fields_ = [(n, C.c_int32) for n in ("slots_uniform", "slots", "visit", "min_ready", "chunk", "pkg_per_block",
                                          "w_pool", "w_thr_hi", "w_thr_lo", "w_min_ready", "atom_stride")]
 
 

@@ -1,17 +1,19 @@
 // dies_fly.cuh -- the tracker of runs whose package weights are fixed at launch (plain, k_bg, FFI; every configuration
-// of BASELINE.json): lane-owned pool slots.
+// of BASELINE.json).
 //
-// Every warp keeps a pool of 32 M photon packages in shared memory; slot (m, l) belongs to lane l.  The warp
-// alternates between
-//   (1) a CROSSING phase (Eq. 4): each lane flies one package of ITS OWN slots in registers.  A block
-//       of kSteps predicated crossing steps (no random numbers, no global memory, no branches) is followed by a short
-//       lane-private block end: a tangent passage turns the flight around in place; a flight that ended (event or
-//       escape) is stored into its slot and marked in the lane's status word, and the lane loads its next ready slot.
-//       No ballots, ranks or queues: a stopped lane never waits for other lanes to stop.
-//   (2) an EVENT phase: the pending events of the whole pool are gathered BY TYPE into batches of 32 (any lane handles
-//       any slot), and one of three specialised routines runs on the full warp: absorption + re-emission (L87),
-//       scattering (L85), or escape tally + launch of the next package id (L51-65, L87, L132-149).  The package goes
-//       back into the slot it came from, ready to fly for its owner.
+// Every warp keeps a pool of P photon packages in shared memory (32 bytes each) and four stacks of pool slots: packages
+// ready to fly, and packages waiting for an absorption, a scattering, or a source event (escape tally + launch of the
+// next package id).  The warp alternates between
+//   (1) a CROSSING phase (Eq. 4): each lane flies one package in registers.  A block of kSteps
+//       predicated crossing steps (no random numbers, no global memory, no branches) is followed by a short block end
+//       without votes or ranks: a tangent passage turns the flight around in place; a flight that ended (event or
+//       escape) is stored into its slot, which is pushed on the stack of its event type (one shared-memory atomic gives
+//       the position), and a lane without a flight pops the ready stack (one more atomic).  A stopped lane never waits
+//       for other lanes to stop, and any lane flies any package.
+//   (2) an EVENT phase: batches of 32 slots popped from ONE stack run one of three specialised routines on the full
+//       warp: absorption + re-emission (L87), scattering (L85), or escape tally + launch of the next package id
+//       (L51-65, L87, L132-149); the packages go back into their slots and onto the ready stack.  Partial batches run
+//       only while too few packages are ready to fly.
 // Differences from the paper's OpenCL design are listed in DESIGN.md ("What differs from the paper").
 #pragma once
 #include "dies_tracker.cuh"
@@ -21,19 +23,18 @@ namespace dies {
 constexpr int kFlyBlock = 1024;      // threads per block: ONE block per SM, so that its 32 warps share one set of tables
 constexpr int kFlyWarps = kFlyBlock / 32;
 constexpr int kSteps = 8;            // crossing steps per block
-constexpr int kMaxSlots = 8;         // pool slots per lane (the fields of the status word are bytes)
+constexpr int kMaxSlots = 8;         // pool slots per lane: P = 32 slots <= 256 (stack entries are bytes)
 // The unfolded shell table is read once per crossing step by every lane, at an address that is random from lane to
 // lane: with one copy of the table an 8-byte read of a warp takes about six passes of the shared-memory data pipe
 // (measured: that pipe, not instruction issue, bounded the first kernels).  The table is therefore kept in 2^LOGC
 // interleaved copies, copy (lane mod 2^LOGC) for each lane: with 16 copies the 16 lanes of a half-warp read 16
 // different bank pairs whatever entries they are at -- two passes, the minimum for 256 bytes.
 
-// status word of a lane: bit m of byte 0: slot m is ready to fly; of byte 1 / 2 / 3: it waits for an absorption /
-// a scattering / a source event (escape tally + next package id).  The slot the lane flies has no bit set.
-constexpr unsigned FS_ABS = 8u, FS_SCA = 16u, FS_SRC = 24u;
+// the stacks of a warp: stack t holds P bytes at queues + t P, its length is word t of the warp's counter quad
+enum { FQ_READY = 0, FQ_ABS, FQ_SCA, FQ_SRC, FQ_N };
 
 // shared-memory plan of a block (byte offsets), computed by the host and passed as a kernel parameter
-struct FlyPlan { unsigned bin, cs, tab, eps, omega, row, esc, A, poolA, poolB, poolQ, list, trace, total; };
+struct FlyPlan { unsigned bin, cs, tab, eps, omega, row, esc, A, poolA, poolB, poolQ, queues, cnt, trace, total; };
 __host__ __device__ inline FlyPlan plan_fly(int K, int nT, int ldS, int ldT, int M, bool trace, bool with_q, int logc)
 {
     constexpr unsigned kWarps = kFlyWarps;
@@ -54,11 +55,21 @@ __host__ __device__ inline FlyPlan plan_fly(int K, int nT, int ldS, int ldT, int
     p.poolA = o; o += 16u * kWarps * P;              // float4 {a, b2 (sign bit: next event is an absorption), col, c}
     p.poolB = o; o += 16u * kWarps * P;              // uint4  {id lo, id hi, blk, flags}
     p.poolQ = o; if (with_q) o += 8u * kWarps * P;   // raw quantum of the package (not stored when all are equal)
-    p.list = o;  o += 32u * kWarps;                  // the slots of the current batch
+    p.queues = o; o += (unsigned)FQ_N * kWarps * P;  // byte stacks of pool slots
     o = (o + 15u) & ~15u;
+    p.cnt = o;   o += 16u * kWarps;                  // int4 per warp: lengths of the four stacks
+
     p.trace = o; if (trace) o += 12u * kWarps * P;   // pkg, n_ev, crossings so far
     p.total = (o + 15u) & ~15u;
     return p;
+}
+
+// returning 32-bit add on a shared-memory word (the stack lengths of a warp)
+__device__ __forceinline__ unsigned atoms_add(unsigned a, unsigned v)
+{
+    unsigned old;
+    asm volatile("atom.shared.add.u32 %0, [%1], %2;" : "=r"(old) : "r"(a), "r"(v) : "memory");
+    return old;
 }
 
 // new free paths at an event or a launch (Eq. 1): column (units of 1/kappa_ref) to the next event and its type.
@@ -74,7 +85,6 @@ __device__ __forceinline__ void draw_column(const float4 bt, float tauS, float t
 // MODE 1: fixed temperature (row from fixed_row; tallies privatised in shared memory)
 // TRACE : replay tp.count packages of one model, tallies read-only, events recorded
 // LOGC : log2 of the number of interleaved copies of the shell table (4, or 0 when 16 copies do not fit)
-constexpr int kDeadSlot = (int)0x80000000;           // entry index of a slot that holds no package
 template <int MODE, bool TRACE, int LOGC>
 __global__ void __launch_bounds__(kFlyBlock, 1) dies_fly(DeviceModel D, RunParams R, TraceParams tp, FlyPlan sp)
 {
@@ -100,8 +110,8 @@ __global__ void __launch_bounds__(kFlyBlock, 1) dies_fly(DeviceModel D, RunParam
     const unsigned aA = sbase + sp.poolA + 16u * (unsigned)(wid * P);          // float4 {a, +-b2, col, entry index c} per slot
     const unsigned aB = sbase + sp.poolB + 16u * (unsigned)(wid * P);          // uint4 {id lo, id hi, blk, flags}
     const unsigned aQ = sbase + sp.poolQ + 8u * (unsigned)(wid * P);           // raw quantum
-    const unsigned aAl = aA + 16u * (unsigned)lane;                            // slot (0, lane); slot (m, lane) is 512 m further
-    const unsigned lst = sbase + sp.list + 32u * (unsigned)wid;                // slots of the current batch
+    const unsigned qb = sbase + sp.queues + (unsigned)(wid * FQ_N * P);        // stack t at qb + t P
+    const unsigned cq = sbase + sp.cnt + 16u * (unsigned)wid;                  // lengths {ready, abs, sca, src}
     int* const pT = reinterpret_cast<int*>(smem_raw + sp.trace) + wid * 3 * P;      // TRACE only
 
     for (int x = tid; x < K; x += kBlock) { s_bin[x] = D.bintab[x]; s_omega[x] = D.omega[x]; }
@@ -134,7 +144,8 @@ __global__ void __launch_bounds__(kFlyBlock, 1) dies_fly(DeviceModel D, RunParam
         }
         for (int x = tid; x < 2 * K; x += kBlock) s_esc[x] = 0u;
         // every slot of the pool is free and waits for a package id
-        for (int x = lane; x < P; x += 32) sts_u4(aB + 16u * x, 0u, 0u, 0u, 0u);
+        for (int x = lane; x < P; x += 32) { sts_u4(aB + 16u * x, 0u, 0u, 0u, 0u); sts_u8(qb + (unsigned)(FQ_SRC * P + x), (unsigned)x); }
+        if (lane == 0) sts_u4(cq, 0u, 0u, 0u, (unsigned)P);
         __syncthreads();
 
         unsigned long long* const gA = D.A + (size_t)m * ldS * kTallyStride;
@@ -150,9 +161,8 @@ __global__ void __launch_bounds__(kFlyBlock, 1) dies_fly(DeviceModel D, RunParam
         const unsigned long long q_uni =
             (unsigned long long)__float2ll_rn((mp.has_ext ? mp.qs_ext : mp.qs_point) * R.qscale);
 
-        unsigned st = ((1u << M) - 1u) << FS_SRC;    // status of the lane's own slots: all wait for a package id
         bool has = false;                            // the lane flies a package (state parked in its slot during events)
-        unsigned cb = 0, sa = aAl;                   // bit and pool address of the slot the lane flies
+        unsigned fslot = 0;                          // the slot of that package
         unsigned long long ch_next = 0, ch_end = 0;  // warp-uniform id chunk
         bool exhausted = false;
         // flight state: a = +-s along-ray coordinate, positive along the direction of the entry ahead; b2s = impact
@@ -166,48 +176,32 @@ __global__ void __launch_bounds__(kFlyBlock, 1) dies_fly(DeviceModel D, RunParam
             // EVENT phase: typed batches of up to 32 pending events of the whole pool
             // =====================================================================================
             if (has) {
-                sts_f4(sa, a, b2s, col, __int_as_float((int)(pa - tab0) >> ESH));
-                if (TRACE) { pT[2 * P + (int)((sa - aA) >> 4)] += (int)((pa - pa0) >> ESH); pa0 = pa; }
+                sts_f4(aA + 16u * fslot, a, b2s, col, __int_as_float((int)(pa - tab0) >> ESH));
+                if (TRACE) { pT[2 * P + (int)fslot] += (int)((pa - pa0) >> ESH); pa0 = pa; }
             }
             __syncwarp();
+            int nR;
             for (;;) {
-                const unsigned c3 = __popc(st & 0xff00u) | (__popc(st & 0xff0000u) << 10) | (__popc(st >> 24) << 20);
-                const unsigned tot = __reduce_add_sync(kFull, c3);
-                const int nA = (int)(tot & 1023u), nS = (int)((tot >> 10) & 1023u), nL = (int)(tot >> 20);
-                unsigned fs;
-                if (nA >= 32) fs = FS_ABS;
-                else if (nL >= 32) fs = FS_SRC;
-                else if (nS >= 32) fs = FS_SCA;
+                // lengths of the stacks (lanes that found the ready stack empty have driven its length below zero)
+                const uint4 c4 = lds_u4(cq);
+                nR = max((int)c4.x, 0);
+                const int nA = (int)c4.y, nS = (int)c4.z, nL = (int)c4.w;
+                int ft, nq;
+                if (nA >= 32) { ft = FQ_ABS; nq = nA; }
+                else if (nL >= 32) { ft = FQ_SRC; nq = nL; }
+                else if (nS >= 32) { ft = FQ_SCA; nq = nS; }
                 else {
-                    if (nA + nS + nL == 0) break;
-                    // partial batches only while lanes starve: nothing to fly and nothing ready
-                    const unsigned idle = __ballot_sync(kFull, !has && (st & 0xffu) == 0u);
-                    if (__popc(idle) < R.thr_idle) break;
-                    fs = (nA >= nS && nA >= nL) ? FS_ABS : (nL >= nS ? FS_SRC : FS_SCA);
+                    // partial batches only while too few packages are ready to fly
+                    if (nA + nS + nL == 0 || nR >= R.min_ready) break;
+                    if (nA >= nS && nA >= nL) { ft = FQ_ABS; nq = nA; }
+                    else if (nL >= nS) { ft = FQ_SRC; nq = nL; }
+                    else { ft = FQ_SCA; nq = nS; }
                 }
-                // ---- the batch: the first 32 slots (in slot-major order) whose event is of this type; their owners
-                //      mark them ready (a slot that ends without a package is found dead when it is taken)
-                int cnt = 0;
-                {
-                    const unsigned f = (st >> fs) & 0xffu;
-#pragma unroll
-                    for (int mm = 0; mm < kMaxSlots; mm++) {
-                        if (mm < M && cnt < 32) {
-                            const bool p = (f >> mm) & 1u;
-                            const unsigned bm = __ballot_sync(kFull, p);
-                            const int r = cnt + __popc(bm & lt_mask);
-                            if (p && r < 32) {
-                                sts_u8(lst + (unsigned)r, (unsigned)(mm * 32 + lane));
-                                st ^= (1u << (fs + mm)) | (1u << mm);
-                            }
-                            cnt += __popc(bm);
-                        }
-                    }
-                    cnt = min(cnt, 32);
-                }
-                __syncwarp();
+                // ---- the batch: the last 32 slots of the stack
+                const int cnt = min(nq, 32);
                 const bool act = lane < cnt;
-                const unsigned slot = act ? lds_u8(lst + (unsigned)lane) : 0u;
+                const unsigned slot = act ? lds_u8(qb + (unsigned)(ft * P + nq - 1 - lane)) : 0u;
+                const bool issrc = ft == FQ_SRC;
 
                 // ---- the package of the slot
                 float es = 0.f, eb2 = 0.f, ecol = 0.f;
@@ -227,9 +221,9 @@ __global__ void __launch_bounds__(kFlyBlock, 1) dies_fly(DeviceModel D, RunParam
                 int k = (int)(kf & KF_K);
                 bool fly = false, ev_absorb = false;
 
-                if (fs != FS_SRC) {
+                if (!issrc) {
                     // ================= absorption + re-emission (L87) or scattering (L85) =================
-                    const bool isabs = fs == FS_ABS;
+                    const bool isabs = ft == FQ_ABS;
                     // the flight stopped after committing the passage before entry ec with col < 0: the event lies in
                     // the shell traversed on the way to that surface, col / rho^ before it
                     const int ci = ec - 1;
@@ -239,6 +233,7 @@ __global__ void __launch_bounds__(kFlyBlock, 1) dies_fly(DeviceModel D, RunParam
                     unsigned long long old = 0;
                     unsigned peers = 0;
                     int leader = 0;
+                    const unsigned actm = __ballot_sync(kFull, act);
                     if (isabs) {
                         // (1) add the package's quantum to the shell tally, keep the old value (L87).  The returning
                         //     atomic is issued here and its result is only needed after the Philox block.
@@ -269,7 +264,7 @@ __global__ void __launch_bounds__(kFlyBlock, 1) dies_fly(DeviceModel D, RunParam
                             } else {
                                 const int hint = s_row[j];
                                 if (!TRACE && R.uniform_q)
-                                    old = __shfl_sync(__activemask(), old, leader) + q * (unsigned long long)__popc(peers & lt_mask);
+                                    old = __shfl_sync(actm, old, leader) + q * (unsigned long long)__popc(peers & lt_mask);
                                 // emitted power per mass before and after this absorption; rows of the table (R4)
                                 const double cs = s_cs[j];
                                 const float eps_old = (float)((double)old * cs);
@@ -469,22 +464,27 @@ __global__ void __launch_bounds__(kFlyBlock, 1) dies_fly(DeviceModel D, RunParam
                         }
                     }
                 }
-                // ---- the package goes back into its slot; a slot that got no package id is dead
-                if (act) {
-                    if (fly) {
-                        const float b2w = __uint_as_float(__float_as_uint(eb2) | (ev_absorb ? 0x80000000u : 0u));
-                        sts_f4(aA + 16u * slot, fabsf(es), b2w, ecol, __int_as_float(ec));
-                        sts_u4(aB + 16u * slot, (unsigned)id, (unsigned)(id >> 32), blk, (unsigned)k | KF_OCC);
-                        if (!R.uniform_q) sts_u64(aQ + 8u * slot, q);
-                        if (TRACE) { pT[slot] = pkg; pT[P + slot] = n_ev; pT[2 * P + slot] = (int)ncross; }
-                    } else {
-                        sts_f4(aA + 16u * slot, 0.f, 0.f, 0.f, __int_as_float(kDeadSlot));
-                        sts_u4(aB + 16u * slot, 0u, 0u, 0u, 0u);
-                    }
+                // ---- the package goes back into its slot and onto the ready stack; a slot that got no package id
+                //      (the ids of the ticket are exhausted) leaves the pool
+                const unsigned flym = __ballot_sync(kFull, fly);
+                if (fly) {
+                    const float b2w = __uint_as_float(__float_as_uint(eb2) | (ev_absorb ? 0x80000000u : 0u));
+                    sts_f4(aA + 16u * slot, fabsf(es), b2w, ecol, __int_as_float(ec));
+                    sts_u4(aB + 16u * slot, (unsigned)id, (unsigned)(id >> 32), blk, (unsigned)k | KF_OCC);
+                    if (!R.uniform_q) sts_u64(aQ + 8u * slot, q);
+                    if (TRACE) { pT[slot] = pkg; pT[P + slot] = n_ev; pT[2 * P + slot] = (int)ncross; }
+                    sts_u8(qb + (unsigned)(nR + __popc(flym & lt_mask)), slot);
+                }
+                if (lane == 0) {
+                    sts_u32(cq, (unsigned)(nR + __popc(flym)));
+                    sts_u32(cq + 4u * (unsigned)ft, (unsigned)(nq - cnt));
                 }
                 __syncwarp();
             }
-            if (!__any_sync(kFull, has || st != 0u)) break;          // every slot of the pool is dead: the ticket is drained
+            // every slot of the pool has left it: the ticket is drained
+            if (nR == 0 && !__any_sync(kFull, has)) break;
+            if (lane == 0) sts_u32(cq, (unsigned)nR);                // (a length below zero starts again at zero)
+            __syncwarp();
 
             // =====================================================================================
             // CROSSING phase (Eq. 4): no RNG, no global memory, no branches in the crossing itself.
@@ -494,23 +494,19 @@ __global__ void __launch_bounds__(kFlyBlock, 1) dies_fly(DeviceModel D, RunParam
             // before the surface (R7: an event exactly on a surface is a passage).
             // =====================================================================================
             if (has) {
-                const float4 a4 = lds_f4(sa);
+                const float4 a4 = lds_f4(aA + 16u * fslot);
                 a = a4.x; b2s = a4.y; col = a4.z; pa = tab0 + ES * (unsigned)__float_as_int(a4.w);
             }
             for (int it = 0; it < R.visit; it++) {
-                // ---- a lane without a flight takes its next ready slot
-                {
-                    const unsigned r = st & 0xffu;
-                    if (!has && r != 0u) {
-                        const unsigned nb = r & (0u - r);
-                        st ^= nb; cb = nb;
-                        sa = aAl + ((unsigned)(31 - __clz(nb)) << 9);
-                        const float4 a4 = lds_f4(sa);
-                        const int c = __float_as_int(a4.w);
-                        a = a4.x; b2s = a4.y; col = a4.z;
-                        has = c != kDeadSlot;                    // a slot that ended without a package
-                        pa = tab0 + (has ? ES * (unsigned)c : 0u);
+                // ---- a lane without a flight pops the ready stack (a length that has reached zero goes on falling)
+                if (!has) {
+                    const int idx = (int)atoms_add(cq, 0xffffffffu) - 1;
+                    if (idx >= 0) {
+                        fslot = lds_u8(qb + (unsigned)idx);
+                        const float4 a4 = lds_f4(aA + 16u * fslot);
+                        a = a4.x; b2s = a4.y; col = a4.z; pa = tab0 + ES * (unsigned)__float_as_int(a4.w);
                         pa0 = pa;
+                        has = true;
                     }
                 }
                 // ---- kSteps crossings.  The table is walked from pb with constant offsets; the entries are read two
@@ -549,12 +545,15 @@ __global__ void __launch_bounds__(kFlyBlock, 1) dies_fly(DeviceModel D, RunParam
                     a = -a;
                 }
                 if (has && !alive && !tang) {
-                    sts_f4(sa, a, b2s, col, __int_as_float((int)(pa - tab0) >> ESH));
-                    st |= cb << (colpos ? FS_SRC : ((__float_as_int(b2s) < 0) ? FS_ABS : FS_SCA));
-                    if (TRACE) pT[2 * P + (int)((sa - aA) >> 4)] += (int)((pa - pa0) >> ESH);
+                    sts_f4(aA + 16u * fslot, a, b2s, col, __int_as_float((int)(pa - tab0) >> ESH));
+                    const unsigned ft = colpos ? (unsigned)FQ_SRC : ((__float_as_int(b2s) < 0) ? (unsigned)FQ_ABS : (unsigned)FQ_SCA);
+                    const unsigned pos = atoms_add(cq + 4u * ft, 1u);
+                    sts_u8(qb + ft * (unsigned)P + pos, fslot);
+                    if (TRACE) pT[2 * P + (int)fslot] += (int)((pa - pa0) >> ESH);
                     has = false;
                 }
             }
+            __syncwarp();
             // counters: flush before a 32-bit count can wrap
             if (__any_sync(kFull, ((lc8 >> 2) | lc_ffi | wc_pkg | wc_sca | wc_abs | wc_esc) >> 29) != 0u) {
                 atomicAdd(&s_cnt[LC_CROSSINGS], (unsigned long long)(lc8 >> ESH));

@@ -411,7 +411,7 @@ static int check_device()
 }
 
 // ------------------------------------------------------------------ launch tuning (include/dies.h: dies_tuning)
-static const dies_tuning kTuningDefaults = {5, 4, 6, 8, (int32_t)kChunk, kFlyWarps * 32, 96, 20, 16, 32, kTallyStride};
+static const dies_tuning kTuningDefaults = {5, 4, 8, 32, (int32_t)kChunk, kFlyWarps * 32, 96, 20, 16, 32, kTallyStride};
 static dies_tuning g_tuning = kTuningDefaults;
 static std::mutex g_tuning_mutex;
 
@@ -428,7 +428,7 @@ extern "C" int dies_set_tuning(const dies_tuning* t)
     dies_tuning n = g_tuning;
     struct { int32_t dies_tuning::*f; int lo, hi; const char* name; } spec[] = {
         {&dies_tuning::slots_uniform, 1, kMaxSlots, "slots_uniform"}, {&dies_tuning::slots, 1, kMaxSlots, "slots"},
-        {&dies_tuning::visit, 1, 64, "visit"}, {&dies_tuning::thr_idle, 1, 32, "thr_idle"},
+        {&dies_tuning::visit, 1, 64, "visit"}, {&dies_tuning::min_ready, 1, 256, "min_ready"},
         {&dies_tuning::chunk, 32, 4096, "chunk"}, {&dies_tuning::pkg_per_block, 32, 1 << 20, "pkg_per_block"},
         {&dies_tuning::w_pool, 32, kMaxPool, "w_pool"}, {&dies_tuning::w_thr_hi, 1, 32, "w_thr_hi"},
         {&dies_tuning::w_thr_lo, 1, 32, "w_thr_lo"}, {&dies_tuning::w_min_ready, 1, kMaxPool, "w_min_ready"},
@@ -766,7 +766,8 @@ static int fill_run_params(dies_model* m, uint64_t n_packages, uint64_t seed, co
     R->pool = tn.w_pool;
     R->thr_hi = tn.w_thr_hi; R->thr_lo = tn.w_thr_lo; R->min_ready = tn.w_min_ready;
     R->slots = fly_slots(R->uniform_q != 0);
-    R->visit = tn.visit; R->thr_idle = tn.thr_idle;
+    R->visit = tn.visit;
+    if (!weighted) R->min_ready = tn.min_ready;
     R->n_tickets = 0; R->parts = 1;
     return DIES_OK;
 }

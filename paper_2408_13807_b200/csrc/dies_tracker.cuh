@@ -133,7 +133,6 @@ struct RunParams {
     int min_ready;                   // event phase: mixed batches only while fewer packages are ready
     int slots;                       // dies_fly: pool slots per lane (1 <= slots <= kMaxSlots)
     int visit;                       // dies_fly: crossing blocks between two event phases
-    int thr_idle;                    // dies_fly: partial event batches while at least this many lanes starve
 };
 
 struct TraceParams {
