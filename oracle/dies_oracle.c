@@ -395,6 +395,20 @@ void dies_oracle_kA_profile(const oracle_model* o, double k_dense, double k_dilu
 /* Launch direction of a background package (Eq. 2: mu = sqrt(u) w.r.t. the inward
  * normal; L99-103, Eq. 5: mu = u^k_bg with weight W = 2 k_bg mu^(2-1/k_bg); k_bg = 0.5 is Eq. 2).
  * Exposed for the E[W] = 1 and direction-distribution pins. */
+/* L85: direction cosine w.r.t. the radius after a deflection by Theta (cosine ct) with azimuth phi about the old
+ * direction, whose cosine w.r.t. the radius was mu: mu' = mu cos Theta + sqrt(1 - mu^2) sin Theta cos phi.
+ * (The scattering step of the package loop calls this function; it is exported so that a test can pin it to
+ * E[mu' | mu] = g mu and the second moment of the Henyey-Greenstein function.) */
+double dies_oracle_scatter_direction(double mu, double ct, double phi)
+{
+    double st = sqrt(fmax(1.0 - ct * ct, 0.0));
+    double sm = sqrt(fmax(1.0 - mu * mu, 0.0));
+    double m = mu * ct + sm * st * cos(phi);
+    if (m > 1.0) m = 1.0;
+    if (m < -1.0) m = -1.0;
+    return m;
+}
+
 void dies_oracle_launch_direction(double u, double k_bg, double* mu_in, double* W)
 {
     if (k_bg == 0.5) { *mu_in = sqrt(u); *W = 1.0; }
@@ -553,13 +567,7 @@ static void follow_package(const oracle_model* o, const run_opts* opt, tallies* 
                 ta->sums[D_REWEIGHT] += (W - W_old) * e;
                 mu = mu1;
             } else {
-            double ct = dies_oracle_hg_cos(o->g[k], u[0]);
-            double phi = 2.0 * PI * u[1];
-            double st = sqrt(fmax(1.0 - ct * ct, 0.0));
-            double sm = sqrt(fmax(1.0 - mu * mu, 0.0));
-            mu = mu * ct + sm * st * cos(phi);
-            if (mu > 1.0) mu = 1.0;
-            if (mu < -1.0) mu = -1.0;
+            mu = dies_oracle_scatter_direction(mu, dies_oracle_hg_cos(o->g[k], u[0]), 2.0 * PI * u[1]);
             }
             tauS = -log(u[2]);
             tauA = -log(u[3]);

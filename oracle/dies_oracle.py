@@ -44,6 +44,8 @@ _lib.dies_oracle_chord_walk.argtypes = [C.c_int, _dp, C.c_int, C.c_double, C.c_d
 _lib.dies_oracle_hg_cos.restype = C.c_double
 _lib.dies_oracle_hg_cos.argtypes = [C.c_double, C.c_double]
 _lib.dies_oracle_launch_direction.argtypes = [C.c_double, C.c_double, _dp, _dp]
+_lib.dies_oracle_scatter_direction.restype = C.c_double
+_lib.dies_oracle_scatter_direction.argtypes = [C.c_double, C.c_double, C.c_double]
 _lib.dies_oracle_uniform.restype = C.c_double
 _lib.dies_oracle_uniform.argtypes = [C.c_uint32]
 _lib.dies_oracle_philox4x32_10.argtypes = [C.POINTER(C.c_uint32), C.POINTER(C.c_uint32), C.POINTER(C.c_uint32)]
@@ -71,6 +73,11 @@ def uniform(word: int) -> float:
 
 def hg_cos(g: float, u: float) -> float:
     return float(_lib.dies_oracle_hg_cos(g, u))
+
+
+def scatter_direction(mu: float, cos_theta: float, phi: float) -> float:
+    """The direction cosine after a scattering, as the package loop computes it."""
+    return float(_lib.dies_oracle_scatter_direction(mu, cos_theta, phi))
 
 
 def launch_direction(u: float, k_bg: float):

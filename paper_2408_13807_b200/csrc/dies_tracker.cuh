@@ -453,9 +453,14 @@ __global__ void __launch_bounds__(kBlock, kMinBlocks) dies_track(DeviceModel D, 
                 //     flight the true survival probability over the biased one is e^{kappa_A (CA - C)} for the
                 //     absorption clock and e^{kappa_S (k_S - 1) C} for the scattering clock (C: column traversed,
                 //     CA: the same weighted with k_A of every shell); the event that ended the flight adds 1/k.
-                float colS = 0.f, cA0 = 0.f, cS0 = 0.f, q0f = 0.f, off = 0.f;
+                // The package carries its launch quantum q0 and its weight relative to the launch weight, wrel (fp32);
+                // the quantum it adds to a tally is q = round(q0 wrel) (R18).  A quantum that has rounded to nothing
+                // does not end the package: it flies on, adding nothing, until the rule of L119 ends it.
+                float colS = 0.f, cA0 = 0.f, cS0 = 0.f, wrel = 1.f, off = 0.f;
+                unsigned long long q0 = q;
                 if (WT) {
-                    if (type >= 0) { const float4 w4 = lds_f4(aW + 16u * slot); colS = w4.x; cA0 = w4.y; cS0 = w4.z; q0f = w4.w; }
+                    if (type >= 0) { const float4 w4 = lds_f4(aW + 16u * slot); colS = w4.x; cA0 = w4.y; cS0 = w4.z; wrel = w4.w; }
+                    q = (unsigned long long)__double2ll_rn((double)q0 * (double)wrel);
                     long long dq = 0;
                     if (isev || esc) {
                         const float4 bt = s_bin[k];
@@ -471,8 +476,8 @@ __global__ void __launch_bounds__(kBlock, kMinBlocks) dies_track(DeviceModel D, 
                         }
                         const float kapA = bt.x < 3.0e38f ? 1.f / bt.x : 0.f, kapS = bt.y < 3.0e38f ? 1.f / bt.y : 0.f;
                         const float lnW = fmaf(kapA, CA - C, kapS * (R.k_S - 1.f) * C);
-                        const unsigned long long qn =
-                            (unsigned long long)__double2ll_rn((double)q * (double)(expf(lnW) / kdiv));
+                        wrel *= expf(lnW) / kdiv;
+                        const unsigned long long qn = (unsigned long long)__double2ll_rn((double)q0 * (double)wrel);
                         dq = (long long)qn - (long long)q;
                         q = qn;
                     }
@@ -638,7 +643,7 @@ __global__ void __launch_bounds__(kBlock, kMinBlocks) dies_track(DeviceModel D, 
                         if (launch) {
                             ncross = 0; n_ev = 0;
                             q = (unsigned long long)__float2ll_rn(w * (point ? mp.qs_point : mp.qs_ext) * R.qscale);
-                            q0f = (float)q;
+                            q0 = q; wrel = 1.f;
                             q_inj = q;                           // (FFI splits the quantum below)
                             record<TRACE>(tp, pkg, n_ev, 0 /*LAUNCH*/, j - mp.cav, k, 0);
                         }
@@ -765,15 +770,15 @@ __global__ void __launch_bounds__(kBlock, kMinBlocks) dies_track(DeviceModel D, 
                         // the quantum the package carries away from a reweighted direction
                         long long dq = 0;
                         if (wdir != 1.f) {
-                            const unsigned long long qn = (unsigned long long)__double2ll_rn((double)q * (double)wdir);
+                            wrel *= wdir;
+                            const unsigned long long qn = (unsigned long long)__double2ll_rn((double)q0 * (double)wrel);
                             dq = (long long)qn - (long long)q;
                             q = qn;
                         }
                         if (dq != 0) atomicAdd(&s_cnt[LC_REWEIGHT_RAW], (unsigned long long)dq);
                     }
-                    // L119: a package whose weight fell by ten orders of magnitude is terminated (its quantum may also
-                    // have rounded to nothing at the resolution 2^-S of the tallies, R18)
-                    if (WT && isev && (q == 0ull || (float)q < 1e-10f * q0f)) {
+                    // L119: a package whose weight fell by ten orders of magnitude is terminated
+                    if (WT && isev && wrel < 1e-10f) {
                         record<TRACE>(tp, pkg, n_ev, 4 /*TERMINATE*/, j - mp.cav, k, ncross);
                         if (TRACE) tp.n_events[pkg] = n_ev;
                         atomicAdd(&s_cnt[LC_TERMINATED], 1ull);
@@ -792,8 +797,8 @@ __global__ void __launch_bounds__(kBlock, kMinBlocks) dies_track(DeviceModel D, 
                         : ((unsigned)k | (ev_absorb ? KF_EVABS : 0u) | KF_OCC);
                     sts_f4(aA + 16u * slot, s, b2, col, __uint_as_float(pa));
                     sts_u4(aB + 16u * slot, (unsigned)id, (unsigned)(id >> 32), blk, nkf);
-                    if (!R.uniform_q) sts_u64(aQ + 8u * slot, q);
-                    if (WT) sts_f4(aW + 16u * slot, colS, cA0, cS0, q0f);
+                    if (!R.uniform_q) sts_u64(aQ + 8u * slot, WT ? q0 : q);
+                    if (WT) sts_f4(aW + 16u * slot, colS, cA0, cS0, wrel);
                     if (TRACE) { pT[slot] = pkg; pT[P + slot] = n_ev; pT[2 * P + slot] = (int)ncross; }
                 }
                 if (!R.uniform_q) {
@@ -1047,6 +1052,7 @@ __global__ void __launch_bounds__(kBlock, kMinBlocks) dies_track(DeviceModel D, 
                     atomicAdd(&s_cnt[LC_SCATTERINGS], (unsigned long long)wc_sca);
                     atomicAdd(&s_cnt[LC_ABSORPTIONS], (unsigned long long)wc_abs);
                     atomicAdd(&s_cnt[LC_ESCAPED], (unsigned long long)wc_esc);
+                    if (R.uniform_q) atomicAdd(&s_cnt[LC_INJECTED_RAW], q_uni * (unsigned long long)wc_pkg);
                 }
                 lc_cross = lc_ffi = wc_pkg = wc_sca = wc_abs = wc_esc = 0u;
             }

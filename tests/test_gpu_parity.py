@@ -163,6 +163,52 @@ def test_fixed_T_is_deterministic_and_splittable():
             assert r[2][k] == res[0][2][k]
 
 
+@pytest.mark.parametrize("kw", [{}, dict(k_bg=0.2), dict(ffi=1)])
+def test_fixed_T_tallies_do_not_depend_on_tuning_or_stream(kw):
+    """dies_set_tuning (pool depth, blocks per visit, batch threshold, id chunks) changes the order in which packages
+    are followed, never what is computed: in fixed-temperature mode the integer tallies, the escape spectrum and the
+    counters are bit-identical; the runs go through a non-default (non-blocking) CUDA stream, the first of them right
+    after dies_set_sources."""
+    import torch
+    p = synth.config2(n_shells=50, n_freq=64, tau_V=5.0)
+    n = 300_000
+    res = []
+    try:
+        for tune in ({}, dict(visit=1, slots_uniform=1, slots=1), dict(visit=16, min_ready=1, chunk=32),
+                     dict(slots_uniform=3, slots=2, min_ready=200, pkg_per_block=4096)):
+            dies.dies_set_tuning()
+            if tune:
+                dies.dies_set_tuning(**tune)
+            st = torch.cuda.Stream()
+            m = dies.Model(p)
+            m.dies_set_fixed_temperature(_fixed_T(p.n_shells))
+            m.dies_set_sources(p.ext_bin_intensity)
+            m.dies_run(n, seed=4, mode=dies.DIES_MODE_FIXED_T, stream=st.cuda_stream, **kw)
+            raw, _, _ = m.dies_get_absorbed()
+            res.append((raw.copy(), m.dies_get_escape_spectrum().copy(), m.dies_get_counters()))
+            m.close()
+    finally:
+        dies.dies_set_tuning()
+    for r in res[1:]:
+        assert np.array_equal(r[0], res[0][0])
+        assert np.array_equal(r[1], res[0][1])
+        for k in ("packages", "crossings", "ffi_crossings", "scatterings", "absorptions", "escaped", "injected_raw",
+                  "escaped_raw"):
+            assert r[2][k] == res[0][2][k], k
+    assert res[0][2]["packages"] == n
+
+
+def test_tuning_argument_errors():
+    with pytest.raises(dies.DiesError) as e:
+        dies.dies_set_tuning(visit=1000)
+    assert e.value.code == dies.DIES_EINVAL
+    t0 = dies.dies_get_tuning()
+    dies.dies_set_tuning(visit=5)
+    assert dies.dies_get_tuning()["visit"] == 5 and dies.dies_get_tuning()["chunk"] == t0["chunk"]
+    dies.dies_set_tuning()
+    assert dies.dies_get_tuning() == t0
+
+
 # ------------------------------------------------------------------ full IRE, statistical
 def _ire_stats(orc, p, n, seeds, model_kw=None, **kw):
     To, Tg = [], []

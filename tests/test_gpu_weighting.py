@@ -103,6 +103,9 @@ def test_weighted_thin_sphere_matches_the_plain_method(orc):
 
 
 def test_weight_guard_and_bookkeeping(orc):
+    """The live weight guard: a package is terminated when its weight has fallen below 1e-10 of its
+    launch weight, on the GPU exactly as in the oracle (the kernel carries the relative weight in fp32 beside the
+    fixed-point quantum, R18).  Thick scattering toy sphere with k_S = 10: most packages end by the guard."""
     p = toy_problem(n_shells=4, tau=20.0, kappa_sca=9.0, g=0.0)
     n = 20000
     m = dies.Model(p)
@@ -110,10 +113,41 @@ def test_weight_guard_and_bookkeeping(orc):
     c = m.dies_get_counters()
     o = orc.Oracle(p).run(n, seed=2, k_S=10.0)
     assert c["packages"] == n == c["escaped"] + c["terminated"]
-    # the GPU terminates at the tally resolution 2^-24 (R18), the oracle at 1e-10: both terminate most packages
-    assert c["terminated"] > 0.5 * o.counters["terminated"] > 0
+    assert o.counters["terminated"] > 0.2 * n
+    # identical streams: the same packages are terminated, up to the fp32/fp64 flips of R14
+    assert abs(c["terminated"] - o.counters["terminated"]) <= max(3, 1e-3 * o.counters["terminated"]), \
+        (c["terminated"], o.counters["terminated"])
+    for k in ("scatterings", "absorptions", "crossings"):
+        assert abs(c[k] - o.counters[k]) <= 2e-3 * o.counters[k] + 3, (k, c[k], o.counters[k])
     assert _identity(c)
     assert c["terminated_raw"] < 1e-6 * c["injected_raw"]
+    m.close()
+
+
+def test_weight_guard_trace_bit_exact(orc):
+    """Event lists that END WITH DIES_EV_TERMINATE, bit-exact against the oracle on identical Philox streams."""
+    p = toy_problem(n_shells=4, tau=20.0, kappa_sca=9.0, g=0.0)
+    n_total, count, max_ev = 20000, 1500, 4096
+    Tfix = np.full(p.n_shells, 15.0)
+    o = orc.Oracle(p)
+    o.set_fixed_temperature(Tfix)
+    m = dies.Model(p)
+    m.dies_set_fixed_temperature(Tfix)
+    ev, nev = m.dies_trace_packages(0, count, n_total, seed=2, max_events=max_ev, mode=dies.DIES_MODE_FIXED_T, k_S=10.0)
+    safe = same = n_term = n_term_same = 0
+    for pid in range(count):
+        ref, nref, margin = o.trace(n_total, pid, seed=2, mode=1, max_events=max_ev, k_S=10.0)
+        ok = (nref == nev[pid]) and nref <= max_ev and np.array_equal(ref, ev[pid, :nref])
+        same += ok
+        term = nref <= max_ev and ref[nref - 1][0] == 4          # DIES_EV_TERMINATE
+        n_term += term
+        n_term_same += term and ok
+        if margin > 1e-3 and nref <= max_ev:
+            safe += 1
+            assert ok, (pid, margin, ref[:6], ev[pid, :6], nref, nev[pid])
+    assert n_term > 0.2 * count, n_term                       # the guard is exercised
+    assert n_term_same >= 0.98 * n_term, (n_term_same, n_term)
+    assert same >= 0.98 * count, same / count
     m.close()
 
 

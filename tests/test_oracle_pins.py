@@ -214,10 +214,32 @@ def test_henyey_greenstein_sampler(g):
     assert np.max(np.abs(hist - expect)) <= 2.0
 
 
-def test_scattering_redistribution_is_isotropic_for_g0():
-    """After an isotropic (g = 0) scattering the new direction cosine w.r.t. the radius must be uniform
-    whatever the old one was (pins the mu' = mu cos T + sqrt(1-mu^2) sin T cos phi composition):
-    a purely scattering sphere re-emits what enters it, and the escaping flux is conserved."""
+@pytest.mark.parametrize("g", [0.0, 0.5, -0.3])
+def test_scattering_composition_moments(g):
+    """The composition mu' = mu cos T + sqrt(1 - mu^2) sin T cos phi, the very function the package loop
+    calls, against closed forms: with cos T from the Henyey-Greenstein function (L167) and phi uniform,
+    E[mu' | mu] = g mu and E[mu'^2 | mu] = mu^2 c2 + (1 - mu^2)(1 - c2) / 2 with c2 = E[cos^2 T] = (1 + 2 g^2) / 3.
+    A transposed operand, a dropped term or sin/cos swapped fails one of the two; stratified sampling makes the
+    comparison deterministic."""
+    n = 400
+    u0 = (np.arange(n) + 0.5) / n
+    phis = 2 * np.pi * (np.arange(n) + 0.5) / n
+    ct = np.array([orc.hg_cos(g, u) for u in u0])
+    assert abs(ct.mean() - g) < 2e-4 and abs((ct ** 2).mean() - (1 + 2 * g * g) / 3) < 2e-4
+    c2 = (1 + 2 * g * g) / 3
+    for mu in (-1.0, -0.6, 0.0, 0.3, 0.9, 1.0):
+        m1 = m2 = 0.0
+        for c in ct:
+            v = np.array([orc.scatter_direction(mu, c, ph) for ph in phis[::8]])
+            m1 += v.mean(); m2 += (v ** 2).mean()
+        m1 /= n; m2 /= n
+        assert abs(m1 - g * mu) < 5e-4, (mu, m1)
+        assert abs(m2 - (mu * mu * c2 + (1 - mu * mu) * (1 - c2) / 2)) < 5e-4, (mu, m2)
+
+
+def test_pure_scattering_sphere_conserves_packages():
+    """A purely scattering sphere (kappa_abs << kappa_sca, g = 0) returns every package it receives: counts of events
+    and conservation of the escaping flux (the composition of directions is pinned by the test above)."""
     p = toy_problem(n_shells=3, tau=2.0, kappa_sca=1e6, g=0.0)     # kappa_abs << kappa_sca: pure scattering
     o = orc.Oracle(p)
     n = 50000
