@@ -195,13 +195,22 @@ def run_ours(args, rank, world, local_rank):
         dies.dies_set_tuning(**{k: int(v) for k, v in (kv.split("=") for kv in args.tune.split(","))})
     p = make_problem(args.workload, args.packages)
     batch = isinstance(p, synth.BatchProblem)
+    model0 = 0
+    if batch and world > 1:
+        # config 5 shards: the spheres are dealt to the ranks, no exchange
+        p, model0 = sharding.batch_shard(p, rank, world)
     n_models = p.n_models if batch else 1
     n_per_model = p.n_packages
     n = n_per_model * n_models                              # packages per step on this rank
     k_bg, ffi = getattr(p, "k_bg", 0.5), getattr(p, "ffi", 0)
     n_shells, n_freq, n_T = int(p.rho.shape[-1]), int(p.freq.size), int(p.T_grid.size)
     opts = dict(k_bg=k_bg, ffi=ffi)
-    make = (lambda: dies.Model(batch=p, device=str(dev))) if batch else (lambda: dies.Model(p, device=str(dev)))
+    def make():
+        if not batch:
+            return dies.Model(p, device=str(dev))
+        mm = dies.Model(batch=p, device=str(dev))
+        mm.dies_set_model_offset(model0)
+        return mm
     m = make()
     info = dies.dies_device_info()
     stream = torch.cuda.current_stream(dev)
@@ -213,7 +222,7 @@ def run_ours(args, rank, world, local_rank):
         torch.cuda.synchronize(dev)
 
     for w in range(args.warmup):
-        m.dies_run(n_per_model, seed=sharding.replica_seed(1000, w, rank), **opts)
+        m.dies_run(n_per_model, seed=sharding.replica_seed(1000, w, 0 if batch else rank), **opts)
     torch.cuda.synchronize(dev)
     c0 = m.dies_get_counters()
 
@@ -227,7 +236,7 @@ def run_ours(args, rank, world, local_rank):
     for s in range(args.steps):
         flush.fill_(s & 0xFF)
         ev[s][0].record(stream)
-        m.dies_run(n_per_model, seed=sharding.replica_seed(1, s, rank), **opts)
+        m.dies_run(n_per_model, seed=sharding.replica_seed(1, s, 0 if batch else rank), **opts)
         ev[s][1].record(stream)
     barrier()
     t_wall = time.perf_counter() - t_wall
@@ -239,8 +248,9 @@ def run_ours(args, rank, world, local_rank):
         tot_counts[k] = c1[k]
     step_ms = float(np.sum(ms)) / args.steps
     total_ms = sharding.max_over_ranks(float(np.sum(ms)), dev)
-    value = world * n * args.steps / (total_ms * 1e-3)
-    crossings_per_s = world * c1["crossings"] * args.steps / (total_ms * 1e-3)
+    n_all = sharding.sum_over_ranks(n, dev)                # packages per step of the whole job
+    value = n_all * args.steps / (total_ms * 1e-3)
+    crossings_per_s = sharding.sum_over_ranks(c1["crossings"], dev) * args.steps / (total_ms * 1e-3)
 
     # ---- end to end through the C ABI with host buffers: create + sources + run + both getters
     e2e_t = []
@@ -253,7 +263,7 @@ def run_ours(args, rank, world, local_rank):
         Lesc = m2.dies_get_escape_spectrum()
         e2e_t.append(time.perf_counter() - t0)
         m2.close()
-    e2e_val = world * n / float(np.median(e2e_t))
+    e2e_val = n_all / sharding.max_over_ranks(float(np.median(e2e_t)), dev)
     h2d = 8 * (p.emis.size + p.T_grid.size + 3 * n_freq + p.r_bounds.size + p.rho.size + 2 * n_freq * n_models)
     d2h = 8 * n_models * (n_shells + n_freq) + 64
 
@@ -277,8 +287,8 @@ def run_ours(args, rank, world, local_rank):
                 vs_baseline=None, dtype="f32", data="synthetic",
                 crossings_per_s=crossings_per_s,
                 config=dict(workload=args.workload, n_models=n_models, n_shells=n_shells, n_freq=n_freq, n_T=n_T,
-                            packages_per_step=n, mode="full IRE", k_bg=k_bg, ffi=ffi,
-                            parallelism="replicas only" if world > 1 else "1 GPU", l2="flushed between steps (256 MiB fill)",
+                            packages_per_step=int(n_all), mode="full IRE", k_bg=k_bg, ffi=ffi,
+                            parallelism=("model shards, no collective" if batch else "replicas only") if world > 1 else "1 GPU", l2="flushed between steps (256 MiB fill)",
                             per_package=dict(crossings=c1["crossings"] / n, scatterings=c1["scatterings"] / n,
                                              absorptions=c1["absorptions"] / n),
                             grid=dict(**info)),
@@ -316,32 +326,44 @@ def run_ours(args, rank, world, local_rank):
 
 
 def run_noise_study(args):
-    """Config 4 (BASELINE.json: "noise per shell vs packages reported"; section 3.2): standard deviation
-    of the shell temperatures over 8 seeds against the number of packages, forced first interaction on and off.
-    One JSON line; every run goes through the C ABI (dies_run + dies_get_temperature), nothing is timed here."""
+    """Accuracy against the number of packages (section 3.1, Fig. 2-3; section 3.2; BASELINE.json
+    configs[3] "noise per shell vs packages reported"): for configs 2 (k_bg = 0.5 and 0.2), 3 and 4 (FFI on / off) the shell
+    temperatures of 8 seeds at N = 1e5 ... 1e8 packages against a reference run with 1e9 packages.  Per radius decile:
+    the statistical error (standard deviation over the seeds / mean) and the systematic error (mean over the seeds
+    against the reference).  One JSON line; every run goes through the C ABI (dies_run + dies_get_temperature),
+    nothing is timed here."""
     import torch
     from paper_2408_13807_b200 import binding as dies
     dev = torch.device("cuda", 0)
     torch.cuda.set_device(dev)
     seeds = list(range(1, 9))
+    cases = [("config2", synth.config2(), {}), ("config2_kbg0.2", synth.config2(k_bg=0.2), dict(k_bg=0.2)),
+             ("config3", synth.config3(), {}), ("config4_ffi", synth.config4(ffi=1), dict(ffi=1)),
+             ("config4_noffi", synth.config4(ffi=0), {})]
     rows = []
-    for ffi in (0, 1):
-        p = synth.config4(ffi=ffi)
+    for name, p, kw in cases:
         m = dies.Model(p, device=str(dev))
+        m.dies_run(10**9, seed=1001, **kw)
+        Tref = m.dies_get_temperature()
+        edges = np.linspace(0, p.n_shells, 11).astype(int)
         for n in (10**5, 10**6, 10**7, 10**8):
             T = []
             for sd in seeds:
-                m.dies_run(n, seed=sd, k_bg=0.5, ffi=ffi)
+                m.dies_run(n, seed=sd, **kw)
                 T.append(m.dies_get_temperature())
             T = np.array(T)
-            rel = T.std(0, ddof=1) / T.mean(0)
-            h = p.n_shells // 2
-            rows.append(dict(ffi=ffi, packages=n, rel_sigma_T_mean=float(rel.mean()), rel_sigma_T_max=float(rel.max()),
-                             rel_sigma_T_inner_half=float(rel[:h].mean()), rel_sigma_T_outer_half=float(rel[h:].mean()),
-                             T_mean_K=float(T.mean())))
+            ok = T.min(0) > p.T_grid[0] * 1.001                   # shells every seed reached
+            rel = np.where(ok, T.std(0, ddof=1) / T.mean(0), np.nan)
+            sys_ = np.where(ok, T.mean(0) / Tref - 1.0, np.nan)
+            dec = lambda v: [None if not np.any(np.isfinite(v[a:b])) else float(np.nanmean(v[a:b]))
+                             for a, b in zip(edges[:-1], edges[1:])]
+            rows.append(dict(case=name, packages=n, shells_reached=int(ok.sum()),
+                             rel_sigma_T_mean=float(np.nanmean(rel)), rel_sigma_T_max=float(np.nanmax(rel)),
+                             rel_sigma_T_deciles=dec(rel), sys_error_deciles=dec(sys_),
+                             abs_sys_error_mean=float(np.nanmean(np.abs(sys_))), T_mean_K=float(T.mean())))
         m.close()
-    print(json.dumps(dict(study="config4 noise per shell vs packages", seeds=len(seeds), n_shells=p.n_shells,
-                          data="synthetic", rows=rows)))
+    print(json.dumps(dict(study="noise and systematic error per radius decile vs packages", seeds=len(seeds),
+                          reference_packages=10**9, data="synthetic", rows=rows)))
 
 
 def main():
@@ -359,7 +381,7 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--tune", default="", help="launch tuning for dies_set_tuning, e.g. visit=2,slots_uniform=5 (include/dies.h: dies_tuning)")
     ap.add_argument("--cpu-all-cores", action="store_true", help="also time the oracle on all host cores (one process each)")
-    ap.add_argument("--noise-study", action="store_true", help="config 4: sigma_T per shell over 8 seeds vs packages, FFI on / off")
+    ap.add_argument("--noise-study", action="store_true", help="configs 2, 3, 4: sigma_T and systematic error per radius decile over 8 seeds vs packages")
     args = ap.parse_args()
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))

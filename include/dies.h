@@ -135,6 +135,12 @@ int dies_run(dies_model*, uint64_t n_packages, uint64_t seed, const dies_run_opt
 int dies_seek(dies_model*, uint64_t first_id);
 int dies_run_batch(dies_model*, uint64_t n_packages_per_model, uint64_t seed, const dies_run_opts* opts,
                    void* cuda_stream);
+/* Sharding of a batch over processes / GPUs (config 5): the models of this handle are the models
+ * first_model .. first_model + n_models - 1 of a larger batch.  The model index is word 3 of the Philox counter (RNG
+ * contract), so a shard created from a slice of the batch's arrays follows exactly the packages the whole batch would
+ * follow for these models: the results of the shards, concatenated, are those of the one-GPU batch (bit for bit in
+ * fixed-temperature mode).  No exchange between shards is needed.  Default 0. */
+int dies_set_model_offset(dies_model*, uint32_t first_model);
 
 /* Dust temperatures from the absorbed-energy tallies (L87 lookup table; log-log interpolation, R6):
  * T[n_models x n_shells]; n must equal that size.  Synchronises the stream of the last run. */

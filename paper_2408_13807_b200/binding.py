@@ -24,7 +24,7 @@ EXPORTS = ("dies_workspace_bytes", "dies_create_model", "dies_create_batch", "di
            "dies_set_sources_batch", "dies_run", "dies_run_batch", "dies_get_temperature", "dies_get_escape_spectrum",
            "dies_set_fixed_temperature", "dies_get_absorbed", "dies_get_counters", "dies_trace_packages",
            "dies_trace_package", "dies_test_philox", "dies_get_tables", "dies_destroy", "dies_last_error",
-           "dies_device_info", "dies_bench_atomics", "dies_seek", "dies_set_tuning", "dies_get_tuning")
+           "dies_device_info", "dies_bench_atomics", "dies_seek", "dies_set_tuning", "dies_get_tuning", "dies_set_model_offset")
 
 
 class DiesError(RuntimeError):
@@ -69,6 +69,7 @@ def lib():
     L.dies_run.argtypes = [vp, u64, u64, C.POINTER(dies_run_opts), vp]
     L.dies_run_batch.argtypes = [vp, u64, u64, C.POINTER(dies_run_opts), vp]
     L.dies_seek.argtypes = [vp, u64]
+    L.dies_set_model_offset.argtypes = [vp, C.c_uint32]
     L.dies_get_temperature.argtypes = [vp, _dp, C.c_int]
     L.dies_get_escape_spectrum.argtypes = [vp, _dp, C.c_int]
     L.dies_set_fixed_temperature.argtypes = [vp, _dp, C.c_int]
@@ -222,6 +223,9 @@ class Model:
         _chk(lib().dies_run(self._h, int(n_packages), int(seed), C.byref(o), C.c_void_p(s)))
 
     dies_run_batch = dies_run
+
+    def dies_set_model_offset(self, first_model):
+        _chk(lib().dies_set_model_offset(self._h, int(first_model)))
 
     def dies_seek(self, first_id):
         _chk(lib().dies_seek(self._h, int(first_id)))

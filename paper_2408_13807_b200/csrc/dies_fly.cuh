@@ -255,7 +255,7 @@ __global__ void __launch_bounds__(kFlyBlock, 1) dies_fly(DeviceModel D, RunParam
                     if (act) {
                         uint32_t xw[4];
                         unsigned b = blk;
-                        philox4x32_10_rk(R.rk, (uint32_t)id, (uint32_t)(id >> 32), b, (uint32_t)m, xw);
+                        philox4x32_10_rk(R.rk, (uint32_t)id, (uint32_t)(id >> 32), b, (uint32_t)m + R.model0, xw);
                         float u0 = uniform24(xw[0]);
                         if (isabs) {
                             int row;
@@ -279,7 +279,7 @@ __global__ void __launch_bounds__(kFlyBlock, 1) dies_fly(DeviceModel D, RunParam
                                     row = row_from(s_eps, nT, row, es_);
                                     atomicAdd(&s_cnt[LC_EXTRA_BLOCKS], 1ull);
                                     b++;
-                                    philox4x32_10_rk(R.rk, (uint32_t)id, (uint32_t)(id >> 32), b, (uint32_t)m, xw);
+                                    philox4x32_10_rk(R.rk, (uint32_t)id, (uint32_t)(id >> 32), b, (uint32_t)m + R.model0, xw);
                                     u0 = uniform24(xw[0]);
                                 }
                             }
@@ -373,7 +373,7 @@ __global__ void __launch_bounds__(kFlyBlock, 1) dies_fly(DeviceModel D, RunParam
                             // ---- launch: one Philox block
                             uint32_t xw[4];
                             const bool point = mp.has_ext ? ((id - R.id_base) >= R.n_total) : true;
-                            philox4x32_10_rk(R.rk, (uint32_t)id, (uint32_t)(id >> 32), 0u, (uint32_t)m, xw);
+                            philox4x32_10_rk(R.rk, (uint32_t)id, (uint32_t)(id >> 32), 0u, (uint32_t)m + R.model0, xw);
                             blk = 1u;
                             const float u0 = uniform24(xw[0]), u1 = uniform24(xw[1]);
                             k = sample_cdf(g_src + (point ? K : 0), g_srcguide + (point ? kGuide : 0), u0);   // L55

@@ -93,6 +93,7 @@ struct dies_model {
     unsigned long long done, n_total;     // packages per source already followed / planned
     unsigned long long next_first;        // dies_seek: first package id (per source) of the next fresh run
     int shift;
+    uint32_t model0;                      // dies_set_model_offset
     cudaStream_t stream;
     int grid_max, blocks_per_sm, n_sms;
     int pool;                             // pool slots per warp of the tracker
@@ -598,7 +599,7 @@ extern "C" int dies_create_batch(int n_models, int n_shells, const double* r_bou
     m->N = N; m->K = K; m->nT = nT; m->M = M; m->ldS = N + 1;
     m->L = L; m->ws = (unsigned char*)workspace_dev;
     m->sources_set = m->fixed_set = m->ran = m->finalized = false;
-    m->done = m->n_total = 0; m->next_first = 0; m->shift = 24; m->stream = 0; m->launches = 0;
+    m->done = m->n_total = 0; m->next_first = 0; m->shift = 24; m->model0 = 0; m->stream = 0; m->launches = 0;
     m->L_point.assign(M, 0.0); m->has_ext.assign(M, 0); m->has_point.assign(M, 0);
     m->smem_bytes = smem; m->smem_trace_bytes = smem_trace; m->pool = pool; m->kref = kref;
     DeviceModel& D = m->D;
@@ -754,6 +755,7 @@ static int fill_run_params(dies_model* m, uint64_t n_packages, uint64_t seed, co
     for (int i = 0; i < m->M; i++) two |= (m->has_ext[i] && m->has_point[i]);
     R->n_run = n_packages; R->n_total = d.n_total; R->id_base = 0;
     R->key0 = (uint32_t)seed; R->key1 = (uint32_t)(seed >> 32);
+    R->model0 = m->model0;
     for (int r = 0; r < 10; r++) { R->rk[2 * r] = R->key0 + (uint32_t)r * 0x9E3779B9u; R->rk[2 * r + 1] = R->key1 + (uint32_t)r * 0xBB67AE85u; }
     R->k_bg = (float)d.k_bg; R->ffi = d.ffi ? 1 : 0;
     R->uniform_q = (d.k_bg == 0.5 && !d.ffi && !two && !weighted) ? 1 : 0;
@@ -853,6 +855,14 @@ extern "C" int dies_seek(dies_model* m, uint64_t first_id)
 {
     if (!m) return fail(DIES_EINVAL, "model is NULL");
     m->next_first = first_id;
+    return DIES_OK;
+}
+
+extern "C" int dies_set_model_offset(dies_model* m, uint32_t first_model)
+{
+    if (!m) return fail(DIES_EINVAL, "model is NULL");
+    if ((uint64_t)first_model + (uint64_t)m->M > 0xffffffffull) return fail(DIES_EINVAL, "model index beyond 2^32");
+    m->model0 = first_model;
     return DIES_OK;
 }
 

@@ -114,6 +114,7 @@ struct RunParams {
     unsigned long long id_base;      // packages per source done by earlier calls (accumulate)
     unsigned long long n_total;      // packages per source over the whole run
     uint32_t key0, key1;
+    uint32_t model0;                 // index of the handle's first model in the Philox counter (a shard of a batch)
     uint32_t rk[20];                 // Philox round keys: rk[2r] = key0 + r 0x9E3779B9, rk[2r+1] = key1 + r 0xBB67AE85
     float k_bg;
     int ffi;
@@ -576,7 +577,7 @@ __global__ void __launch_bounds__(kBlock, kMinBlocks) dies_track(DeviceModel D, 
                     const bool atsrc = launch;                                      // the event site is the source
                     const bool point = atsrc && (mp.has_ext ? ((id - R.id_base) >= R.n_total) : true);
                     unsigned b = blk;
-                    philox4x32_10_rk(R.rk, (uint32_t)id, (uint32_t)(id >> 32), b, (uint32_t)m, xw);
+                    philox4x32_10_rk(R.rk, (uint32_t)id, (uint32_t)(id >> 32), b, (uint32_t)m + R.model0, xw);
                     const float* cdf = nullptr;      // table the new frequency bin is drawn from (launch, re-emission)
                     const unsigned short* guide = nullptr;
                     if (isabs) {
@@ -602,7 +603,7 @@ __global__ void __launch_bounds__(kBlock, kMinBlocks) dies_track(DeviceModel D, 
                                 row = row_from(s_eps, nT, row, es);
                                 atomicAdd(&s_cnt[LC_EXTRA_BLOCKS], 1ull);
                                 b++;
-                                philox4x32_10_rk(R.rk, (uint32_t)id, (uint32_t)(id >> 32), b, (uint32_t)m, xw);
+                                philox4x32_10_rk(R.rk, (uint32_t)id, (uint32_t)(id >> 32), b, (uint32_t)m + R.model0, xw);
                             }
                         }
                         cdf = D.F + (size_t)row * K;
@@ -657,7 +658,7 @@ __global__ void __launch_bounds__(kBlock, kMinBlocks) dies_track(DeviceModel D, 
                             // L253 (R20): the package is re-emitted from a radius uniform in the volume of shell j;
                             // one more Philox block gives the uniform
                             uint32_t xr[4];
-                            philox4x32_10_rk(R.rk, (uint32_t)id, (uint32_t)(id >> 32), blk++, (uint32_t)m, xr);
+                            philox4x32_10_rk(R.rk, (uint32_t)id, (uint32_t)(id >> 32), blk++, (uint32_t)m + R.model0, xr);
                             const float ri2 = lds_entry4(tab0 + 16u * (unsigned)j).x, ro2 = lds_entry4(tab0 + 16u * (unsigned)(j + 1)).x;
                             const float ri = sqrtf(ri2), ro = sqrtf(ro2);
                             const float ri3 = ri * ri2, ro3 = ro * ro2;

@@ -7,7 +7,8 @@ One process per GPU.  What shards, and how:
     ranges (`package_range`), each rank follows its range with `dies_run(..., n_total=n, accumulate)` semantics
     (ids continue, energies are L / n_total), and the 64-bit integer tallies are summed with one all-reduce
     (`allreduce_tallies`): integer sums are order independent, so the result is bit-identical to one GPU;
-  * config 5 (independent spheres): models are dealt to ranks (`model_range`), no collective at all.
+  * config 5 (independent spheres): models are dealt to ranks (`model_range`, `batch_shard`; the shard's handle
+    keeps the models' indices in the Philox counter with dies_set_model_offset), no collective at all.
 """
 from __future__ import annotations
 
@@ -33,6 +34,25 @@ def package_range(n_packages: int, rank: int, world: int) -> tuple[int, int]:
 def model_range(n_models: int, rank: int, world: int) -> tuple[int, int]:
     """Contiguous range of model indices of rank `rank` (config 5: independent spheres, no exchange)."""
     return package_range(n_models, rank, world)
+
+
+def batch_shard(batch, rank: int, world: int):
+    """The spheres of a config-5 batch dealt to rank `rank`: (sub-batch, index of its first model).  The shard's handle
+    takes that index with dies_set_model_offset, so that its packages are those the whole batch would follow."""
+    import dataclasses
+    first, count = model_range(batch.n_models, rank, world)
+    sl = slice(first, first + count)
+    meta = {k: (v[sl] if hasattr(v, "shape") and getattr(v, "shape", ()) and v.shape[0] == batch.n_models else v)
+            for k, v in batch.meta.items()}
+    return dataclasses.replace(batch, r_bounds=batch.r_bounds[sl], rho=batch.rho[sl],
+                               ext_bin_intensity=batch.ext_bin_intensity[sl], meta=meta), first
+
+
+def sum_over_ranks(x: float, device) -> float:
+    t = torch.tensor([float(x)], dtype=torch.float64, device=device)
+    if dist.is_available() and dist.is_initialized() and dist.get_world_size() > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.SUM)
+    return float(t.item())
 
 
 def allreduce_tallies(*tallies: torch.Tensor) -> list[torch.Tensor]:
@@ -68,8 +88,8 @@ def run_fixed_T_shard(model, n_total: int, seed: int, rank: int, world: int, **o
     from . import binding
 
     first, count = package_range(n_total, rank, world)
-    model.dies_seek(first)
     if count > 0:
+        model.dies_seek(first)
         model.dies_run(count, seed=seed, mode=binding.DIES_MODE_FIXED_T, n_total=n_total, **opts)
         raw, unit, _ = model.dies_get_absorbed()
         esc = model.dies_get_escape_spectrum()

@@ -432,6 +432,38 @@ def test_fixed_T_shards_add_up_bit_exactly():
     whole.close()
 
 
+def test_batch_shards_equal_the_whole_batch_bit_for_bit():
+    """Config 5 sharded over ranks: two shards of the batch, each a handle of its own with
+    dies_set_model_offset, give the tallies of the one-handle batch bit for bit in fixed-temperature mode."""
+    from paper_2408_13807_b200 import sharding
+    b = synth.config5(n_models=7, n_packages=40_000, n_shells=24, n_freq=32, n_T=200)
+    Tfix = np.linspace(8.0, 30.0, 24)
+
+    def run(batch, first):
+        m = dies.Model(batch=batch)
+        m.dies_set_model_offset(first)
+        m.dies_set_fixed_temperature(np.tile(Tfix, (batch.n_models, 1)))
+        m.dies_run(batch.n_packages, seed=6, mode=dies.DIES_MODE_FIXED_T)
+        raw, _, _ = m.dies_get_absorbed()
+        esc = m.dies_get_escape_spectrum()
+        c = m.dies_get_counters()
+        m.close()
+        return raw.reshape(batch.n_models, -1).copy(), esc.reshape(batch.n_models, -1).copy(), c
+
+    raw, esc, c = run(b, 0)
+    parts = [run(*sharding.batch_shard(b, r, 3)) for r in range(3)]
+    assert np.array_equal(np.concatenate([q[0] for q in parts]), raw)
+    assert np.array_equal(np.concatenate([q[1] for q in parts]), esc)
+    for k in ("packages", "crossings", "scatterings", "absorptions", "escaped_raw"):
+        assert sum(q[2][k] for q in parts) == c[k], k
+    # without the offset the second shard would follow other packages
+    m = dies.Model(batch=sharding.batch_shard(b, 1, 3)[0])
+    m.dies_set_fixed_temperature(np.tile(Tfix, (m.n_models, 1)))
+    m.dies_run(b.n_packages, seed=6, mode=dies.DIES_MODE_FIXED_T)
+    assert not np.array_equal(m.dies_get_absorbed()[0].reshape(m.n_models, -1), parts[1][0])
+    m.close()
+
+
 def test_batch_full_ire_temperature_over_8_seeds(orc):
     """Config 5 reduced (4 spheres of 64 shells, one launch per seed): per-shell T of every model within 1 % or 3
     combined standard errors of the oracle's 8-seed mean; shells flagged once are re-examined on seeds 9-16."""

@@ -87,3 +87,60 @@ def test_fixed_T_shards_sum_to_the_single_run(tmp_path):
     assert np.array_equal(got["cnt"], cnt)
     assert got["cnt"][0] == N_PKG and a.sum() > 0
     assert float(got["slow"]) == 11.0
+
+
+# ------------------------------------------------------------------ config 5: the spheres of a batch dealt to ranks
+N_MODELS, N_BATCH_PKG = 5, 1500
+
+
+def _batch():
+    return synth.config5(n_models=N_MODELS, n_packages=N_BATCH_PKG, n_shells=8, n_freq=16, n_T=50)
+
+
+def _batch_T(orc, b, first):
+    """Temperatures of the models of (sub-)batch b, whose first model has index `first` in the whole batch."""
+    T = []
+    for i in range(b.n_models):
+        o = orc.Oracle(b.model(i))
+        o.run(b.n_packages, seed=SEED, model_index=first + i)
+        T.append(o.temperature())
+    return np.array(T)
+
+
+def _batch_worker(rank, world, port, outdir):
+    os.environ["MASTER_ADDR"] = "127.0.0.1"
+    os.environ["MASTER_PORT"] = str(port)
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    try:
+        from oracle import dies_oracle as orc
+        sub, first = sharding.batch_shard(_batch(), rank, world)
+        T = _batch_T(orc, sub, first)
+        n_all = sharding.sum_over_ranks(sub.n_models * sub.n_packages, "cpu")
+        np.savez(os.path.join(outdir, f"shard{rank}.npz"), T=T, first=first, n_all=n_all)
+    finally:
+        dist.destroy_process_group()
+
+
+def test_batch_shards_tile_the_models():
+    b = _batch()
+    for world in (1, 2, 3, 5, 8):
+        firsts, total = [], 0
+        for rank in range(world):
+            sub, first = sharding.batch_shard(b, rank, world)
+            assert np.array_equal(sub.rho, b.rho[first:first + sub.n_models])
+            assert np.array_equal(sub.ext_bin_intensity, b.ext_bin_intensity[first:first + sub.n_models])
+            assert len(sub.meta["tau_V"]) == sub.n_models
+            firsts.append(first); total += sub.n_models
+        assert total == b.n_models and firsts == sorted(firsts)
+
+
+def test_batch_shards_reproduce_the_whole_batch(tmp_path):
+    """World size 2 over gloo, no data-path collective: each rank follows its spheres with their indices of the whole
+    batch in the Philox counter; the concatenated temperatures equal those of the one-process batch exactly."""
+    from oracle import dies_oracle as orc
+    mp.spawn(_batch_worker, args=(2, _free_port(), str(tmp_path)), nprocs=2, join=True)
+    parts = [np.load(tmp_path / f"shard{r}.npz") for r in range(2)]
+    assert int(parts[0]["first"]) == 0 and int(parts[1]["first"]) == 3
+    assert float(parts[0]["n_all"]) == N_MODELS * N_BATCH_PKG
+    T = np.concatenate([q["T"] for q in parts])
+    assert np.array_equal(T, _batch_T(orc, _batch(), 0))
