@@ -94,6 +94,7 @@ struct dies_model {
     unsigned long long next_first;        // dies_seek: first package id (per source) of the next fresh run
     int shift;
     uint32_t model0;                      // dies_set_model_offset
+    int visit_auto;                       // crossing blocks per crossing phase, from the counters of the last read-out
     cudaStream_t stream;
     int grid_max, blocks_per_sm, n_sms;
     int pool;                             // pool slots per warp of the tracker
@@ -412,7 +413,7 @@ static int check_device()
 }
 
 // ------------------------------------------------------------------ launch tuning (include/dies.h: dies_tuning)
-static const dies_tuning kTuningDefaults = {5, 4, 8, 32, (int32_t)kChunk, kFlyWarps * 32, 96, 20, 16, 32, kTallyStride};
+static const dies_tuning kTuningDefaults = {5, 4, 0, 32, (int32_t)kChunk, kFlyWarps * 32, 96, 20, 16, 32, kTallyStride};
 static dies_tuning g_tuning = kTuningDefaults;
 static std::mutex g_tuning_mutex;
 
@@ -599,7 +600,7 @@ extern "C" int dies_create_batch(int n_models, int n_shells, const double* r_bou
     m->N = N; m->K = K; m->nT = nT; m->M = M; m->ldS = N + 1;
     m->L = L; m->ws = (unsigned char*)workspace_dev;
     m->sources_set = m->fixed_set = m->ran = m->finalized = false;
-    m->done = m->n_total = 0; m->next_first = 0; m->shift = 24; m->model0 = 0; m->stream = 0; m->launches = 0;
+    m->done = m->n_total = 0; m->next_first = 0; m->shift = 24; m->model0 = 0; m->visit_auto = 8; m->stream = 0; m->launches = 0;
     m->L_point.assign(M, 0.0); m->has_ext.assign(M, 0); m->has_point.assign(M, 0);
     m->smem_bytes = smem; m->smem_trace_bytes = smem_trace; m->pool = pool; m->kref = kref;
     DeviceModel& D = m->D;
@@ -768,7 +769,7 @@ static int fill_run_params(dies_model* m, uint64_t n_packages, uint64_t seed, co
     R->pool = tn.w_pool;
     R->thr_hi = tn.w_thr_hi; R->thr_lo = tn.w_thr_lo; R->min_ready = tn.w_min_ready;
     R->slots = fly_slots(R->uniform_q != 0);
-    R->visit = tn.visit;
+    R->visit = tn.visit > 0 ? tn.visit : m->visit_auto;
     if (!weighted) R->min_ready = tn.min_ready;
     R->n_tickets = 0; R->parts = 1;
     return DIES_OK;
@@ -888,10 +889,22 @@ static int finalize(dies_model* m)
     k_sum_escaped<<<1, 256, 0, m->stream>>>(m->D);
     m->launches += 2;
     int hf[2];
+    unsigned long long hc[DIES_C_ABSORPTIONS + 1];
     CUDA_TRY(cudaMemcpyAsync(hf, flags, sizeof(hf), cudaMemcpyDeviceToHost, m->stream));
+    CUDA_TRY(cudaMemcpyAsync(hc, m->ws + m->L.counters, sizeof(hc), cudaMemcpyDeviceToHost, m->stream));
     CUDA_TRY(cudaStreamSynchronize(m->stream));
     CUDA_TRY(cudaGetLastError());
     if (hf[1]) return fail(DIES_EOVERFLOW, "a tally exceeded 2^62");
+    {
+        // launch tuning of the next runs of this model (dies_tuning.visit = 0): a crossing phase of dies_fly lasts
+        // about two mean flights (a flight: the crossings between two events of a package).  Order of work only.
+        const double flights = (double)(hc[DIES_C_PACKAGES] + hc[DIES_C_SCATTERINGS] + hc[DIES_C_ABSORPTIONS]);
+        if (flights > 0.0) {
+            const double steps = 2.0 * (double)hc[DIES_C_CROSSINGS] / flights;
+            int v = (int)(steps / kSteps + 0.999);
+            m->visit_auto = v < 2 ? 2 : (v > 8 ? 8 : v);
+        }
+    }
     m->finalized = true;
     return DIES_OK;
 }
