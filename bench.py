@@ -28,14 +28,21 @@ if ROOT not in sys.path:
 
 from paper_2408_13807_b200 import sharding, synth  # noqa: E402
 
-# Algorithmic thread-instructions per unit of work in the shipped tracker (profiles/r1q_ncu_full.md and
-# r1r_ncu_full.md):
-# crossing = SASS instructions of one predicated crossing step; scattering / absorption / package = predicated-on
-# thread-instructions executed on the unit's own source lines (shared event stream + its own branch) per unit,
-# from the ncu source page of the same workload.  Queue handling, swaps, votes, fix-ups and idle lanes are NOT work.
-INSTR = dict(crossing=8, scattering=231, absorption=332, package=252)
-# dram__bytes_read.sum + dram__bytes_write.sum of one dies_track launch (ncu --set full, profiles/r1r_ncu_full.md)
-TRAFFIC_BYTES_PER_LAUNCH = 734464
+# Algorithmic thread-instructions per unit of work in the shipped tracker dies_fly (profiles/r2_ncu_full.md,
+# profiles/r2_cross_step.sass): crossing = SASS instructions of one crossing step on a live lane; scattering /
+# absorption / package = predicated-on thread-instructions of the unit's own code (+ its share of the code the two event
+# types have in common) per unit, from the ncu source page of this workload through
+# `python -m paper_2408_13807_b200.profile_parts`.  Stack handling, batch composition, slot load / store, block ends and
+# idle lanes are NOT work.  The constants belong to ONE version of the kernel sources: KERNEL_SHA256 is the hash they were
+# derived at, and a roofline is only printed while the sources still have it.
+INSTR = dict(crossing=8, scattering=174, absorption=345, package=260)
+KERNEL_SHA256 = "a84e3db16bb33b0ed5791fb51d0a618d4104bd72c7814918120e8f7f5da46b41"
+# of the same ncu --set full capture (one dies_fly launch of config 2, 1e7 packages):
+# dram__bytes_read.sum + dram__bytes_write.sum; busy fractions of the XU pipe (MUFU.SQRT of the crossings, 8 cycles per
+# warp instruction) and of the shared-memory data pipe (l1tex__data_pipe_lsu_wavefronts, 1 wavefront per cycle and SM)
+TRAFFIC_BYTES_PER_LAUNCH = 731904
+NCU_PIPE_BUSY = dict(issue=0.795, xu=0.305, smem_data=0.810)
+XU_CYCLES_PER_WARP_INSTR = 8
 SM_COUNT, SCHEDULERS, LANES = 148, 4, 32
 
 
@@ -83,7 +90,7 @@ class ClockSampler:
              "clocks_event_reasons.sw_power_cap")
         try:
             self.proc = subprocess.Popen(["nvidia-smi", f"--query-gpu={q}", "--format=csv,noheader,nounits",
-                                          "-i", str(self.index), "-lms", "50"], stdout=subprocess.PIPE, text=True)
+                                          "-i", str(self.index), "-lms", "10"], stdout=subprocess.PIPE, text=True)
             self.t = threading.Thread(target=self._read, daemon=True)
             self.t.start()
         except Exception:
@@ -91,9 +98,10 @@ class ClockSampler:
 
     def _read(self):
         for line in self.proc.stdout:
-            self.rows.append(line.strip())
+            self.rows.append((time.perf_counter(), line.strip()))
 
-    def stop(self):
+    def stop(self, t0=None, t1=None):
+        """Summary of the samples taken in [t0, t1] (perf_counter times; all samples if none fall inside)."""
         if not self.proc:
             return dict(sm_mhz=None, sm_max_mhz=None, reasons=["nvidia-smi unavailable"])
         self.proc.terminate()
@@ -102,7 +110,10 @@ class ClockSampler:
         except Exception:
             self.proc.kill()
         sm, mx, reasons = [], [], set()
-        for r in self.rows:
+        rows = [r for t, r in self.rows if t0 is None or t0 <= t <= t1 + 0.02]
+        if not rows:
+            rows = [r for _, r in self.rows]
+        for r in rows:
             f = [x.strip() for x in r.split(",")]
             if len(f) < 7:
                 continue
@@ -221,16 +232,17 @@ def run_ours(args, rank, world, local_rank):
             dist.barrier()
         torch.cuda.synchronize(dev)
 
+    sampler = ClockSampler(local_rank)                      # (started before the warm-up: nvidia-smi takes a while to report)
+    sampler.start()
     for w in range(args.warmup):
         m.dies_run(n_per_model, seed=sharding.replica_seed(1000, w, 0 if batch else rank), **opts)
     torch.cuda.synchronize(dev)
     c0 = m.dies_get_counters()
 
     # ---- device-timed steps: CUDA events on the launching stream, L2 flushed between steps
-    sampler = ClockSampler(local_rank)
-    sampler.start()
     barrier()
     t_wall = time.perf_counter()
+    t_begin = t_wall
     ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
     tot_counts = dict(crossings=0, scatterings=0, absorptions=0, packages=0)
     for s in range(args.steps):
@@ -240,7 +252,7 @@ def run_ours(args, rank, world, local_rank):
         ev[s][1].record(stream)
     barrier()
     t_wall = time.perf_counter() - t_wall
-    clocks = sampler.stop()
+    clocks = sampler.stop(t_begin, t_begin + t_wall)
     ms = [a.elapsed_time(b) for a, b in ev]
     c1 = m.dies_get_counters()
     # counters are zeroed by every non-accumulating run: c1 holds the last step; steps are statistically identical
@@ -282,6 +294,10 @@ def run_ours(args, rank, world, local_rank):
             c1["absorptions"] * INSTR["absorption"] + c1["packages"] * INSTR["package"])
     achieved = work / (step_ms * 1e-3) / 1e12
     held = clocks.get("sm_mhz") or sm_max
+    from paper_2408_13807_b200 import profile_parts
+    stale = profile_parts.kernel_hash() != KERNEL_SHA256
+    # the XU pipe executes the one square root of every crossing: 8 cycles per warp instruction and scheduler
+    xu_peak = SM_COUNT * SCHEDULERS * LANES * sm_max * 1e6 / XU_CYCLES_PER_WARP_INSTR
     line = dict(metric="packages_per_s", value=value, unit="packages/s", n_gpus=world, steps=args.steps,
                 warmup=args.warmup, ms_per_step=total_ms / args.steps, higher_is_better=True, scaling="weak",
                 vs_baseline=None, dtype="f32", data="synthetic",
@@ -303,9 +319,19 @@ def run_ours(args, rank, world, local_rank):
                                           peak_atomic_instr_per_s=atom["atomics_per_s"],
                                           frac=c1["absorptions"] / (step_ms * 1e-3) / atom["lane_ops_per_s"],
                                           peak_source=f"dies_bench_atomics({n_shells * min(n_models, 64)} tallies, the run's shell histogram, warp-merged={int(uniform_q)}) on this GPU"),
+                              xu=dict(crossings_per_s=c1["crossings"] / (step_ms * 1e-3), peak_sqrt_per_s=xu_peak,
+                                      frac=c1["crossings"] / (step_ms * 1e-3) / xu_peak,
+                                      note="one MUFU.SQRT per crossing; the XU pipe takes 8 cycles per warp instruction"),
+                              ncu_pipe_busy=NCU_PIPE_BUSY,
                               peak_source=f"148 SMs x 4 schedulers x 32 lanes x {sm_max:.0f} MHz ({peak_src})",
-                              instr_per_unit=INSTR, kernel="dies_track<0,false,false>", kernel_ms=step_ms),
+                              instr_per_unit=INSTR, kernel="dies_fly<0,false,4>", kernel_ms=step_ms),
                 wall_s=t_wall)
+    if stale:
+        # the work-per-unit constants were derived from other kernel sources: no fraction is claimed
+        line["roofline"] = dict(bound="alu", achieved=None, peak=peak, unit="Tinstr/s", frac=None, traffic=None,
+                                stale="kernel sources changed since INSTR was derived: run an ncu source page through "
+                                      "paper_2408_13807_b200.profile_parts and update INSTR and KERNEL_SHA256",
+                                kernel_ms=step_ms)
     # ---- the oracle timed beside it on this box's host cores (rank 0, N = 1 only)
     if world == 1 and not args.no_cpu_baseline:
         # bounded sample: a pilot of 4000 packages sizes the sample to about --cpu-seconds of CPU work

@@ -102,3 +102,13 @@ def test_c_example_compiles_and_links_against_the_library(tmp_path):
                         "-o", str(tmp_path / "c_abi_sphere"), "-L" + pkg, "-ldies", "-L" + os.path.join(cuda, "lib64"),
                         "-lcudart", "-lm", "-Wl,-rpath," + pkg], capture_output=True, text=True)
     assert r.returncode == 0, r.stderr
+
+
+def test_bench_constants_belong_to_the_kernel_sources():
+    """bench.py's work-per-unit constants (INSTR) were derived from an ncu source page of ONE version of the kernel
+    sources; bench.py prints a roofline fraction only while the sources still hash to KERNEL_SHA256.  This test keeps the
+    two from drifting apart unnoticed: after a kernel edit, re-profile, run profile_parts and update both."""
+    import bench
+    from paper_2408_13807_b200 import profile_parts
+    assert bench.KERNEL_SHA256 == profile_parts.kernel_hash()
+    assert set(bench.INSTR) == {"crossing", "scattering", "absorption", "package"}
