@@ -25,6 +25,8 @@
  *   IRE vs iteration ......... agreement with an independent 3-D Cartesian TMC (oracle/tmc_check.c; check d)
  *   k_bg, FFI ................ unbiasedness: same T(r) within errors, E[W] = 1
  *   directional weighting .... Eq. 6-7 (R19): HG normalisation, E[W] = 1, absorbed energy independent of g_S, T(r) of g_E
+ *   TMC iteration ............ L29-37 (R22): dies_oracle_tmc_run; pins in tests/test_oracle_tmc.py (independent
+ *                              Cartesian TMC, IRE fixed point, closed-form first flight, conservation)
  *   free-path weighting ...... Eq. 8 (R17): closed-form first flight under weighting, absorbed energy per shell
  *                              independent of k_A, k_S, k_A(rho); injected + reweight = escaped + terminated; guard (L119)
  * Parity unpinned: absolute T(r) of the optically thick configs 2 and 3 beyond IRE<->TMC agreement
@@ -72,6 +74,7 @@ typedef struct {
     double *kA, *kS, *g;               /* K */
     double *Tg, *eps;                  /* nT */
     double *F;                         /* nT x K row CDFs of the re-emission spectra */
+    double *G;                         /* nT x K row CDFs of the emission spectra themselves (TMC dust packages) */
     int has_ext, has_point;
     double *cdf_ext, *cdf_point;       /* K */
     double L_ext, L_point;
@@ -82,7 +85,7 @@ void dies_oracle_free(oracle_model* o)
 {
     if (!o) return;
     free(o->rb); free(o->rho); free(o->mass); free(o->kA); free(o->kS); free(o->g);
-    free(o->Tg); free(o->eps); free(o->F); free(o->cdf_ext); free(o->cdf_point); free(o->fixed_row);
+    free(o->Tg); free(o->eps); free(o->F); free(o->G); free(o->cdf_ext); free(o->cdf_point); free(o->fixed_row);
     free(o);
 }
 
@@ -119,10 +122,17 @@ oracle_model* dies_oracle_create(int n_shells, const double* r_bounds, const dou
     }
     o->eps = (double*)malloc(n_T * sizeof(double));
     o->F = (double*)malloc((size_t)n_T * n_freq * sizeof(double));
+    o->G = (double*)malloc((size_t)n_T * n_freq * sizeof(double));
     for (int t = 0; t < n_T; t++) {
         double s = 0.0;
         for (int k = 0; k < n_freq; k++) s += emis[(size_t)t * n_freq + k];
         o->eps[t] = s;
+        {
+            /* G[t][k] = sum_{j<=k} emis[t][j] / eps_t: the emission spectrum of T_t as a table u -> bin */
+            double c = 0.0;
+            for (int k = 0; k < n_freq; k++) { c += emis[(size_t)t * n_freq + k]; o->G[(size_t)t * n_freq + k] = s > 0 ? c / s : 1.0; }
+            o->G[(size_t)t * n_freq + n_freq - 1] = 1.0;
+        }
         if (t > 0 && !(o->eps[t] > o->eps[t - 1])) { dies_oracle_free(o); return NULL; }
         /* normalise by the sum of the differences themselves (= eps_t - eps_{t-1} up to rounding) */
         double tot = 0.0;
@@ -679,6 +689,121 @@ int dies_oracle_trace(const oracle_model* o, uint64_t n_total, uint64_t package_
     *n_events = rec.n_ev;
     *min_margin = rec.margin;
     free(absorbed); free(escaped);
+    return 0;
+}
+
+/* ------------------------------------------------------------------ traditional Monte Carlo (TMC), one iteration
+ * "The calculations can be divided into iterations, where the radiation field is estimated using
+ * up-to-date information on the radiation sources, including the emission from the dust with its current estimated
+ * temperatures.  When the simulation step has been finished, the knowledge of the radiation field is used to update the
+ * dust temperatures in every cell."  L37: "the energy absorption is calculated continuously, with updates made to
+ * every cell along the photon path between discrete scattering events".  L251: in TMC re-emission "happens uniformly
+ * over the cell".  Reading R22:
+ *   - every active source sends n_total packages as in the IRE method (L49-65); the dust sends n_total packages of
+ *     energy L_dust / n_total, L_dust = sum_i m_i eps_i, eps_i the power per mass cell i emits in its current state;
+ *   - a dust package starts in cell i with probability m_i eps_i / L_dust, at a radius uniform in the volume of the
+ *     cell, in an isotropic direction, in a bin drawn from the cell's emission spectrum C(eps_i), the cumulative
+ *     spectrum of reading R4 (piecewise linear in eps between the rows of the emission table): with probability
+ *     eps_{t-1} / eps_i from the spectrum of row t-1 itself, else from the difference spectrum of row t
+ *     (t = #{rows with eps_t <= eps_i});
+ *   - along a step of length l the package of weight W leaves W (1 - e^{-kappa_A rho l}) in the cell (the integral of
+ *     L37's update over the step) and keeps the rest; scatterings are discrete events at tau_S = -ln u (Eq. 1);
+ *   - a package ends when it leaves the model, or below 1e-10 of its launch weight (L119).
+ * Philox blocks of a package (RNG contract): source package: block 0 = (bin, direction, tau_S, -) as in the IRE method;
+ * dust package: block 0 = (cell, radius, direction cosine, row mix), block 1 = (bin, tau_S, -, -); every scattering:
+ * (cos Theta, phi, tau_S, -).  Package ids: the sources first ([0, n_total) ...), then the dust.
+ * The caller iterates: eps_i <- absorbed_i / m_i until the temperatures stop changing (L31). */
+int dies_oracle_tmc_run(const oracle_model* o, uint64_t n_total, uint64_t seed, uint32_t model_index,
+                        const double* eps_cur, double* absorbed, double* escaped, uint64_t* counters, double* sums)
+{
+    if (!o || !(o->has_ext || o->has_point) || n_total == 0) return -4;
+    const int N = o->N, K = o->K, nT = o->nT;
+    const int n_src = o->has_ext + o->has_point;
+    /* the cells as a source table (L55 applied to the dust) */
+    double* cellcdf = (double*)malloc(N * sizeof(double));
+    double L_dust = 0.0;
+    for (int i = 0; i < N; i++) { L_dust += o->mass[i] * (eps_cur ? eps_cur[i] : 0.0); cellcdf[i] = L_dust; }
+    if (L_dust > 0.0) { for (int i = 0; i < N; i++) cellcdf[i] /= L_dust; cellcdf[N - 1] = 1.0; }
+    const uint64_t n_ids = (uint64_t)(n_src + (L_dust > 0.0 ? 1 : 0)) * n_total;
+    for (uint64_t p = 0; p < n_ids; p++) {
+        stream s;
+        s.key[0] = (uint32_t)seed; s.key[1] = (uint32_t)(seed >> 32);
+        s.ctr[0] = (uint32_t)p; s.ctr[1] = (uint32_t)(p >> 32); s.ctr[2] = 0; s.ctr[3] = model_index;
+        const int which = (int)(p / n_total);                 /* 0 .. n_src-1: sources; n_src: dust */
+        double u[4], e, r, mu, tauS;
+        int i, k;
+        draw_block(&s, u);
+        if (which < n_src) {
+            const int src_is_point = (o->has_ext && o->has_point) ? which == 1 : o->has_point;
+            e = (src_is_point ? o->L_point : o->L_ext) / (double)n_total;
+            k = sample_cdf(src_is_point ? o->cdf_point : o->cdf_ext, K, u[0], NULL);
+            if (!src_is_point) { r = o->rb[N]; i = N - 1; mu = -sqrt(u[1]); }            /* Eq. 2 */
+            else { r = o->rb[0]; i = 0; mu = 1.0; }                                      /* L65, R9 */
+            tauS = -log(u[2]);
+        } else {
+            e = L_dust / (double)n_total;
+            i = sample_cdf(cellcdf, N, u[0], NULL);
+            const double ri = o->rb[i], ro = o->rb[i + 1];
+            r = cbrt(ri * ri * ri + u[1] * (ro * ro * ro - ri * ri * ri));               /* L251: uniform over the cell */
+            if (r < ri) r = ri;
+            if (r > ro) r = ro;
+            mu = 2.0 * u[2] - 1.0;
+            const double eps = eps_cur[i];
+            int t = 0;
+            while (t < nT && o->eps[t] <= eps) t++;                                      /* #{rows with eps_t <= eps} */
+            const double* cdf;
+            if (t >= nT) cdf = o->G + (size_t)(nT - 1) * K;                              /* beyond the table: its last row */
+            else if (t > 0 && u[3] < o->eps[t - 1] / eps) cdf = o->G + (size_t)(t - 1) * K;
+            else cdf = o->F + (size_t)t * K;
+            double v[4];
+            draw_block(&s, v);
+            k = sample_cdf(cdf, K, v[0], NULL);
+            tauS = -log(v[1]);
+        }
+        double W = 1.0;
+        uint64_t crossings = 0;
+        counters[C_PACKAGES] += 1;
+        sums[D_INJECTED] += e;
+        for (;;) {
+            double b2, l; int inward;
+            shell_step(o->rb, i, r, mu, &b2, &l, &inward);
+            const double rho = o->rho[i];
+            const double dtauS = o->kS[k] * rho * l;
+            const int event = !(tauS >= dtauS);
+            const double l_e = event ? l * tauS / dtauS : l;
+            /* L37: continuous absorption along the step */
+            const double dep = W * -expm1(-o->kA[k] * rho * l_e);
+            absorbed[i] += e * dep;
+            W -= dep;
+            if (!event) {
+                tauS -= dtauS;
+                if (cross_boundary(o->rb, N, &i, &r, &mu, b2, inward, &crossings)) {
+                    escaped[k] += W * e;
+                    sums[D_ESCAPED] += W * e;
+                    counters[C_ESCAPED] += 1;
+                    break;
+                }
+            } else {
+                double sp = r * mu + l_e;
+                double re = sqrt(b2 + sp * sp);
+                mu = re > 0.0 ? sp / re : 1.0;
+                if (mu > 1.0) mu = 1.0;
+                if (mu < -1.0) mu = -1.0;
+                r = re;
+                draw_block(&s, u);
+                mu = dies_oracle_scatter_direction(mu, dies_oracle_hg_cos(o->g[k], u[0]), 2.0 * PI * u[1]);
+                tauS = -log(u[2]);
+                counters[C_SCATTERINGS] += 1;
+            }
+            if (W < 1e-10) {                                   /* L119 */
+                sums[D_TERMINATED] += W * e;
+                counters[C_TERMINATED] += 1;
+                break;
+            }
+        }
+        counters[C_CROSSINGS] += crossings;
+    }
+    free(cellcdf);
     return 0;
 }
 

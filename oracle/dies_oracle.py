@@ -36,6 +36,7 @@ _lib.dies_oracle_run.argtypes = [_vp, _u64, _u64, _u64, _u64, _u64, C.c_uint32, 
 _lib.dies_oracle_trace.argtypes = [_vp, _u64, _u64, _u64, C.c_uint32, C.c_double, C.c_int, C.c_int, _dp, C.c_double,
                                    C.c_double, C.c_double, C.c_int, C.c_int,
                                    _dp, C.POINTER(C.c_int32), C.c_int, C.POINTER(C.c_int), _dp]
+_lib.dies_oracle_tmc_run.argtypes = [_vp, _u64, _u64, C.c_uint32, _dp, _dp, _dp, C.POINTER(_u64), _dp]
 _lib.dies_oracle_hg_pdf.restype = C.c_double
 _lib.dies_oracle_hg_pdf.argtypes = [C.c_double, C.c_double]
 _lib.dies_oracle_kA_profile.argtypes = [_vp, C.c_double, C.c_double, _dp]
@@ -169,6 +170,32 @@ class Oracle:
         if rc != 0:
             raise RuntimeError(f"dies_oracle_run failed: {rc}")
         return self
+
+    def tmc_run(self, n_total, seed=1, eps_cur=None, model_index=0):
+        """One iteration of the traditional Monte Carlo (reading R22): every active source and the
+        dust (cells emitting eps_cur, power per mass; None = cold dust) send n_total packages each, absorption is
+        continuous along the paths.  The tallies are reset first; returns self (absorbed, escaped, counters, sums)."""
+        self.reset()
+        e = None if eps_cur is None else _arr(eps_cur)
+        rc = _lib.dies_oracle_tmc_run(self._h, int(n_total), int(seed), int(model_index), _d(e), _d(self.absorbed),
+                                      _d(self.escaped), self._counters.ctypes.data_as(C.POINTER(_u64)), _d(self._sums))
+        if rc != 0:
+            raise RuntimeError(f"dies_oracle_tmc_run failed: {rc}")
+        return self
+
+    def tmc_solve(self, n_total, seed=1, max_iter=30, tol=3e-3, eps0=None, skip=0):
+        """TMC iterations eps <- absorbed / mass (L31) until max |dT / T| < tol over the shells from `skip` on (the
+        innermost shells of an externally heated sphere stay noisy, L177); returns (T, iterations, eps)."""
+        _, _, mass = self.tables()
+        eps, T_old = eps0, None
+        for it in range(1, max_iter + 1):
+            self.tmc_run(n_total, seed=seed + it, eps_cur=eps)
+            eps = np.where(mass > 0, self.absorbed / np.where(mass > 0, mass, 1.0), 0.0)
+            T = self.temperature()
+            if T_old is not None and np.max(np.abs(T / T_old - 1.0)[skip:]) < tol:
+                return T, it, eps
+            T_old = T
+        return T, max_iter, eps
 
     @property
     def counters(self):

@@ -30,3 +30,83 @@ def test_ire_matches_tmc_iteration(tau_V):
     # the temperature gradient is real: centre colder than surface for tau_V = 8
     if tau_V > 5:
         assert T_tmc[-1] > T_tmc[2] * 1.5
+
+
+# ------------------------------------------------------------------ the oracle's own TMC iteration (reading R22)
+# dies_oracle_tmc_run is the reference of the GPU's TMC mode; it is pinned here to things other than itself.
+def _toy(tau, kappa_sca=0.0, n_shells=6):
+    from test_oracle_pins import toy_problem
+    return toy_problem(n_shells=n_shells, tau=tau, kappa_sca=kappa_sca, g=0.3)
+
+
+@pytest.mark.parametrize("tau", [0.5, 1.0, 10.0])
+def test_tmc_first_flight_closed_form(tau):
+    """Uniform sphere, no scattering, the dust emits only in a transparent bin: the energy the continuous absorption
+     leaves in the sphere is the first-flight extinction 1 - [1 - (1 + 2 tau) e^{-2 tau}] / (2 tau^2)
+    of an isotropic field; with continuous absorption every package contributes its expectation along its chord, so
+    the estimate is far less noisy than counting absorption events."""
+    p = _toy(tau)
+    o = orc.Oracle(p)
+    n = 100000
+    o.tmc_run(n, seed=3)
+    expect = 1.0 - (1.0 - (1.0 + 2.0 * tau) * np.exp(-2.0 * tau)) / (2.0 * tau * tau)
+    got = o.absorbed.sum() / o.sums["injected"]
+    assert abs(got / expect - 1.0) < 2.5e-3, (got, expect)
+    # energy conservation to rounding: absorbed + escaped + terminated = injected
+    tot = o.absorbed.sum() + o.sums["escaped"] + o.sums["terminated"]
+    assert abs(tot / o.sums["injected"] - 1.0) < 1e-10
+    assert o.counters["packages"] == n and o.counters["scatterings"] == 0
+
+
+def test_tmc_conservation_with_scattering_and_dust_packages():
+    p = synth.config1(tau_V=4.0)
+    o = orc.Oracle(p)
+    o.tmc_run(20000, seed=1)
+    _, _, mass = o.tables()
+    eps = o.absorbed / mass
+    L_dust = float(np.sum(mass * eps))
+    o.tmc_run(20000, seed=2, eps_cur=eps)
+    assert o.counters["packages"] == 40000 and o.counters["scatterings"] > 0
+    # the dust re-emits exactly what the cells absorbed in the iteration before
+    assert abs(o.sums["injected"] / (4 * np.pi * p.r_bounds[-1] ** 2 * np.pi * p.ext_bin_intensity.sum() + L_dust) - 1) < 1e-12
+    tot = o.absorbed.sum() + o.sums["escaped"] + o.sums["terminated"]
+    assert abs(tot / o.sums["injected"] - 1.0) < 1e-10
+
+
+def test_tmc_dust_package_spectrum_is_the_cell_spectrum():
+    """A single transparent shell emitting eps between two table rows: the escaping spectrum of the dust packages is
+    C(eps) of reading R4 -- the spectrum of the row below plus the share of the difference spectrum of the row above."""
+    p = synth.config1(n_shells=1, tau_V=1e-9)
+    p.ext_bin_intensity = p.ext_bin_intensity * 1e-30          # a source there must be; it carries no energy here
+    o = orc.Oracle(p)
+    eps_t, F, mass = o.tables()
+    t = 300
+    eps = 0.5 * (eps_t[t - 1] + eps_t[t])
+    n = 400000
+    o.tmc_run(n, seed=4, eps_cur=np.array([eps]))
+    src = 4 * np.pi * p.r_bounds[-1] ** 2 * np.pi * p.ext_bin_intensity        # the external field passes through
+    got = (o.escaped - src) / (mass[0] * eps)
+    expect = (p.emis[t - 1] + 0.5 * (p.emis[t] - p.emis[t - 1])) / eps
+    sig = np.sqrt(np.maximum(expect, 1e-12) / n)
+    assert np.max(np.abs(got - expect) / (sig + 2e-4)) < 5.0
+
+
+@pytest.mark.parametrize("tau_V", [1.0, 8.0])
+def test_tmc_oracle_matches_independent_tmc_and_ire(tau_V):
+    """Converged temperatures of config 1: the oracle's TMC iteration (r / mu geometry, Philox) against the independent
+    Cartesian TMC of tmc_check.c and against the oracle's IRE."""
+    p = synth.config1(tau_V=tau_V)
+    T_ref, it_ref = tmc_check.tmc_solve(p, n_src=400000, n_dust=320000, max_iter=30, tol=3e-3, seed=5)
+    o = orc.Oracle(p)
+    T, it, eps = o.tmc_solve(150000, seed=10, max_iter=30, tol=4e-3, skip=8)
+    assert 1 < it < 30 and 1 <= it_ref < 30
+    assert np.max(np.abs(T / T_ref - 1.0)[8:]) < 0.012, T / T_ref
+    Ti = np.array([orc.Oracle(p).run(250000, seed=s).temperature() for s in (1, 2)]).mean(0)
+    assert np.max(np.abs(T[12:] / Ti[12:] - 1.0)) < 0.012, T / Ti
+    # the IRE solution is a fixed point of the TMC iteration (within the noise of both)
+    o2 = orc.Oracle(p).run(250000, seed=7)
+    _, _, mass = o2.tables()
+    eps_ire = o2.absorbed / mass
+    o3 = orc.Oracle(p)
+    o3.tmc_run(150000, seed=11, eps_cur=eps_ire)
+    assert np.max(np.abs(o3.temperature()[12:] / o2.temperature()[12:] - 1.0)) < 0.02   # (IRE noise of one seed)
