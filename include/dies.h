@@ -48,7 +48,15 @@ enum {
 };
 
 /* modes of dies_run */
-enum { DIES_MODE_IRE = 0, DIES_MODE_FIXED_T = 1 };
+enum { DIES_MODE_IRE = 0, DIES_MODE_FIXED_T = 1,
+       /* One iteration of the traditional Monte Carlo (R22): every active source and the
+        * dust send n_packages packages each, absorption is tallied continuously along the paths, scatterings are
+        * discrete events.  The dust emits, uniformly over every cell (L251), the power per mass the cell absorbed in the
+        * PREVIOUS run of the handle (whatever its mode; nothing before the first run), with the cell's emission spectrum.
+        * Calling dies_run with this mode repeatedly is the TMC iteration; dies_get_temperature after each run gives the
+        * temperatures to watch for convergence (L31).  Plain runs only: k_bg = 0.5, no ffi, no weighting, no accumulate,
+        * fixed_shift <= 24. */
+       DIES_MODE_TMC = 2 };
 
 /* event types of dies_trace_* (quadruples: type, shell, freq_bin, crossings so far) */
 enum { DIES_EV_LAUNCH = 0, DIES_EV_SCATTER = 1, DIES_EV_ABSORB = 2, DIES_EV_ESCAPE = 3,
@@ -65,7 +73,7 @@ enum { DIES_C_PACKAGES = 0, DIES_C_CROSSINGS, DIES_C_FFI_CROSSINGS, DIES_C_SCATT
 typedef struct {
     double   k_bg;        /* Eq. 5: mu = u^k_bg, W = 2 k_bg mu^(2-1/k_bg); 0.5 = unweighted (Eq. 2)          */
     int32_t  ffi;         /* Eq. 9-12: forced first interaction on the launch flight (R11)                  */
-    int32_t  mode;        /* DIES_MODE_IRE or DIES_MODE_FIXED_T (rows from dies_set_fixed_temperature)      */
+    int32_t  mode;        /* DIES_MODE_IRE, DIES_MODE_FIXED_T (rows from dies_set_fixed_temperature) or _TMC */
     int32_t  accumulate;  /* 0: zero tallies and counters first; 1: continue (package ids continue too)     */
     int32_t  fixed_shift; /* S: a package of weight W adds round(W 2^S) to the 64-bit tallies; 0 -> 24      */
     uint64_t n_total;     /* packages per source over the whole (possibly split) run; package energy is

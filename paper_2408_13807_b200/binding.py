@@ -15,7 +15,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(HERE, "libdies.so")
 
 DIES_OK, DIES_EINVAL, DIES_ENOMEM, DIES_ECUDA, DIES_ESTATE, DIES_EOVERFLOW = 0, -1, -2, -3, -4, -5
-DIES_MODE_IRE, DIES_MODE_FIXED_T = 0, 1
+DIES_MODE_IRE, DIES_MODE_FIXED_T, DIES_MODE_TMC = 0, 1, 2
 COUNTER_NAMES = ("packages", "crossings", "ffi_crossings", "scatterings", "absorptions", "escaped", "uninteracted",
                  "terminated", "extra_blocks", "clamp_hi_samples", "injected_raw", "terminated_raw", "reweight_raw",
                  "escaped_raw", "T_clamp_lo", "T_clamp_hi", "kernel_launches")

@@ -12,6 +12,7 @@
 #include "../../include/dies.h"
 #include "dies_tracker.cuh"
 #include "dies_fly.cuh"
+#include "dies_tmc.cuh"
 
 using namespace dies;
 
@@ -35,6 +36,7 @@ extern "C" const char* dies_last_error(void) { return g_err; }
 
 // ------------------------------------------------------------------ workspace layout
 struct Layout {
+    size_t G, epscur, cellcdf, tmcrow, tmcmix, Ldust, qsdust;      // TMC mode (dies_tmc.cuh)
     size_t emis, eps, Tgrid, epsgrid, F, guideF, guideS, stabW, bintab, omega, dustin, rb, rho, mass, stab, cscale, srccdf, srcin, Lsrc, mp,
         fixed_row, Tfix, A, esc, next_id, counters, ticket, T_out, Lesc_out, eunit, flags, epsref, total;
 };
@@ -50,6 +52,13 @@ static Layout make_layout(int N, int K, int nT, int M)
     L.Tgrid = take((size_t)nT * 8);
     L.epsgrid = take((size_t)nT * 4);
     L.F = take((size_t)nT * K * 4);
+    L.G = take((size_t)nT * K * 4);
+    L.epscur = take((size_t)M * ldS * 8);
+    L.cellcdf = take((size_t)M * ldS * 4);
+    L.tmcrow = take((size_t)M * ldS * 4);
+    L.tmcmix = take((size_t)M * ldS * 4);
+    L.Ldust = take((size_t)M * 8);
+    L.qsdust = take((size_t)M * 4);
     L.guideF = take((size_t)nT * kGuide * 2);
     L.guideS = take((size_t)M * 2 * kGuide * 2);
     L.stabW = take((size_t)M * 2 * (ldS + 1) * 16);
@@ -109,7 +118,7 @@ static T* wsp(dies_model* m, size_t off) { return reinterpret_cast<T*>(m->ws + o
 // ------------------------------------------------------------------ table construction kernels
 // eps_t = sum_k emis[t][k];  F[t][k] = cumsum_k(emis[t] - emis[t-1]) / sum_k(emis[t] - emis[t-1])   (R4)
 __global__ void k_build_tables(const double* __restrict__ emis, int nT, int K, double* __restrict__ eps,
-                               float* __restrict__ F, int* flags)
+                               float* __restrict__ F, float* __restrict__ G, int* flags)
 {
     // one warp per temperature row: lane l owns the bins [l c, (l+1) c), c = ceil(K / 32)
     const int t = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
@@ -126,20 +135,24 @@ __global__ void k_build_tables(const double* __restrict__ emis, int nT, int K, d
         part += d;
     }
     // totals and the exclusive prefix of the partial sums of the increments
-    double tot = part, ssum = s, pre = part;
+    double tot = part, ssum = s, pre = part, pres = s;
     for (int o = 1; o < 32; o <<= 1) {
-        const double v = __shfl_up_sync(0xffffffffu, pre, o);
-        if (lane >= o) pre += v;
+        const double v = __shfl_up_sync(0xffffffffu, pre, o), vs = __shfl_up_sync(0xffffffffu, pres, o);
+        if (lane >= o) { pre += v; pres += vs; }
     }
+    pres -= s;
     for (int o = 16; o > 0; o >>= 1) { tot += __shfl_xor_sync(0xffffffffu, tot, o); ssum += __shfl_xor_sync(0xffffffffu, ssum, o); }
     pre -= part;
     if (__any_sync(0xffffffffu, bad) || !(tot > 0.0)) { if (lane == 0) atomicOr(flags, 1); }
     if (lane == 0) eps[t] = ssum;
     float* f = F + (size_t)t * K;
-    double cum = pre;
+    float* gt = G + (size_t)t * K;                           // the spectrum of T_t itself (TMC dust packages, R22)
+    double cum = pre, cums = pres;
     for (int k = k0; k < k1; k++) {
         cum += row[k] - (prev ? prev[k] : 0.0);
+        cums += row[k];
         f[k] = (k == K - 1) ? 1.0f : (float)(cum / tot);
+        gt[k] = (k == K - 1 || !(ssum > 0.0)) ? 1.0f : (float)(cums / ssum);
     }
 }
 
@@ -316,9 +329,42 @@ __global__ void k_fixed_rows(const double* __restrict__ Tfix, const double* __re
 }
 
 // per run: energy scale of the raw tallies, zeroing, counters
+// TMC mode (dies_tmc.cuh; R22): the state of the dust for the next iteration from the tallies of the run before:
+// eps_i = absorbed_i / m_i (0 before any run), the cells as a source table, the table row and the mixing share of every
+// cell's spectrum C(eps_i), the dust luminosity.  One thread per model; runs before k_prepare_run rescales the tallies.
+__global__ void k_tmc_prepare(DeviceModel D, const double* __restrict__ mass, const double* __restrict__ eunit,
+                              const double* __restrict__ eps, int have_state, double* epscur, float* cellcdf, int* row,
+                              float* mix, double* Ldust)
+{
+    const int m = blockIdx.x * blockDim.x + threadIdx.x;
+    if (m >= D.n_models) return;
+    const int ldS = D.ldS, nT = D.nT, Np = D.mp[m].Np;
+    double L = 0.0;
+    for (int j = 0; j < ldS; j++) {
+        const size_t x = (size_t)m * ldS + j;
+        const double ms = j < Np ? mass[x] : 0.0;
+        const double e = (have_state && ms > 0.0) ? (double)D.A[x * kTallyStride] * eunit[m] / ms : 0.0;
+        epscur[x] = e;
+        int lo = 0, hi = nT;                           // #{rows with eps_t <= e}
+        while (lo < hi) { const int mid = (lo + hi) >> 1; if (eps[mid] > e) hi = mid; else lo = mid + 1; }
+        row[x] = lo;
+        mix[x] = lo == 0 ? 0.f : (lo >= nT ? 1.f : (float)(eps[lo - 1] / e));
+        L += ms * e;
+    }
+    Ldust[m] = L;
+    double c = 0.0;
+    for (int j = 0; j < ldS; j++) {
+        const size_t x = (size_t)m * ldS + j;
+        c += (j < Np ? mass[x] : 0.0) * epscur[x];
+        cellcdf[x] = L > 0.0 ? (float)(c / L) : 1.f;
+    }
+    if (L > 0.0) for (int j = Np - 1; j < ldS; j++) cellcdf[(size_t)m * ldS + j] = 1.f;
+}
+
 __global__ void k_prepare_run(DeviceModel D, const double* __restrict__ mass, const double* __restrict__ Lsrc,
                               const double* __restrict__ epsref, double* cscale, double* eunit, ModelParams* mp,
-                              double n_total, double qscale, int zero)
+                              double n_total, double qscale, int zero, const double* __restrict__ Ldust = nullptr,
+                              float* qsdust = nullptr)
 {
     const int ldS = D.ldS;
     const int idx = blockIdx.x * blockDim.x + threadIdx.x;
@@ -327,9 +373,11 @@ __global__ void k_prepare_run(DeviceModel D, const double* __restrict__ mass, co
         D.next_id[idx] = 0ull;
         ModelParams p = mp[idx];
         const double Le = p.has_ext ? Lsrc[2 * idx] : 0.0, Lp = p.has_point ? Lsrc[2 * idx + 1] : 0.0;
-        const double Lref = fmax(Le, Lp);
+        const double Ld = Ldust ? Ldust[idx] : 0.0;          // TMC mode: the dust is a source of its own (R22)
+        const double Lref = fmax(fmax(Le, Lp), Ld);
         p.qs_ext = Lref > 0 ? (float)(Le / Lref) : 0.f;
         p.qs_point = Lref > 0 ? (float)(Lp / Lref) : 0.f;
+        if (qsdust) qsdust[idx] = Lref > 0 ? (float)(Ld / Lref) : 0.f;
         mp[idx] = p;
         eunit[idx] = Lref / n_total / qscale;
     }
@@ -337,7 +385,7 @@ __global__ void k_prepare_run(DeviceModel D, const double* __restrict__ mass, co
         const int m = idx / ldS;
         const ModelParams p = mp[m];
         const double Le = p.has_ext ? Lsrc[2 * m] : 0.0, Lp = p.has_point ? Lsrc[2 * m + 1] : 0.0;
-        const double eu = fmax(Le, Lp) / n_total / qscale;
+        const double eu = fmax(fmax(Le, Lp), Ldust ? Ldust[m] : 0.0) / n_total / qscale;
         const double ms = mass[idx];
         cscale[idx] = ms > 0.0 ? eu / (ms * *epsref) : 0.0;
         if (zero) D.A[(size_t)idx * kTallyStride] = 0ull;
@@ -627,7 +675,7 @@ extern "C" int dies_create_batch(int n_models, int n_shells, const double* r_bou
     TRY_OR_FREE(cudaMemcpyAsync(m->ws + L.rb, r_bounds, (size_t)M * (N + 1) * 8, cudaMemcpyHostToDevice, 0));
     TRY_OR_FREE(cudaMemcpyAsync(m->ws + L.rho, rho, (size_t)M * N * 8, cudaMemcpyHostToDevice, 0));
     int* flags = wsp<int>(m, L.flags);
-    k_build_tables<<<(nT * 32 + 127) / 128, 128>>>(wsp<double>(m, L.emis), nT, K, wsp<double>(m, L.eps), wsp<float>(m, L.F), flags);
+    k_build_tables<<<(nT * 32 + 127) / 128, 128>>>(wsp<double>(m, L.emis), nT, K, wsp<double>(m, L.eps), wsp<float>(m, L.F), wsp<float>(m, L.G), flags);
     k_build_guide<<<(nT * kGuide + 255) / 256, 256>>>(wsp<float>(m, L.F), nT, K, wsp<unsigned short>(m, L.guideF));
     k_build_epsgrid<<<(nT + 127) / 128, 128>>>(wsp<double>(m, L.eps), nT, wsp<float>(m, L.epsgrid), wsp<double>(m, L.epsref), flags);
     k_build_dust<<<(K + 127) / 128, 128>>>(wsp<double>(m, L.dustin), K, kref, wsp<float4>(m, L.bintab), wsp<float>(m, L.omega));
@@ -746,7 +794,9 @@ static int fill_run_params(dies_model* m, uint64_t n_packages, uint64_t seed, co
                           d.reemit_in_cell != 0;
     if (weighted && d.ffi) return fail(DIES_EINVAL, "free-path / directional weighting and forced first interaction are alternatives, not combined");
     if (!(d.k_bg > 0.0) || d.k_bg > 1.0) return fail(DIES_EINVAL, "k_bg must be in (0, 1]");
-    if (d.mode != DIES_MODE_IRE && d.mode != DIES_MODE_FIXED_T) return fail(DIES_EINVAL, "bad mode");
+    if (d.mode != DIES_MODE_IRE && d.mode != DIES_MODE_FIXED_T && d.mode != DIES_MODE_TMC) return fail(DIES_EINVAL, "bad mode");
+    if (d.mode == DIES_MODE_TMC && (weighted || d.ffi || d.k_bg != 0.5 || d.accumulate || (d.n_total && d.n_total != n_packages)))
+        return fail(DIES_EINVAL, "a TMC iteration is one plain run: no weighting, no forced first interaction, no accumulate");
     if (d.fixed_shift == 0) d.fixed_shift = 24;
     if (d.fixed_shift < 1 || d.fixed_shift > 30) return fail(DIES_EINVAL, "fixed_shift must be in [1, 30]");
     if (d.n_total == 0) d.n_total = n_packages;
@@ -797,6 +847,44 @@ extern "C" int dies_run(dies_model* m, uint64_t n_packages, uint64_t seed, const
     if (m->ran && st != m->stream) CUDA_TRY(cudaStreamSynchronize(m->stream));
     m->stream = st;
     m->n_total = n_total; m->shift = shift;
+
+    if (mode == DIES_MODE_TMC) {
+        // one iteration of the traditional Monte Carlo (dies_tmc.cuh): the dust emits what the run before left in it
+        if (m->shift > 24) return fail(DIES_EINVAL, "TMC mode keeps package quanta in 32 bits: fixed_shift <= 24");
+        const TmcPlan tpn = plan_tmc(m->K, m->ldS, m->D.ldT);
+        static std::mutex mu;
+        {
+            std::lock_guard<std::mutex> lock(mu);
+            CUDA_TRY(cudaFuncSetAttribute(dies_tmc, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
+        }
+        if (tpn.total > 200 * 1024) return fail(DIES_EINVAL, "tables do not fit in shared memory");
+        int bps = 0;
+        CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&bps, dies_tmc, kBlock, tpn.total));
+        if (bps < 1) return fail(DIES_ECUDA, "tracker does not fit on an SM");
+        const int grid = m->n_sms * bps;
+        R.chunk = 32u * 8u;
+        if (m->M == 1) { R.parts = grid; R.n_tickets = grid; }
+        else { R.parts = (8 * grid + m->M - 1) / m->M; if (R.parts < 1) R.parts = 1; R.n_tickets = m->M * R.parts; }
+        k_tmc_prepare<<<(m->M + 63) / 64, 64, 0, st>>>(m->D, wsp<double>(m, m->L.mass), wsp<double>(m, m->L.eunit),
+                                                      wsp<double>(m, m->L.eps), m->ran ? 1 : 0, wsp<double>(m, m->L.epscur),
+                                                      wsp<float>(m, m->L.cellcdf), wsp<int>(m, m->L.tmcrow),
+                                                      wsp<float>(m, m->L.tmcmix), wsp<double>(m, m->L.Ldust));
+        const int prep = m->M * (m->K > m->ldS ? m->K : m->ldS);
+        k_prepare_run<<<(prep + 255) / 256, 256, 0, st>>>(m->D, wsp<double>(m, m->L.mass), wsp<double>(m, m->L.Lsrc),
+                                                        wsp<double>(m, m->L.epsref), wsp<double>(m, m->L.cscale),
+                                                        wsp<double>(m, m->L.eunit), wsp<ModelParams>(m, m->L.mp),
+                                                        (double)n_total, (double)R.qscale, 1, wsp<double>(m, m->L.Ldust),
+                                                        wsp<float>(m, m->L.qsdust));
+        const TmcModel Tm = {wsp<float>(m, m->L.G), wsp<float>(m, m->L.cellcdf), wsp<int>(m, m->L.tmcrow),
+                             wsp<float>(m, m->L.tmcmix), wsp<float>(m, m->L.qsdust)};
+        dies_tmc<<<grid, kBlock, tpn.total, st>>>(m->D, R, Tm, tpn);
+        m->launches += 3;
+        CUDA_TRY(cudaGetLastError());
+        m->done += n_packages;
+        m->ran = true;
+        m->finalized = false;
+        return DIES_OK;
+    }
 
     // launch shape: shared memory of this run's pool, persistent blocks (as many as fit on an SM), fewer for tiny runs
     const bool wt = R.weighted != 0;
