@@ -216,6 +216,11 @@ def run_ours(args, rank, world, local_rank):
     k_bg, ffi = getattr(p, "k_bg", 0.5), getattr(p, "ffi", 0)
     n_shells, n_freq, n_T = int(p.rho.shape[-1]), int(p.freq.size), int(p.T_grid.size)
     opts = dict(k_bg=k_bg, ffi=ffi)
+    tmc = args.mode == "tmc"
+    if tmc:
+        # the second workload (R22): a step is one iteration of the traditional Monte Carlo with continuous
+        # absorption in its steady state (sources + as many dust packages); plain runs only
+        opts = dict(mode=dies.DIES_MODE_TMC)
     def make():
         if not batch:
             return dies.Model(p, device=str(dev))
@@ -260,6 +265,8 @@ def run_ours(args, rank, world, local_rank):
         tot_counts[k] = c1[k]
     step_ms = float(np.sum(ms)) / args.steps
     total_ms = sharding.max_over_ranks(float(np.sum(ms)), dev)
+    if tmc:
+        n = int(c1["packages"])                             # sources + dust packages of an iteration
     n_all = sharding.sum_over_ranks(n, dev)                # packages per step of the whole job
     value = n_all * args.steps / (total_ms * 1e-3)
     crossings_per_s = sharding.sum_over_ranks(c1["crossings"], dev) * args.steps / (total_ms * 1e-3)
@@ -275,7 +282,9 @@ def run_ours(args, rank, world, local_rank):
         Lesc = m2.dies_get_escape_spectrum()
         e2e_t.append(time.perf_counter() - t0)
         m2.close()
-    e2e_val = n_all / sharding.max_over_ranks(float(np.median(e2e_t)), dev)
+    # (a fresh handle's first TMC iteration has no dust packages yet: its end-to-end figure counts the source packages)
+    e2e_n = sharding.sum_over_ranks(n_per_model * n_models, dev) if tmc else n_all
+    e2e_val = e2e_n / sharding.max_over_ranks(float(np.median(e2e_t)), dev)
     h2d = 8 * (p.emis.size + p.T_grid.size + 3 * n_freq + p.r_bounds.size + p.rho.size + 2 * n_freq * n_models)
     d2h = 8 * n_models * (n_shells + n_freq) + 64
 
@@ -326,7 +335,12 @@ def run_ours(args, rank, world, local_rank):
                               peak_source=f"148 SMs x 4 schedulers x 32 lanes x {sm_max:.0f} MHz ({peak_src})",
                               instr_per_unit=INSTR, kernel="dies_fly<0,false,4>", kernel_ms=step_ms),
                 wall_s=t_wall)
-    if stale:
+    if tmc:
+        line["config"]["mode"] = "TMC iteration (continuous absorption), steady state"
+        line["roofline"] = dict(bound="alu", achieved=None, peak=peak, unit="Tinstr/s", frac=None, traffic=None,
+                                kernel="dies_tmc", kernel_ms=step_ms,
+                                note="second workload: no work-per-unit constants were derived for dies_tmc")
+    elif stale:
         # the work-per-unit constants were derived from other kernel sources: no fraction is claimed
         line["roofline"] = dict(bound="alu", achieved=None, peak=peak, unit="Tinstr/s", frac=None, traffic=None,
                                 stale="kernel sources changed since INSTR was derived: run an ncu source page through "
@@ -405,6 +419,7 @@ def main():
     ap.add_argument("--ref-sample", type=int, default=1_000_000)
     ap.add_argument("--ref-total", type=int, default=20_000_000)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--mode", default="ire", choices=["ire", "tmc"], help="full IRE (the headline) or one TMC iteration per step")
     ap.add_argument("--tune", default="", help="launch tuning for dies_set_tuning, e.g. visit=2,slots_uniform=5 (include/dies.h: dies_tuning)")
     ap.add_argument("--cpu-all-cores", action="store_true", help="also time the oracle on all host cores (one process each)")
     ap.add_argument("--noise-study", action="store_true", help="configs 2, 3, 4: sigma_T and systematic error per radius decile over 8 seeds vs packages")
