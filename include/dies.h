@@ -170,6 +170,37 @@ int dies_trace_packages(dies_model*, int model_index, uint64_t first_id, int cou
                         const dies_run_opts* opts, int32_t* events, int max_events, int32_t* n_events);
 int dies_trace_package(dies_model*, uint64_t package_id, uint64_t n_total, uint64_t seed, const dies_run_opts* opts,
                        int32_t* events, int max_events, int32_t* n_events);
+/* dies_trace_packages for callers that must not allocate device memory.
+ *
+ * Who needs it: a process in which a framework's caching allocator (PyTorch's, for one) has already taken nearly all of
+ * the GPU, so that a raw cudaMalloc from this library fails although the framework still has room to hand out; and a
+ * service that replays packages while other streams run trackers, where cudaMalloc / cudaFree would stall the whole
+ * device (cudaFree waits for all work on it).  dies_trace_packages does both per call; this entry point does neither.
+ *
+ * How: the event lists, the event counts and the package counter live in one fixed array inside the library image
+ * (1 MiB + 16 KiB + 256 B).  Every GPU on which libdies.so is loaded holds that array until the process exits, used or
+ * not.  Inputs (the handle and its caller-owned workspace) and outputs (the host buffers events / n_events) are passed
+ * exactly as for dies_trace_packages, and the results are the same, with one difference: entries of events[p] past
+ * n_events[p] are zero here and undefined there.
+ *
+ * Limits: count <= DIES_TRACE_STATIC_MAX_PACKAGES and count * max_events <= DIES_TRACE_STATIC_MAX_EVENTS, else
+ * DIES_EINVAL with a message that names the limit (nothing is launched); split a longer id range over several calls.
+ *
+ * Set-up: the first call on each GPU looks up the array's device address (once per device, under a lock, with the
+ * calling thread's current device, which must be the one the handle's workspace lives on).  Make that first call
+ * before any stream capture begins.
+ *
+ * Sharing: all calls, of all handles and threads, use the same array on a GPU.  It keeps the contents of the last
+ * call; this entry point clears the part it uses before launching.  Two calls whose device work overlaps (two threads,
+ * two handles) race on it and corrupt each other's lists: serialise them.  The call synchronises the device before it
+ * returns, so calls made one after the other from one thread never overlap.
+ *
+ * No cudaMalloc, cudaFree or allocating library routine is called. */
+#define DIES_TRACE_STATIC_MAX_PACKAGES 4096
+#define DIES_TRACE_STATIC_MAX_EVENTS   65536
+int dies_trace_packages_static(dies_model*, int model_index, uint64_t first_id, int count, uint64_t n_total,
+                               uint64_t seed, const dies_run_opts* opts, int32_t* events, int max_events,
+                               int32_t* n_events);
 /* The device Philox and uniform of the RNG contract: out[4*j..] = words of block `block` of package first_id+j. */
 int dies_test_philox(uint64_t seed, uint64_t first_id, uint32_t block, uint32_t model_index, int n,
                      uint32_t* words, float* uniforms);

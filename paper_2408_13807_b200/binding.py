@@ -24,7 +24,10 @@ EXPORTS = ("dies_workspace_bytes", "dies_create_model", "dies_create_batch", "di
            "dies_set_sources_batch", "dies_run", "dies_run_batch", "dies_get_temperature", "dies_get_escape_spectrum",
            "dies_set_fixed_temperature", "dies_get_absorbed", "dies_get_counters", "dies_trace_packages",
            "dies_trace_package", "dies_test_philox", "dies_get_tables", "dies_destroy", "dies_last_error",
-           "dies_device_info", "dies_bench_atomics", "dies_seek", "dies_set_tuning", "dies_get_tuning", "dies_set_model_offset")
+           "dies_device_info", "dies_bench_atomics", "dies_seek", "dies_set_tuning", "dies_get_tuning", "dies_set_model_offset",
+           "dies_trace_packages_static")
+# limits of dies_trace_packages_static (include/dies.h)
+DIES_TRACE_STATIC_MAX_PACKAGES, DIES_TRACE_STATIC_MAX_EVENTS = 4096, 65536
 
 
 class DiesError(RuntimeError):
@@ -77,6 +80,7 @@ def lib():
     L.dies_get_counters.argtypes = [vp, C.POINTER(u64), C.c_int]
     L.dies_trace_packages.argtypes = [vp, C.c_int, u64, C.c_int, u64, u64, C.POINTER(dies_run_opts), i32p, C.c_int, i32p]
     L.dies_trace_package.argtypes = [vp, u64, u64, u64, C.POINTER(dies_run_opts), i32p, C.c_int, i32p]
+    L.dies_trace_packages_static.argtypes = L.dies_trace_packages.argtypes
     L.dies_test_philox.argtypes = [u64, u64, C.c_uint32, C.c_uint32, C.c_int, C.POINTER(C.c_uint32),
                                    C.POINTER(C.c_float)]
     L.dies_get_tables.argtypes = [vp, _dp, C.POINTER(C.c_float)]
@@ -277,6 +281,22 @@ class Model:
         i32p = C.POINTER(C.c_int32)
         _chk(lib().dies_trace_packages(self._h, model_index, int(first_id), count, int(n_total), int(seed),
                                        C.byref(o), ev.ctypes.data_as(i32p), max_events, n.ctypes.data_as(i32p)))
+        return ev, n
+
+    def dies_trace_packages_static(self, first_id, count, n_total, seed=1, model_index=0, max_events=256, **opts):
+        """dies_trace_packages without device allocation: the scratch is a fixed array inside libdies.so.  For processes
+        whose framework allocator already owns the GPU's memory, or that cannot afford the device-wide stall of
+        cudaMalloc / cudaFree.  count <= DIES_TRACE_STATIC_MAX_PACKAGES and count * max_events <=
+        DIES_TRACE_STATIC_MAX_EVENTS, else DiesError(DIES_EINVAL).  Calls share the array: do not overlap them."""
+        opts.setdefault("mode", DIES_MODE_FIXED_T)
+        o = _opts(**opts)
+        # max(..., 1): a rejected size must reach the library's own check, not fail in numpy
+        ev = np.zeros((max(count, 1), max(max_events, 1), 4), dtype=np.int32)
+        n = np.zeros(max(count, 1), dtype=np.int32)
+        i32p = C.POINTER(C.c_int32)
+        _chk(lib().dies_trace_packages_static(self._h, model_index, int(first_id), count, int(n_total), int(seed),
+                                              C.byref(o), ev.ctypes.data_as(i32p), max_events,
+                                              n.ctypes.data_as(i32p)))
         return ev, n
 
     def dies_trace_package(self, package_id, n_total, seed=1, max_events=4096, **opts):

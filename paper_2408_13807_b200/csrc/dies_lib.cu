@@ -1140,6 +1140,122 @@ extern "C" int dies_trace_package(dies_model* m, uint64_t package_id, uint64_t n
     return dies_trace_packages(m, 0, package_id, 1, n_total, seed, opts, events, max_events, n_events);
 }
 
+// ------------------------------------------------------------------ trace without any device allocation
+// dies_trace_packages needs device scratch beyond the model's workspace: the event lists (count x max_events x 16
+// bytes), the per-package event counts and the 64-bit counter the traced package indices are handed out from.  It
+// gets them from cudaMalloc / cudaFree.  dies_trace_packages_static keeps the same scratch in the array below, which
+// is part of the library image: every GPU that loads libdies.so holds these ~1.02 MiB until the process exits, and
+// nothing is allocated or freed at call time.
+//
+// g_trace_scratch is a DEVICE symbol.  In host code its name is only a host-side stand-in and not a device address, so
+// the host never passes `g_trace_scratch` itself to a kernel: trace_scratch() asks the runtime for the address once
+// per device, with that device current, and hands that pointer on.
+constexpr size_t kTraceStaticEvBytes = (size_t)DIES_TRACE_STATIC_MAX_EVENTS * 16;          // event quadruples
+constexpr size_t kTraceStaticNBytes = (size_t)DIES_TRACE_STATIC_MAX_PACKAGES * 4;          // n_events
+constexpr size_t kTraceStaticBytes = kTraceStaticEvBytes + kTraceStaticNBytes + 256;       // + the package counter
+static __device__ __align__(256) unsigned char g_trace_scratch[kTraceStaticBytes];
+
+static int trace_scratch(unsigned char** out)
+{
+    static std::mutex mu;
+    static unsigned char* addr[64] = {};          // per device ordinal; the address differs from GPU to GPU
+    int dev = 0;
+    CUDA_TRY(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= 64) return fail(DIES_ECUDA, "device ordinal %d beyond the 64 this entry point keeps scratch addresses for", dev);
+    std::lock_guard<std::mutex> lock(mu);
+    if (!addr[dev]) {
+        void* p = nullptr;
+        CUDA_TRY(cudaGetSymbolAddress(&p, g_trace_scratch));
+        if (!p) return fail(DIES_ECUDA, "cudaGetSymbolAddress gave no address for the trace scratch");
+        addr[dev] = static_cast<unsigned char*>(p);
+    }
+    *out = addr[dev];
+    return DIES_OK;
+}
+
+extern "C" int dies_trace_packages_static(dies_model* m, int model_index, uint64_t first_id, int count, uint64_t n_total,
+                                          uint64_t seed, const dies_run_opts* opts, int32_t* events, int max_events,
+                                          int32_t* n_events)
+{
+    if (!m || !events || !n_events) return fail(DIES_EINVAL, "NULL argument");
+    if (!m->sources_set) return fail(DIES_ESTATE, "trace before dies_set_sources");
+    if (model_index < 0 || model_index >= m->M || count < 1 || max_events < 1 || n_total == 0)
+        return fail(DIES_EINVAL, "bad trace arguments");
+    if (count > DIES_TRACE_STATIC_MAX_PACKAGES)
+        return fail(DIES_EINVAL, "dies_trace_packages_static: count %d exceeds DIES_TRACE_STATIC_MAX_PACKAGES = %d "
+                    "(split the id range, or use dies_trace_packages, which allocates)", count, DIES_TRACE_STATIC_MAX_PACKAGES);
+    if ((unsigned long long)count * (unsigned long long)max_events > (unsigned long long)DIES_TRACE_STATIC_MAX_EVENTS)
+        return fail(DIES_EINVAL, "dies_trace_packages_static: count * max_events = %llu exceeds DIES_TRACE_STATIC_MAX_EVENTS = %d "
+                    "(split the id range, or use dies_trace_packages, which allocates)",
+                    (unsigned long long)count * (unsigned long long)max_events, DIES_TRACE_STATIC_MAX_EVENTS);
+    RunParams R;
+    int mode, accumulate, shift; uint64_t nt;
+    dies_run_opts o = {0.5, 0, DIES_MODE_FIXED_T, 0, 24, n_total, 1.0, 0.0, 1.0, 0.0, 0.0, 0, 0};
+    if (opts) o = *opts;
+    o.n_total = n_total;
+    int rc = fill_run_params(m, 1, seed, &o, &R, &mode, &accumulate, &shift, &nt);
+    if (rc) return rc;
+    if (mode == DIES_MODE_IRE && (!m->ran || nt != m->n_total || shift != m->shift))
+        return fail(DIES_ESTATE, "IRE-mode trace replays against the tallies of a run with the same n_total");
+    unsigned char* scratch = nullptr;             // device address of g_trace_scratch on the current GPU
+    rc = trace_scratch(&scratch);
+    if (rc) return rc;
+    CUDA_TRY(cudaStreamSynchronize(m->stream));
+    if (!m->ran) {
+        // energy scales are set per run; a trace before any run sets them for n_total
+        k_prepare_run<<<(m->M * (m->K > m->ldS ? m->K : m->ldS) + 255) / 256, 256>>>(
+            m->D, wsp<double>(m, m->L.mass), wsp<double>(m, m->L.Lsrc), wsp<double>(m, m->L.epsref),
+            wsp<double>(m, m->L.cscale), wsp<double>(m, m->L.eunit), wsp<ModelParams>(m, m->L.mp), (double)nt,
+            (double)R.qscale, 1);
+        m->launches += 1;
+    }
+    R.n_run = nt; R.id_base = 0;
+    R.uniform_q = 0;                                       // the trace kernels keep the quantum per package
+    R.slots = fly_slots(false);
+    R.chunk = 32;
+    // The array still holds what the last call (of any handle, any thread) left in it.  The event counts and the
+    // package counter must start at zero; the event lists of this call are cleared too, so that entries past a
+    // package's n_events read as zeros rather than as another call's events.
+    int32_t* const d_ev = reinterpret_cast<int32_t*>(scratch);
+    int32_t* const d_n = reinterpret_cast<int32_t*>(scratch + kTraceStaticEvBytes);
+    unsigned long long* const d_counter = reinterpret_cast<unsigned long long*>(scratch + kTraceStaticEvBytes + kTraceStaticNBytes);
+    CUDA_TRY(cudaMemsetAsync(d_ev, 0, (size_t)count * max_events * 16, 0));
+    CUDA_TRY(cudaMemsetAsync(d_n, 0, kTraceStaticNBytes + 8, 0));
+    TraceParams tp = {model_index, first_id, count, d_ev, max_events, d_n, d_counter};
+    cudaError_t ge = cudaSuccess;
+    if (R.weighted) {
+        int grid = (count + kBlock - 1) / kBlock;
+        if (grid > 4 * m->n_sms) grid = 4 * m->n_sms;
+        const int nw = m->M * (2 * m->ldS + 2);
+        k_build_wshells<<<(nw + 127) / 128, 128>>>(wsp<double>(m, m->L.rb), wsp<double>(m, m->L.rho), m->N, m->M, m->kref,
+                                                  R.k_A, R.k_A_dilute, wsp<float4>(m, m->L.stabW));
+        m->launches += 1;
+        const size_t sm = tracker_smem(m->N, m->K, m->nT, R.pool, true, true, true);
+        ge = grant_smem(mode == DIES_MODE_IRE ? KF_TRK0T : KF_TRK1T, sm);
+        if (ge == cudaSuccess) {
+            if (mode == DIES_MODE_IRE) dies_track<0, true, true><<<grid, kBlock, sm>>>(m->D, R, tp);
+            else dies_track<1, true, true><<<grid, kBlock, sm>>>(m->D, R, tp);
+        }
+    } else {
+        int grid = (count + kFlyBlock - 1) / kFlyBlock;
+        if (grid > m->grid_max) grid = m->grid_max;
+        int logc = 0;
+        if (!fly_shape(m->N, m->K, m->nT, R.slots, true, true, &logc, &R.slots))
+            return fail(DIES_ECUDA, "tracker does not fit on an SM");
+        const FlyPlan fp = plan_fly(m->K, m->nT, m->ldS, m->D.ldT, R.slots, true, true, logc);
+        const int kf = fly_kernel(mode, true, logc);
+        ge = grant_smem(kf, fp.total);
+        if (ge == cudaSuccess) launch_fly(kf, grid, fp.total, 0, m->D, R, tp, fp);
+    }
+    if (ge != cudaSuccess) return fail(DIES_ECUDA, "trace: %s", cudaGetErrorString(ge));
+    m->launches += 1;
+    cudaError_t e = cudaDeviceSynchronize();
+    if (e == cudaSuccess) e = cudaMemcpy(events, d_ev, (size_t)count * max_events * 16, cudaMemcpyDeviceToHost);
+    if (e == cudaSuccess) e = cudaMemcpy(n_events, d_n, (size_t)count * 4, cudaMemcpyDeviceToHost);
+    if (e != cudaSuccess) return fail(DIES_ECUDA, "trace: %s", cudaGetErrorString(e));
+    return DIES_OK;
+}
+
 extern "C" int dies_test_philox(uint64_t seed, uint64_t first_id, uint32_t block, uint32_t model_index, int n,
                                 uint32_t* words, float* uniforms)
 {
