@@ -7,7 +7,11 @@
 // W (1 - e^{-kappa_A rho l}) of its energy in the cell (L37: "updates made to every cell along the photon path") and
 // keeps the rest; scatterings are discrete events at tau_S = -ln u (Eq. 1).  Energies are 64-bit fixed-point
 // integers as in the IRE trackers (R13): a package starts with its quantum and hands it out in integer pieces, so
-// injected = absorbed + escaped + terminated holds exactly.  The tallies of a block are privatised in shared memory.
+// injected = absorbed + escaped + terminated holds exactly.  The pieces are cut with a carried remainder that starts
+// at a uniform random offset per package (a spare word of its launch block): the deposit of a step is
+// floor(acc + q f) with acc the fraction left over by the steps before, so the expectation of every deposit is the
+// exact q f however small it is (thin cells, weak sources, attenuated packages: rounding each step to the nearest
+// integer would leave nothing there and bias T low).  The launch quantum of a package is cut the same way.  The tallies of a block are privatised in shared memory.
 // Lanes that finished their package wait until a quarter of the warp is idle, then the idle lanes launch new packages
 // together.
 #pragma once
@@ -108,7 +112,7 @@ __global__ void __launch_bounds__(kBlock, kMinBlocks) dies_tmc(DeviceModel D, Ru
         bool active = false;
         unsigned long long id = 0;
         int k = 0;
-        float kapA = 0.f, kapS = 0.f, g = 0.f, a = 0.f, b2 = 0.f, tauS = 0.f, w = 0.f;
+        float kapA = 0.f, kapS = 0.f, g = 0.f, a = 0.f, b2 = 0.f, tauS = 0.f, w = 0.f, acc = 0.f;
         unsigned pa = tab0, qrem = 0, blk = 0;
         unsigned long long ch_next = 0, ch_end = 0;
         bool exhausted = false;
@@ -144,7 +148,7 @@ __global__ void __launch_bounds__(kBlock, kMinBlocks) dies_tmc(DeviceModel D, Ru
                     uint32_t xw[4];
                     philox4x32_10_rk(R.rk, (uint32_t)id, (uint32_t)(id >> 32), 0u, (uint32_t)m + R.model0, xw);
                     blk = 1u;
-                    float re, re2, mu, qs;
+                    float re, re2, mu, qs, uq;
                     int j;
                     if (which < n_src) {
                         // ---- a package of a source, as in the IRE method
@@ -157,6 +161,9 @@ __global__ void __launch_bounds__(kBlock, kMinBlocks) dies_tmc(DeviceModel D, Ru
                             mu = 1.f; re = mp.r0hat; re2 = re * re; j = mp.cav;          // L65, R9
                         }
                         tauS = neg_log(uniform24(xw[2]));
+                        // the spare word of the block, halved: offsets of the quantum and of the deposits
+                        uq = ((float)(xw[3] >> 16) + 0.5f) * (1.f / 65536.f);
+                        acc = ((float)(xw[3] & 0xffffu) + 0.5f) * (1.f / 65536.f);
                         qs = point ? mp.qs_point : mp.qs_ext;
                     } else {
                         // ---- a dust package: cell by luminosity, radius uniform in its volume (L251), isotropic,
@@ -178,13 +185,18 @@ __global__ void __launch_bounds__(kBlock, kMinBlocks) dies_tmc(DeviceModel D, Ru
                         if (lower) k = bisect_cdf(Tm.G + (size_t)(t >= nT ? nT - 1 : t - 1) * K, K, u0);
                         else k = sample_cdf(D.F + (size_t)t * K, D.guideF + (size_t)t * kGuide, u0);
                         tauS = neg_log(uniform24(xv[1]));
+                        uq = uniform24(xv[2]);                                           // spare words: offsets of the
+                        acc = uniform24(xv[3]);                                          // quantum and of the deposits
                         qs = qs_dust;
                     }
                     const float4 bt = s_bin[k];
                     kapA = bt.x < 3.0e38f ? 1.f / bt.x : 0.f;
                     kapS = bt.y < 3.0e38f ? 1.f / bt.y : 0.f;
                     g = bt.z;
-                    qrem = (unsigned)__float2ll_rn(qs * R.qscale);
+                    // quantum of the package: floor(qs 2^S + offset), so that a weak source (qs << 1, a quantum of tens
+                    // or thousands of units) injects its luminosity without the bias of one fixed rounding; the
+                    // reference source (qs = 1) keeps exactly 2^S
+                    qrem = __float2uint_rz(fmaf(qs, R.qscale, uq));
                     w = 1.f;
                     lc_inj += qrem;
                     lc_pkg++;
@@ -216,7 +228,10 @@ __global__ void __launch_bounds__(kBlock, kMinBlocks) dies_tmc(DeviceModel D, Ru
                 // L37: continuous absorption along the step
                 const float dtA = kapA * dc * f;
                 const float frac = -expm1f(-dtA);
-                const unsigned dq = min(qrem, (unsigned)__float2uint_rn((float)qrem * frac));
+                // integer piece with the carried remainder (unbiased for pieces far below one unit, see the header)
+                const float x = fmaf((float)qrem, frac, acc);
+                const unsigned dq = min(qrem, __float2uint_rz(x));
+                acc = x - (float)dq;
                 const int c = (int)(pa - tab0) / 8;
                 const int j = c <= 0 ? -c : c - 1;
                 if (dq) smem_add64(&s_A[j], &s_A[ldS + j], (unsigned long long)dq);

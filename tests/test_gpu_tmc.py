@@ -103,3 +103,70 @@ def test_tmc_batch_and_errors(orc):
             m.dies_run(1000, mode=dies.DIES_MODE_TMC, **kw)
         assert e.value.code == dies.DIES_EINVAL
     m.close()
+
+
+@pytest.mark.parametrize("tau,bar", [(1e-6, 3e-3), (1e-8, 2e-2)])
+def test_tmc_thin_sphere_deposits_are_unbiased(orc, tau, bar):
+    """A nearly transparent sphere: a package leaves far less than one fixed-point unit per step (about 5 units at
+    tau = 1e-6, 0.05 at 1e-8, of a quantum of 2^24).  The pieces are cut with a carried remainder that starts at a
+    random offset per package, so their sum over many packages is the continuous absorption of the oracle up to the
+    noise of that cut (bars: some five standard deviations of it); rounding every step to the nearest integer would
+    tally exactly nothing at 1e-8."""
+    p, n = toy_problem(n_shells=5, tau=tau), 1_000_000
+    m = dies.Model(p)
+    o = orc.Oracle(p)
+    m.dies_run(n, seed=6, mode=dies.DIES_MODE_TMC)
+    o.tmc_run(n, seed=6)
+    raw, unit, energy = m.dies_get_absorbed()
+    c = m.dies_get_counters()
+    assert _identity(c, raw), c
+    assert np.all(raw > 0)
+    assert np.max(np.abs(energy / o.absorbed - 1)) < bar, energy / o.absorbed
+    assert abs(energy.sum() / o.absorbed.sum() - 1) < bar / 2
+    assert c["crossings"] == o.counters["crossings"] and c["terminated"] == 0
+    m.close()
+
+
+def test_tmc_weak_second_source(orc):
+    """Two sources with a luminosity ratio of 1e4: the external field shines in the transparent bin (never absorbed),
+    the point source, 1e-4 of it, in the absorbing bin of a thin sphere (tau = 1e-3).  Its packages carry 1e-4 of the
+    reference quantum (about 1678 units) and leave a third of a unit per step: every tally comes from pieces below one
+    unit of the weak source."""
+    p = toy_problem(n_shells=5, tau=1e-3)
+    L_ext = 4.0 * np.pi ** 2                       # 4 pi R^2 * pi * sum_k J_k with R = 1, J = (1, 0)
+    p.ext_bin_intensity = np.array([1.0, 0.0])
+    p.L_point, p.point_bin_weights = 1e-4 * L_ext, np.array([0.0, 1.0])
+    n = 1_000_000
+    m = dies.Model(p)
+    o = orc.Oracle(p)
+    m.dies_run(n, seed=8, mode=dies.DIES_MODE_TMC)
+    o.tmc_run(n, seed=8)
+    raw, unit, energy = m.dies_get_absorbed()
+    c = m.dies_get_counters()
+    assert c["packages"] == 2 * n == o.counters["packages"]
+    assert _identity(c, raw), c
+    assert np.all(raw > 0)
+    assert np.max(np.abs(energy / o.absorbed - 1)) < 1e-2, energy / o.absorbed
+    assert abs(energy.sum() / o.absorbed.sum() - 1) < 4e-3
+    esc = m.dies_get_escape_spectrum()
+    np.testing.assert_allclose(esc, o.escaped, rtol=1e-4)
+    m.close()
+
+
+def test_tmc_weight_guard_fires(orc):
+    """PAPER.md L119 in the TMC: in a very thick, purely absorbing sphere nearly every package falls below 1e-10 of
+    its launch weight before it gets out; both sides must end those packages (terminated > 0), at the same count up to
+    fp32 / fp64 flips of the comparison, and the energy bookkeeping stays exact."""
+    p, n = toy_problem(n_shells=5, tau=400.0), 100_000
+    m = dies.Model(p)
+    o = orc.Oracle(p)
+    m.dies_run(n, seed=3, mode=dies.DIES_MODE_TMC)
+    o.tmc_run(n, seed=3)
+    raw, unit, energy = m.dies_get_absorbed()
+    c = m.dies_get_counters()
+    assert o.counters["terminated"] > 0.5 * n and c["terminated"] > 0.5 * n
+    assert abs(c["terminated"] - o.counters["terminated"]) <= 2e-4 * n + 3
+    assert c["terminated"] + c["escaped"] == n
+    assert _identity(c, raw), c
+    assert np.all(np.abs(energy - o.absorbed) <= np.maximum(1e-4 * o.absorbed, 3 * o.sums["injected"] / n))
+    m.close()
