@@ -55,7 +55,10 @@ enum { DIES_MODE_IRE = 0, DIES_MODE_FIXED_T = 1,
         * PREVIOUS run of the handle (whatever its mode; nothing before the first run), with the cell's emission spectrum.
         * Calling dies_run with this mode repeatedly is the TMC iteration; dies_get_temperature after each run gives the
         * temperatures to watch for convergence (L31).  Plain runs only: k_bg = 0.5, no ffi, no weighting, no accumulate,
-        * fixed_shift <= 24. */
+        * fixed_shift <= 24 (DIES_EINVAL otherwise; a rejected call leaves the handle, a pending dies_seek included, as
+        * it was).  The tallies of a TMC run are in an energy unit that includes the dust luminosity: a later run in
+        * another mode cannot accumulate onto them and an IRE-mode trace cannot replay against them (DIES_ESTATE);
+        * traces themselves are IRE or fixed-temperature only (DIES_EINVAL for this mode). */
        DIES_MODE_TMC = 2 };
 
 /* event types of dies_trace_* (quadruples: type, shell, freq_bin, crossings so far) */

@@ -102,6 +102,7 @@ struct dies_model {
     unsigned long long done, n_total;     // packages per source already followed / planned
     unsigned long long next_first;        // dies_seek: first package id (per source) of the next fresh run
     int shift;
+    int last_mode;                        // mode of the last run (its tallies are in that mode's energy unit)
     uint32_t model0;                      // dies_set_model_offset
     int visit_auto;                       // crossing blocks per crossing phase, from the counters of the last read-out
     cudaStream_t stream;
@@ -648,6 +649,7 @@ extern "C" int dies_create_batch(int n_models, int n_shells, const double* r_bou
     m->N = N; m->K = K; m->nT = nT; m->M = M; m->ldS = N + 1;
     m->L = L; m->ws = (unsigned char*)workspace_dev;
     m->sources_set = m->fixed_set = m->ran = m->finalized = false;
+    m->last_mode = DIES_MODE_IRE;
     m->done = m->n_total = 0; m->next_first = 0; m->shift = 24; m->model0 = 0; m->visit_auto = 8; m->stream = 0; m->launches = 0;
     m->L_point.assign(M, 0.0); m->has_ext.assign(M, 0); m->has_point.assign(M, 0);
     m->smem_bytes = smem; m->smem_trace_bytes = smem_trace; m->pool = pool; m->kref = kref;
@@ -781,6 +783,7 @@ extern "C" int dies_set_fixed_temperature(dies_model* m, const double* T, int n)
 
 // ------------------------------------------------------------------ run
 
+constexpr unsigned kTmcSmemMax = 200 * 1024;     // dynamic shared memory dies_tmc is allowed
 static int fill_run_params(dies_model* m, uint64_t n_packages, uint64_t seed, const dies_run_opts* o, RunParams* R,
                            int* mode, int* accumulate, int* shift, uint64_t* n_total)
 {
@@ -801,6 +804,12 @@ static int fill_run_params(dies_model* m, uint64_t n_packages, uint64_t seed, co
     if (d.fixed_shift < 1 || d.fixed_shift > 30) return fail(DIES_EINVAL, "fixed_shift must be in [1, 30]");
     if (d.n_total == 0) d.n_total = n_packages;
     if (d.mode == DIES_MODE_FIXED_T && !m->fixed_set) return fail(DIES_ESTATE, "fixed-T mode needs dies_set_fixed_temperature");
+    if (d.mode == DIES_MODE_TMC) {
+        // (checked here, before dies_run writes to the handle: a rejected call must leave dies_seek, n_total and the
+        // stream of the handle as they were)
+        if (d.fixed_shift > 24) return fail(DIES_EINVAL, "TMC mode keeps package quanta in 32 bits: fixed_shift <= 24");
+        if (plan_tmc(m->K, m->ldS, m->D.ldT).total > kTmcSmemMax) return fail(DIES_EINVAL, "tables do not fit in shared memory");
+    }
     *mode = d.mode; *accumulate = d.accumulate; *shift = d.fixed_shift; *n_total = d.n_total;
     int two = 0;
     for (int i = 0; i < m->M; i++) two |= (m->has_ext[i] && m->has_point[i]);
@@ -836,6 +845,8 @@ extern "C" int dies_run(dies_model* m, uint64_t n_packages, uint64_t seed, const
     if (rc) return rc;
     if (accumulate && m->ran) {
         if (n_total != m->n_total || shift != m->shift) return fail(DIES_ESTATE, "accumulate needs the same n_total and fixed_shift");
+        // the raw unit of a TMC run includes the dust luminosity: its tallies cannot be continued by another mode
+        if (m->last_mode == DIES_MODE_TMC) return fail(DIES_ESTATE, "accumulate after a TMC run: the tallies are in the TMC energy unit");
     } else {
         accumulate = 0;
         m->done = m->next_first;
@@ -850,14 +861,12 @@ extern "C" int dies_run(dies_model* m, uint64_t n_packages, uint64_t seed, const
 
     if (mode == DIES_MODE_TMC) {
         // one iteration of the traditional Monte Carlo (dies_tmc.cuh): the dust emits what the run before left in it
-        if (m->shift > 24) return fail(DIES_EINVAL, "TMC mode keeps package quanta in 32 bits: fixed_shift <= 24");
-        const TmcPlan tpn = plan_tmc(m->K, m->ldS, m->D.ldT);
+        const TmcPlan tpn = plan_tmc(m->K, m->ldS, m->D.ldT);      // (size and fixed_shift checked in fill_run_params)
         static std::mutex mu;
         {
             std::lock_guard<std::mutex> lock(mu);
-            CUDA_TRY(cudaFuncSetAttribute(dies_tmc, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
+            CUDA_TRY(cudaFuncSetAttribute(dies_tmc, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kTmcSmemMax));
         }
-        if (tpn.total > 200 * 1024) return fail(DIES_EINVAL, "tables do not fit in shared memory");
         int bps = 0;
         CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&bps, dies_tmc, kBlock, tpn.total));
         if (bps < 1) return fail(DIES_ECUDA, "tracker does not fit on an SM");
@@ -882,6 +891,7 @@ extern "C" int dies_run(dies_model* m, uint64_t n_packages, uint64_t seed, const
         CUDA_TRY(cudaGetLastError());
         m->done += n_packages;
         m->ran = true;
+        m->last_mode = DIES_MODE_TMC;
         m->finalized = false;
         return DIES_OK;
     }
@@ -936,6 +946,7 @@ extern "C" int dies_run(dies_model* m, uint64_t n_packages, uint64_t seed, const
     CUDA_TRY(cudaGetLastError());
     m->done += n_packages;
     m->ran = true;
+    m->last_mode = mode;
     m->finalized = false;
     return DIES_OK;
 }
@@ -1074,8 +1085,9 @@ extern "C" int dies_trace_packages(dies_model* m, int model_index, uint64_t firs
     o.n_total = n_total;
     int rc = fill_run_params(m, 1, seed, &o, &R, &mode, &accumulate, &shift, &nt);
     if (rc) return rc;
-    if (mode == DIES_MODE_IRE && (!m->ran || nt != m->n_total || shift != m->shift))
-        return fail(DIES_ESTATE, "IRE-mode trace replays against the tallies of a run with the same n_total");
+    if (mode == DIES_MODE_TMC) return fail(DIES_EINVAL, "traces replay IRE or fixed-temperature packages, not a TMC iteration");
+    if (mode == DIES_MODE_IRE && (!m->ran || nt != m->n_total || shift != m->shift || m->last_mode == DIES_MODE_TMC))
+        return fail(DIES_ESTATE, "IRE-mode trace replays against the tallies of an IRE or fixed-temperature run with the same n_total");
     CUDA_TRY(cudaStreamSynchronize(m->stream));
     if (!m->ran) {
         // energy scales are set per run; a trace before any run sets them for n_total
@@ -1195,8 +1207,9 @@ extern "C" int dies_trace_packages_static(dies_model* m, int model_index, uint64
     o.n_total = n_total;
     int rc = fill_run_params(m, 1, seed, &o, &R, &mode, &accumulate, &shift, &nt);
     if (rc) return rc;
-    if (mode == DIES_MODE_IRE && (!m->ran || nt != m->n_total || shift != m->shift))
-        return fail(DIES_ESTATE, "IRE-mode trace replays against the tallies of a run with the same n_total");
+    if (mode == DIES_MODE_TMC) return fail(DIES_EINVAL, "traces replay IRE or fixed-temperature packages, not a TMC iteration");
+    if (mode == DIES_MODE_IRE && (!m->ran || nt != m->n_total || shift != m->shift || m->last_mode == DIES_MODE_TMC))
+        return fail(DIES_ESTATE, "IRE-mode trace replays against the tallies of an IRE or fixed-temperature run with the same n_total");
     unsigned char* scratch = nullptr;             // device address of g_trace_scratch on the current GPU
     rc = trace_scratch(&scratch);
     if (rc) return rc;

@@ -102,6 +102,33 @@ def test_tmc_batch_and_errors(orc):
         with pytest.raises(dies.DiesError) as e:
             m.dies_run(1000, mode=dies.DIES_MODE_TMC, **kw)
         assert e.value.code == dies.DIES_EINVAL
+    # a rejected TMC call leaves the handle as it was: the pending dies_seek still applies to the next run
+    m.dies_set_fixed_temperature(np.full(m.N, 15.0))
+    m.dies_seek(5000)
+    with pytest.raises(dies.DiesError) as e:
+        m.dies_run(1000, mode=dies.DIES_MODE_TMC, fixed_shift=26)
+    assert e.value.code == dies.DIES_EINVAL
+    m.dies_run(1000, seed=9, mode=dies.DIES_MODE_FIXED_T, n_total=10_000)
+    ev_run = m.dies_get_absorbed()[0].copy()
+    m.dies_seek(5000)
+    m.dies_run(1000, seed=9, mode=dies.DIES_MODE_FIXED_T, n_total=10_000)
+    assert np.array_equal(ev_run, m.dies_get_absorbed()[0])
+    m.dies_run(1000, seed=9, mode=dies.DIES_MODE_FIXED_T, n_total=10_000)          # ids from 0: other packages
+    assert not np.array_equal(ev_run, m.dies_get_absorbed()[0])
+    # the tallies of a TMC run are in the TMC energy unit: no other mode continues them, no IRE trace replays on them
+    m.dies_run(10_000, seed=9, mode=dies.DIES_MODE_TMC)
+    for mode in (dies.DIES_MODE_IRE, dies.DIES_MODE_FIXED_T):
+        with pytest.raises(dies.DiesError) as e:
+            m.dies_run(1000, seed=9, mode=mode, accumulate=1, n_total=10_000)
+        assert e.value.code == dies.DIES_ESTATE
+    with pytest.raises(dies.DiesError) as e:
+        m.dies_trace_packages(0, 4, 10_000, mode=dies.DIES_MODE_IRE)
+    assert e.value.code == dies.DIES_ESTATE
+    for trace in (m.dies_trace_packages, m.dies_trace_packages_static):
+        with pytest.raises(dies.DiesError) as e:
+            trace(0, 4, 10_000, mode=dies.DIES_MODE_TMC)
+        assert e.value.code == dies.DIES_EINVAL
+    m.dies_run(1000, seed=9, mode=dies.DIES_MODE_IRE)                              # a fresh run in another mode is fine
     m.close()
 
 
