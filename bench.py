@@ -7,7 +7,8 @@ A "step" is one pass of the whole hot path over one batch of synthetic input: di
 heated sphere, 100 shells, 200 frequencies, 1e7 packages, full IRE).  `value` is timed with CUDA events around
 dies_run with the model resident in HBM; `e2e` times create_model + set_sources + run + get_temperature +
 get_escape_spectrum through the C ABI with host buffers.  Full IRE on one model does not shard (DESIGN.md,
-"Multi-GPU": replicas only): with --gpus N every rank runs an independent replica (its own seed).
+"Multi-GPU": replicas only): with --gpus N every rank runs an independent replica (its own seed).  `--gpus N` with
+N > 1 outside torchrun starts the N ranks itself (torch.distributed.run on 127.0.0.1); under torchrun it is one rank.
 --impl reference times the CPU oracle (oracle/, test infrastructure) on a bounded sample of the same workload.
 """
 from __future__ import annotations
@@ -406,7 +407,18 @@ def run_noise_study(args):
                           reference_packages=10**9, data="synthetic", rows=rows)))
 
 
-def main():
+def spawn_command(n_gpus, argv):
+    """The launch line of N ranks on this node (the one the driver uses for N > 1), on a free local port."""
+    import socket
+
+    with socket.socket() as sk:
+        sk.bind(("127.0.0.1", 0))
+        port = sk.getsockname()[1]
+    return [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={n_gpus}",
+            "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__), *argv]
+
+
+def main(argv=None):
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=500)
@@ -423,7 +435,10 @@ def main():
     ap.add_argument("--tune", default="", help="launch tuning for dies_set_tuning, e.g. visit=2,slots_uniform=5 (include/dies.h: dies_tuning)")
     ap.add_argument("--cpu-all-cores", action="store_true", help="also time the oracle on all host cores (one process each)")
     ap.add_argument("--noise-study", action="store_true", help="configs 2, 3, 4: sigma_T and systematic error per radius decile over 8 seeds vs packages")
-    args = ap.parse_args()
+    args = ap.parse_args(argv)
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ and args.impl == "ours" and not args.noise_study:
+        # `python bench.py --gpus N` by itself: start the N ranks (one process per GPU) and let rank 0 print the line
+        sys.exit(subprocess.call(spawn_command(args.gpus, sys.argv[1:] if argv is None else list(argv))))
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))

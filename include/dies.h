@@ -228,7 +228,11 @@ typedef struct {
     int32_t slots;          /* dies_fly: the same with per-package quanta (k_bg, FFI, two sources), 1..8 (4)         */
     int32_t visit;          /* dies_fly: crossing blocks between two event phases, 1..64 (default: chosen per model,
                                2..8, so that a crossing phase lasts about two mean flights as counted by the model's
-                               last read-out; 8 before the first read-out)                                           */
+                               last read-out; 8 before the first read-out).  Because the automatic value follows the
+                               read-outs, the ORDER in which a full-IRE run makes its absorptions -- and so its result,
+                               within the Monte Carlo noise -- depends on whether a getter was called between two runs
+                               of the handle.  Set visit explicitly for results that repeat bit for bit whatever the
+                               getter calls; fixed-temperature tallies never depend on it                            */
     int32_t min_ready;      /* dies_fly: partial event batches only while fewer packages are ready, 1..256 (32)      */
     int32_t chunk;          /* package ids a warp takes from the global counter at a time, 32..4096 (128)            */
     int32_t pkg_per_block;  /* grid sizing of small runs: packages per block, 32..2^20 (256)                         */

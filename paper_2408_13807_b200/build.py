@@ -9,7 +9,23 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libdies.so")
 SOURCES = [os.path.join(CSRC, "dies_lib.cu")]
-DEPS = SOURCES + [os.path.join(CSRC, "dies_tracker.cuh"), os.path.join(HERE, "..", "include", "dies.h")]
+INCLUDE = os.path.join(HERE, "..", "include")
+
+
+def deps() -> list[str]:
+    """Everything libdies.so is compiled from: every file under csrc/ and include/ (listed at call time, so that a
+    new header is a dependency without an edit here)."""
+    out = []
+    for d in (CSRC, INCLUDE):
+        out += [os.path.join(d, f) for f in sorted(os.listdir(d)) if f.endswith((".cu", ".cuh", ".h"))]
+    return out
+
+
+def stale() -> bool:
+    """True when libdies.so is missing or older than one of its sources."""
+    return not os.path.exists(LIB) or any(os.path.getmtime(LIB) < os.path.getmtime(d) for d in deps())
+
+
 NVCC_FLAGS = ["-O3", "-std=c++17", "-lineinfo", "-gencode", "arch=compute_100a,code=sm_100a", "-shared",
               "-Xcompiler", "-fPIC", "-Xptxas", "-v",
               # single-precision division and square root of the event arithmetic at 2 ulp (DESIGN.md R14b)
@@ -17,7 +33,7 @@ NVCC_FLAGS = ["-O3", "-std=c++17", "-lineinfo", "-gencode", "arch=compute_100a,c
 
 
 def build(force: bool = False, verbose: bool = False) -> str:
-    if not force and os.path.exists(LIB) and all(os.path.getmtime(LIB) >= os.path.getmtime(d) for d in DEPS):
+    if not force and not stale():
         return LIB
     nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
     cmd = [nvcc, *NVCC_FLAGS, "-o", LIB, *SOURCES]

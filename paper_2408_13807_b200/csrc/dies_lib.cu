@@ -514,7 +514,10 @@ static size_t fly_smem(int N, int K, int nT, int M, bool trace, bool with_q, int
 
 // Launch shape of dies_fly for a model: 16 interleaved copies of the shell table when they fit beside a pool of at
 // least 3 slots per lane, else one copy; the pool as deep as asked for, or as fits.
-constexpr size_t kFlySmemMax = 227 * 1024;
+// The 227 KiB a block may opt in to cover its static shared memory too (s_ticket, s_cnt: 112 bytes in every tracker),
+// so the plans get 227 KiB less a reserve for it; grant_smem checks that the reserve covers what the kernel declares.
+constexpr size_t kStaticSmemReserve = 256;
+constexpr size_t kFlySmemMax = 227 * 1024 - kStaticSmemReserve;
 static bool fly_shape(int N, int K, int nT, int want_slots, bool trace, bool with_q, int* logc, int* slots)
 {
     for (int lc = 4; lc >= 0; lc -= 4) {
@@ -576,6 +579,10 @@ static cudaError_t grant_smem(int which, size_t bytes)
     if (e != cudaSuccess) return e;
     std::lock_guard<std::mutex> lock(mu);
     if (dev >= 0 && dev < 64 && bytes <= granted[dev][which]) return cudaSuccess;
+    cudaFuncAttributes fa;
+    e = cudaFuncGetAttributes(&fa, kernel_fn(which));
+    if (e != cudaSuccess) return e;
+    if (fa.sharedSizeBytes > kStaticSmemReserve) return cudaErrorInvalidConfiguration;   // (a build-time slip, not a user error)
     e = cudaFuncSetAttribute(kernel_fn(which), cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
     if (e == cudaSuccess && dev >= 0 && dev < 64) granted[dev][which] = bytes;
     return e;

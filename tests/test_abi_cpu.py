@@ -112,3 +112,23 @@ def test_bench_constants_belong_to_the_kernel_sources():
     from paper_2408_13807_b200 import profile_parts
     assert bench.KERNEL_SHA256 == profile_parts.kernel_hash()
     assert set(bench.INSTR) == {"crossing", "scattering", "absorption", "package"}
+
+
+def test_build_sees_every_kernel_source(lib):
+    """build.build() must rebuild after an edit to ANY file the library is compiled from (the hot kernels live in
+    headers: a parity run against a stale libdies.so would be one edit away otherwise).  No compile here: a header's
+    modification time is moved past the library's and back."""
+    names = {os.path.basename(d) for d in build.deps()}
+    csrc = os.path.join(ROOT, "paper_2408_13807_b200", "csrc")
+    assert names >= {f for f in os.listdir(csrc) if f.endswith((".cu", ".cuh"))} | {"dies.h"}
+    assert not build.stale()
+    for name in ("dies_fly.cuh", "dies_tmc.cuh", "dies_tracker.cuh"):
+        path = os.path.join(csrc, name)
+        st = os.stat(path)
+        try:
+            newer = os.path.getmtime(build.LIB) + 10
+            os.utime(path, (newer, newer))
+            assert build.stale(), name
+        finally:
+            os.utime(path, ns=(st.st_atime_ns, st.st_mtime_ns))
+    assert not build.stale()

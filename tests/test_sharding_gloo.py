@@ -144,3 +144,32 @@ def test_batch_shards_reproduce_the_whole_batch(tmp_path):
     assert float(parts[0]["n_all"]) == N_MODELS * N_BATCH_PKG
     T = np.concatenate([q["T"] for q in parts])
     assert np.array_equal(T, _batch_T(orc, _batch(), 0))
+
+
+def test_bench_gpus_n_starts_its_own_ranks(monkeypatch):
+    """`python bench.py --gpus N` (the form the driver uses for N = 1, and a user for any N) must launch N ranks when
+    it is not already one of them; under torchrun (WORLD_SIZE set) it must not spawn again."""
+    import bench
+
+    calls = []
+    monkeypatch.setattr(bench.subprocess, "call", lambda cmd: calls.append(cmd) or 0)
+    monkeypatch.delenv("WORLD_SIZE", raising=False)
+    with pytest.raises(SystemExit) as e:
+        bench.main(["--gpus", "4", "--steps", "5", "--workload", "config5"])
+    assert e.value.code == 0 and len(calls) == 1
+    cmd = calls[0]
+    assert cmd[1:3] == ["-m", "torch.distributed.run"] and "--nproc-per-node=4" in cmd
+    assert cmd[cmd.index("--master-addr") + 1] == "127.0.0.1"
+    assert cmd[-6:] == ["--gpus", "4", "--steps", "5", "--workload", "config5"] and cmd[-7].endswith("bench.py")
+    # the reference arm never spawns (rank 0 alone times the oracle): it goes straight to run_reference
+    seen = []
+    monkeypatch.setattr(bench, "run_reference", lambda a, rank, world: seen.append((rank, world)))
+    bench.main(["--gpus", "4", "--impl", "reference"])
+    assert seen == [(0, 1)] and len(calls) == 1
+    # a rank of a running job does not spawn
+    monkeypatch.setenv("WORLD_SIZE", "4")
+    monkeypatch.setenv("RANK", "3")
+    ours = []
+    monkeypatch.setattr(bench, "run_ours", lambda a, rank, world, lr: ours.append((rank, world)))
+    bench.main(["--gpus", "4"])
+    assert ours == [(3, 4)] and len(calls) == 1
