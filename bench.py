@@ -33,7 +33,7 @@ from paper_2408_13807_b200 import sharding, synth  # noqa: E402
 # profiles/r2_cross_step.sass): crossing = SASS instructions of one crossing step on a live lane; scattering /
 # absorption / package = predicated-on thread-instructions of the unit's own code (+ its share of the code the two event
 # types have in common) per unit, from the ncu source page of this workload through
-# `python -m paper_2408_13807_b200.profile_parts`.  Stack handling, batch composition, slot load / store, block ends and
+# `python profile_parts.py`.  Stack handling, batch composition, slot load / store, block ends and
 # idle lanes are NOT work.  The constants belong to ONE version of the kernel sources: KERNEL_SHA256 is the hash they were
 # derived at, and a roofline is only printed while the sources still have it.
 INSTR = dict(crossing=8, scattering=174, absorption=345, package=260)
@@ -304,8 +304,8 @@ def run_ours(args, rank, world, local_rank):
             c1["absorptions"] * INSTR["absorption"] + c1["packages"] * INSTR["package"])
     achieved = work / (step_ms * 1e-3) / 1e12
     held = clocks.get("sm_mhz") or sm_max
-    from paper_2408_13807_b200 import profile_parts
-    stale = profile_parts.kernel_hash() != KERNEL_SHA256
+    from paper_2408_13807_b200 import build as dies_build
+    stale = dies_build.kernel_hash() != KERNEL_SHA256
     # the XU pipe executes the one square root of every crossing: 8 cycles per warp instruction and scheduler
     xu_peak = SM_COUNT * SCHEDULERS * LANES * sm_max * 1e6 / XU_CYCLES_PER_WARP_INSTR
     line = dict(metric="packages_per_s", value=value, unit="packages/s", n_gpus=world, steps=args.steps,
@@ -345,7 +345,7 @@ def run_ours(args, rank, world, local_rank):
         # the work-per-unit constants were derived from other kernel sources: no fraction is claimed
         line["roofline"] = dict(bound="alu", achieved=None, peak=peak, unit="Tinstr/s", frac=None, traffic=None,
                                 stale="kernel sources changed since INSTR was derived: run an ncu source page through "
-                                      "paper_2408_13807_b200.profile_parts and update INSTR and KERNEL_SHA256",
+                                      "profile_parts.py and update INSTR and KERNEL_SHA256",
                                 kernel_ms=step_ms)
     # ---- the oracle timed beside it on this box's host cores (rank 0, N = 1 only)
     if world == 1 and not args.no_cpu_baseline:

@@ -23,5 +23,26 @@ def build(force: bool = False) -> None:
         subprocess.check_call(cmd)
 
 
+SANITIZED = "libdies_oracle_san.so"
+
+
+def build_sanitized(force: bool = False) -> str:
+    """dies_oracle.c under AddressSanitizer + UndefinedBehaviorSanitizer (any finding aborts): the memory-safety
+    check of the checker itself.  A process loads it in place of libdies_oracle.so when
+    DIES_ORACLE_LIB names it and libasan is preloaded (tests/test_oracle_sanitized.py shows how)."""
+    out = os.path.join(HERE, SANITIZED)
+    src = os.path.join(HERE, "dies_oracle.c")
+    if force or not os.path.exists(out) or os.path.getmtime(out) < os.path.getmtime(src):
+        subprocess.check_call(["gcc", "-O1", "-g", "-fPIC", "-shared", "-Wall", "-Wextra", "-ffp-contract=off",
+                               "-fsanitize=address,undefined", "-fno-sanitize-recover=undefined",
+                               "-fno-omit-frame-pointer", "-o", out, src, "-lm"])
+    return out
+
+
+def asan_runtime() -> str:
+    """Path of gcc's libasan.so, to be preloaded into an interpreter that loads the sanitized library."""
+    return subprocess.check_output(["gcc", "-print-file-name=libasan.so"], text=True).strip()
+
+
 if __name__ == "__main__":
     build(force=True)

@@ -12,7 +12,9 @@ import numpy as np
 from . import build as _build
 
 _build.build()
-_lib = C.CDLL(os.path.join(os.path.dirname(os.path.abspath(__file__)), "libdies_oracle.so"))
+# DIES_ORACLE_LIB: another build of the same source (the sanitizer build of oracle/build.py) instead of the default
+_lib = C.CDLL(os.path.join(os.path.dirname(os.path.abspath(__file__)),
+                           os.environ.get("DIES_ORACLE_LIB", "libdies_oracle.so")))
 
 _dp = C.POINTER(C.c_double)
 _u64 = C.c_uint64

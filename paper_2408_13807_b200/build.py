@@ -1,6 +1,7 @@
 """Build libdies.so (the C-ABI library of include/dies.h) in-tree with nvcc for sm_100a."""
 from __future__ import annotations
 
+import hashlib
 import os
 import subprocess
 import sys
@@ -19,6 +20,19 @@ def deps() -> list[str]:
     for d in (CSRC, INCLUDE):
         out += [os.path.join(d, f) for f in sorted(os.listdir(d)) if f.endswith((".cu", ".cuh", ".h"))]
     return out
+
+
+# the tracker sources bench.py's work-per-unit constants belong to (bench.KERNEL_SHA256)
+KERNEL_SOURCES = ("dies_fly.cuh", "dies_tracker.cuh")
+
+
+def kernel_hash() -> str:
+    """SHA-256 of the tracker sources: bench.py prints a roofline fraction only while it equals the hash its
+    constants were derived at."""
+    h = hashlib.sha256()
+    for name in KERNEL_SOURCES:
+        h.update(open(os.path.join(CSRC, name), "rb").read())
+    return h.hexdigest()
 
 
 def stale() -> bool:

@@ -1,7 +1,7 @@
 """Per-part instruction table of dies_fly from an ncu source page, and the work-per-unit constants of bench.py.
 
     ncu -i prof.ncu-rep --page source --csv --print-source cuda,sass > source.csv
-    python -m paper_2408_13807_b200.profile_parts source.csv --counts crossings scatterings absorptions packages
+    python profile_parts.py source.csv --counts crossings scatterings absorptions packages
 
 The kernel source is cut into parts at anchor comments of csrc/dies_fly.cuh (found by their text in the file, which
 must be the profiled one, so the table does not depend on line numbers).  Every SASS instruction belongs to the part of the nearest preceding instruction (in
@@ -18,12 +18,13 @@ from __future__ import annotations
 
 import argparse
 import csv
-import hashlib
 import os
 import sys
 
-HERE = os.path.dirname(os.path.abspath(__file__))
-KERNEL_SOURCES = ("csrc/dies_fly.cuh", "csrc/dies_tracker.cuh")
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+from paper_2408_13807_b200.build import CSRC as HERE, KERNEL_SOURCES, kernel_hash  # noqa: E402  (the hash guard lives with the build)
 
 # (part, anchor text that starts it), in source order
 ANCHORS = [
@@ -44,14 +45,6 @@ SUB = [
     ("ev_abs", "int row;", "blk = b + 1u;", 2),          # rows of the table, extra Philox block, draw
     ("ev_sca", "// ---- scattering with the HG phase function", "record<TRACE>(tp, pkg, n_ev, isabs", 0),
 ]
-
-
-def kernel_hash() -> str:
-    """SHA-256 of the kernel sources the constants of bench.py were derived from."""
-    h = hashlib.sha256()
-    for rel in KERNEL_SOURCES:
-        h.update(open(os.path.join(HERE, rel), "rb").read())
-    return h.hexdigest()
 
 
 def _num(x: str) -> float:

@@ -109,8 +109,7 @@ def test_bench_constants_belong_to_the_kernel_sources():
     sources; bench.py prints a roofline fraction only while the sources still hash to KERNEL_SHA256.  This test keeps the
     two from drifting apart unnoticed: after a kernel edit, re-profile, run profile_parts and update both."""
     import bench
-    from paper_2408_13807_b200 import profile_parts
-    assert bench.KERNEL_SHA256 == profile_parts.kernel_hash()
+    assert bench.KERNEL_SHA256 == build.kernel_hash()
     assert set(bench.INSTR) == {"crossing", "scattering", "absorption", "package"}
 
 
