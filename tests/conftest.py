@@ -24,3 +24,13 @@ def pytest_collection_modifyitems(config, items):
     for item in items:
         if "gpu" in item.keywords:
             item.add_marker(skip)
+
+
+# Lines the statistical parity tests want in the tail of the run whether they pass or not (how many shells needed
+# the second look of DESIGN.md R21): collected in tests/parity_notes.py, printed after the last test.
+def pytest_terminal_summary(terminalreporter):
+    import parity_notes
+    if parity_notes.NOTES:
+        terminalreporter.section("T(r) parity: shells flagged on seeds 1-8 (DESIGN.md R21)")
+        for line in parity_notes.NOTES:
+            terminalreporter.write_line(line)

@@ -237,21 +237,31 @@ def _T_outliers(To, Tg):
         return bad, (np.nonzero(bad)[0], (mg / mo)[bad], (np.abs(mg - mo) / se)[bad])
 
 
-def _check_T_parity(orc, p, n, model_kw=None, **kw):
+def _two_looks(label, stats):
     """north_star: per-shell T(r) within 1 % or 3 combined standard errors over 8 seeds, whichever is larger.
     With the standard error estimated from 8 + 8 samples a correct implementation still exceeds 3 se in ~1 % of
     the poorly sampled shells (Student t, ~14 degrees of freedom), i.e. in one of 32..200 shells in a good share of
     runs.  So a shell flagged on seeds 1..8 is re-examined on the independent seeds 9..16 and has to pass there: a
     real bias fails twice, a fluctuation fails twice in the same shell with probability ~1e-4.  At most 5 % of the
-    shells may need that second look."""
-    To, Tg = _ire_stats(orc, p, n, range(1, 9), model_kw, **kw)
+    shells may need that second look.  `stats(seeds)` returns (oracle T, GPU T), each seeds x shells.  How many shells
+    were flagged goes into the tail of the pytest run (tests/parity_notes.py), pass or fail."""
+    from parity_notes import note
+    To, Tg = stats(range(1, 9))
     bad, info = _T_outliers(To, Tg)
-    if not np.any(bad):
-        return
-    assert bad.sum() <= max(1, int(0.05 * len(bad))), info
-    To2, Tg2 = _ire_stats(orc, p, n, range(9, 17), model_kw, **kw)
-    bad2, info2 = _T_outliers(To2, Tg2)
-    assert not np.any(bad & bad2), (info, info2)
+    note(f"{label}: {int(bad.sum())} of {bad.size} shells flagged"
+         + (f" (shells {info[0].tolist()}, |dT|/se {np.round(info[2], 2).tolist()}): second look on seeds 9-16" if bad.any() else ""))
+    if np.any(bad):
+        assert bad.sum() <= max(1, int(0.05 * bad.size)), info
+        To2, Tg2 = stats(range(9, 17))
+        bad2, info2 = _T_outliers(To2, Tg2)
+        note(f"{label}: second look flags {int(bad2.sum())} shells, {int((bad & bad2).sum())} of them again")
+        assert not np.any(bad & bad2), (info, info2)
+    return To, Tg
+
+
+def _check_T_parity(orc, p, n, model_kw=None, **kw):
+    label = f"{p.name} n={n:g}" + "".join(f" {k}={v}" for k, v in kw.items())
+    _two_looks(label, lambda seeds: _ire_stats(orc, p, n, seeds, model_kw, **kw))
 
 
 @pytest.mark.parametrize("name,kw", [("plain", {}), ("kbg", dict(k_bg=0.2)), ("ffi", dict(ffi=1))])
@@ -485,13 +495,7 @@ def test_batch_full_ire_temperature_over_8_seeds(orc):
         m.close()
         return To.reshape(len(seeds), -1), Tg.reshape(len(seeds), -1)
 
-    To, Tg = stats(range(1, 9))
-    bad, info = _T_outliers(To, Tg)
-    if np.any(bad):
-        assert bad.sum() <= max(1, int(0.05 * bad.size)), info
-        To2, Tg2 = stats(range(9, 17))
-        bad2, info2 = _T_outliers(To2, Tg2)
-        assert not np.any(bad & bad2), (info, info2)
+    _two_looks("config5 reduced (4 spheres x 4e4)", stats)
 
 
 def test_smallest_dimensions(orc):
