@@ -37,6 +37,10 @@ from paper_2408_13807_b200 import sharding, synth  # noqa: E402
 # idle lanes are NOT work.  The constants belong to ONE version of the kernel sources: KERNEL_SHA256 is the hash they were
 # derived at, and a roofline is only printed while the sources still have it.
 INSTR = dict(crossing=8, scattering=174, absorption=345, package=260)
+# The same constants frozen at their round-2 values: `roofline.frac_frozen_r2` counts work with these whatever the
+# kernel has become, so that a leaner event routine shows as a gain and not as less counted work (INSTR itself is
+# re-derived after every kernel change and would shrink with the code).  Derived on config 2; applied to every workload.
+INSTR_FROZEN_R2 = dict(crossing=8, scattering=174, absorption=345, package=260)
 KERNEL_SHA256 = "a84e3db16bb33b0ed5791fb51d0a618d4104bd72c7814918120e8f7f5da46b41"
 # of the same ncu --set full capture (one dies_fly launch of config 2, 1e7 packages):
 # dram__bytes_read.sum + dram__bytes_write.sum; busy fractions of the XU pipe (MUFU.SQRT of the crossings, 8 cycles per
@@ -217,6 +221,15 @@ def run_ours(args, rank, world, local_rank):
     k_bg, ffi = getattr(p, "k_bg", 0.5), getattr(p, "ffi", 0)
     n_shells, n_freq, n_T = int(p.rho.shape[-1]), int(p.freq.size), int(p.T_grid.size)
     opts = dict(k_bg=k_bg, ffi=ffi)
+    weighted = {}
+    if args.run_opts:
+        # weighting of Table 1 for the timing table of BASELINE.md, e.g. k_A=3,k_S=2 or g_E=0.5,g_S=0.2 (dies_run_opts)
+        weighted = {k: float(v) for k, v in (kv.split("=") for kv in args.run_opts.split(","))}
+        if "reemit_cell" in weighted:
+            weighted["reemit_cell"] = int(weighted["reemit_cell"])
+        opts.update(weighted)
+        if any(k in weighted for k in ("k_A", "k_A_dilute", "k_S", "g_E", "g_S", "reemit_cell")):
+            opts["ffi"] = ffi = 0                           # weighting and forced first interaction are alternatives
     tmc = args.mode == "tmc"
     if tmc:
         # the second workload (R22): a step is one iteration of the traditional Monte Carlo with continuous
@@ -272,12 +285,25 @@ def run_ours(args, rank, world, local_rank):
     value = n_all * args.steps / (total_ms * 1e-3)
     crossings_per_s = sharding.sum_over_ranks(c1["crossings"], dev) * args.steps / (total_ms * 1e-3)
 
-    # ---- end to end through the C ABI with host buffers: create + sources + run + both getters
+    # ---- end to end through the C ABI with host buffers: create + sources + run + both getters.  The inputs sit in
+    #      pinned host memory (the binding passes their addresses through: numpy views of pinned torch tensors)
+    import dataclasses
+    pin = {f.name: torch.from_numpy(np.ascontiguousarray(getattr(p, f.name), dtype=np.float64)).pin_memory().numpy()
+           for f in dataclasses.fields(p) if isinstance(getattr(p, f.name), np.ndarray)}
+    p_pinned = dataclasses.replace(p, **pin)
+
+    def make_e2e():
+        if not batch:
+            return dies.Model(p_pinned, device=str(dev))
+        mm = dies.Model(batch=p_pinned, device=str(dev))
+        mm.dies_set_model_offset(model0)
+        return mm
+
     e2e_t = []
     for s in range(max(1, min(args.steps, 5))):
         torch.cuda.synchronize(dev)
         t0 = time.perf_counter()
-        m2 = make()
+        m2 = make_e2e()
         m2.dies_run(n_per_model, seed=1 + s, **opts)
         T = m2.dies_get_temperature()
         Lesc = m2.dies_get_escape_spectrum()
@@ -300,9 +326,12 @@ def run_ours(args, rank, world, local_rank):
                                    aggregate=1 if uniform_q else 0)
     sm_max, peak_src = load_peaks()
     peak = SM_COUNT * SCHEDULERS * LANES * sm_max * 1e6 / 1e12          # thread-instructions/s, 1e12
-    work = (c1["crossings"] * INSTR["crossing"] + c1["scatterings"] * INSTR["scattering"] +
-            c1["absorptions"] * INSTR["absorption"] + c1["packages"] * INSTR["package"])
-    achieved = work / (step_ms * 1e-3) / 1e12
+    def work_of(instr):
+        # (the crossings of the forced-first-interaction chord walk are crossings too: PAPER.md L132-149)
+        return ((c1["crossings"] + c1["ffi_crossings"]) * instr["crossing"] + c1["scatterings"] * instr["scattering"] +
+                c1["absorptions"] * instr["absorption"] + c1["packages"] * instr["package"])
+    achieved = work_of(INSTR) / (step_ms * 1e-3) / 1e12
+    achieved_frozen = work_of(INSTR_FROZEN_R2) / (step_ms * 1e-3) / 1e12
     held = clocks.get("sm_mhz") or sm_max
     from paper_2408_13807_b200 import build as dies_build
     stale = dies_build.kernel_hash() != KERNEL_SHA256
@@ -320,10 +349,12 @@ def run_ours(args, rank, world, local_rank):
                             grid=dict(**info)),
                 clocks=clocks,
                 e2e=dict(value=e2e_val, unit="packages/s", h2d_bytes_per_step=int(h2d), d2h_bytes_per_step=int(d2h),
-                         ms_per_step=1e3 * float(np.median(e2e_t))),
+                         ms_per_step=1e3 * float(np.median(e2e_t)), host_buffers="pinned inputs, pageable outputs"),
                 gpu_launches=int(2 * args.steps),
                 roofline=dict(bound="alu", achieved=achieved, peak=peak, unit="Tinstr/s", frac=achieved / peak,
-                              frac_at_held_clock=achieved / (peak * held / sm_max), traffic=TRAFFIC_BYTES_PER_LAUNCH,
+                              frac_at_held_clock=achieved / (peak * held / sm_max),
+                              frac_frozen_r2=achieved_frozen / peak, instr_per_unit_frozen_r2=INSTR_FROZEN_R2,
+                              traffic=TRAFFIC_BYTES_PER_LAUNCH,
                               atomic=dict(absorptions_per_s=c1["absorptions"] / (step_ms * 1e-3),
                                           peak_absorptions_per_s=atom["lane_ops_per_s"],
                                           peak_atomic_instr_per_s=atom["atomics_per_s"],
@@ -341,9 +372,17 @@ def run_ours(args, rank, world, local_rank):
         line["roofline"] = dict(bound="alu", achieved=None, peak=peak, unit="Tinstr/s", frac=None, traffic=None,
                                 kernel="dies_tmc", kernel_ms=step_ms,
                                 note="second workload: no work-per-unit constants were derived for dies_tmc")
+    elif weighted:
+        line["config"]["run_opts"] = weighted
+        line["roofline"] = dict(bound="alu", achieved=None, peak=peak, unit="Tinstr/s", frac=None, traffic=None,
+                                frac_frozen_r2=achieved_frozen / peak, instr_per_unit_frozen_r2=INSTR_FROZEN_R2,
+                                kernel="dies_track<0,false,true>", kernel_ms=step_ms,
+                                note="weighted run: dies_track, for which no work-per-unit constants were derived; the "
+                                     "frozen dies_fly constants count the same physical units")
     elif stale:
         # the work-per-unit constants were derived from other kernel sources: no fraction is claimed
         line["roofline"] = dict(bound="alu", achieved=None, peak=peak, unit="Tinstr/s", frac=None, traffic=None,
+                                frac_frozen_r2=achieved_frozen / peak, instr_per_unit_frozen_r2=INSTR_FROZEN_R2,
                                 stale="kernel sources changed since INSTR was derived: run an ncu source page through "
                                       "profile_parts.py and update INSTR and KERNEL_SHA256",
                                 kernel_ms=step_ms)
@@ -432,6 +471,7 @@ def main(argv=None):
     ap.add_argument("--ref-total", type=int, default=20_000_000)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--mode", default="ire", choices=["ire", "tmc"], help="full IRE (the headline) or one TMC iteration per step")
+    ap.add_argument("--run-opts", default="", help="dies_run options of a weighted run, e.g. k_A=3,k_S=2 (include/dies.h: dies_run_opts)")
     ap.add_argument("--tune", default="", help="launch tuning for dies_set_tuning, e.g. visit=2,slots_uniform=5 (include/dies.h: dies_tuning)")
     ap.add_argument("--cpu-all-cores", action="store_true", help="also time the oracle on all host cores (one process each)")
     ap.add_argument("--noise-study", action="store_true", help="configs 2, 3, 4: sigma_T and systematic error per radius decile over 8 seeds vs packages")
