@@ -42,6 +42,13 @@ INSTR = dict(crossing=8, scattering=174, absorption=345, package=260)
 # re-derived after every kernel change and would shrink with the code).  Derived on config 2; applied to every workload.
 INSTR_FROZEN_R2 = dict(crossing=8, scattering=174, absorption=345, package=260)
 KERNEL_SHA256 = "a84e3db16bb33b0ed5791fb51d0a618d4104bd72c7814918120e8f7f5da46b41"
+# The second workload, dies_tmc (python bench.py --mode tmc): predicated-on thread-instructions of the unit's own code per
+# unit, from profiles/r3_tmc_ncu_full.md (`python profile_parts.py source.csv --kernel tmc`); crossing = step +
+# continuous absorption (L37) + weight guard.  They belong to the csrc/dies_tmc.cuh that hashes to TMC_SHA256.
+INSTR_TMC = dict(crossing=115, scattering=380, package=575)
+TMC_SHA256 = "076ca0d2fcfb3783eb1dd2a3e72cde5f2223a480072ce0ccaad815180199bf27"
+TMC_TRAFFIC_BYTES_PER_LAUNCH = 263424
+TMC_NCU_PIPE_BUSY = dict(issue=0.876, smem_data=0.232)
 # of the same ncu --set full capture (one dies_fly launch of config 2, 1e7 packages):
 # dram__bytes_read.sum + dram__bytes_write.sum; busy fractions of the XU pipe (MUFU.SQRT of the crossings, 8 cycles per
 # warp instruction) and of the shared-memory data pipe (l1tex__data_pipe_lsu_wavefronts, 1 wavefront per cycle and SM)
@@ -369,9 +376,19 @@ def run_ours(args, rank, world, local_rank):
                 wall_s=t_wall)
     if tmc:
         line["config"]["mode"] = "TMC iteration (continuous absorption), steady state"
-        line["roofline"] = dict(bound="alu", achieved=None, peak=peak, unit="Tinstr/s", frac=None, traffic=None,
+        import hashlib
+        tmc_src = os.path.join(ROOT, "paper_2408_13807_b200", "csrc", "dies_tmc.cuh")
+        tmc_stale = hashlib.sha256(open(tmc_src, "rb").read()).hexdigest() != TMC_SHA256
+        w_tmc = (c1["crossings"] * INSTR_TMC["crossing"] + c1["scatterings"] * INSTR_TMC["scattering"] +
+                 c1["packages"] * INSTR_TMC["package"]) / (step_ms * 1e-3) / 1e12
+        line["roofline"] = dict(bound="alu", achieved=None if tmc_stale else w_tmc, peak=peak, unit="Tinstr/s",
+                                frac=None if tmc_stale else w_tmc / peak,
+                                traffic=None if tmc_stale else TMC_TRAFFIC_BYTES_PER_LAUNCH,
+                                ncu_pipe_busy=TMC_NCU_PIPE_BUSY, instr_per_unit=INSTR_TMC,
+                                peak_source=f"148 SMs x 4 schedulers x 32 lanes x {sm_max:.0f} MHz ({peak_src})",
                                 kernel="dies_tmc", kernel_ms=step_ms,
-                                note="second workload: no work-per-unit constants were derived for dies_tmc")
+                                note="second workload (DESIGN.md R22); constants from profiles/r3_tmc_ncu_full.md"
+                                     + ("; csrc/dies_tmc.cuh changed since: no fraction claimed" if tmc_stale else ""))
     elif weighted:
         line["config"]["run_opts"] = weighted
         line["roofline"] = dict(bound="alu", achieved=None, peak=peak, unit="Tinstr/s", frac=None, traffic=None,

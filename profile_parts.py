@@ -40,6 +40,16 @@ ANCHORS = [
     ("cross_end", "lc8 += pa - pb;"),
     ("flush", "// counters: flush before a 32-bit count can wrap"),
 ]
+# the second workload: dies_tmc (csrc/dies_tmc.cuh), chosen with --kernel tmc
+TMC_ANCHORS = [
+    ("launch", "// ---- idle lanes launch new packages together"),
+    ("cross", "// ---- kTmcSteps crossings of every active lane"),
+    ("scatter", "// ---- scattering (L85): truncate the step"),
+    ("guard", "if (w < 1e-10f) {"),
+    ("flush", "// ---- flush the block's privatised tallies"),
+]
+SRC = "dies_fly.cuh"          # file the parts are cut in (main() switches it for --kernel tmc)
+
 # sub-ranges inside the common event code that belong to one event type only
 SUB = [
     ("ev_abs", "int row;", "blk = b + 1u;", 2),          # rows of the table, extra Philox block, draw
@@ -71,7 +81,7 @@ def read_source_page(path: str):
             continue
         if r[0].strip().isdigit():                      # a source line; the SASS rows that belong to it follow
             ln = int(r[0])
-            if f == "dies_fly.cuh":
+            if f == SRC:
                 src.setdefault(ln, r[1])
             continue
         if r[0] == "" and r[2].startswith("0x") and len(r) > ix["# Samples"]:
@@ -83,7 +93,7 @@ def read_source_page(path: str):
     best = {}
     for row in sass:
         cur = best.get(row[0])
-        if cur is None or (row[1] == "dies_fly.cuh" and cur[1] != "dies_fly.cuh"):
+        if cur is None or (row[1] == SRC and cur[1] != SRC):
             best[row[0]] = row
     return src, sorted(best.values())
 
@@ -124,15 +134,15 @@ def table(path: str):
     src, sass = read_source_page(path)
     # the page lists only the lines that own instructions: the anchors are looked up in the file itself, which must
     # be the profiled one
-    disk = {i + 1: t.rstrip("\n") for i, t in enumerate(open(os.path.join(HERE, KERNEL_SOURCES[0])))}
+    disk = {i + 1: t.rstrip("\n") for i, t in enumerate(open(os.path.join(HERE, SRC)))}
     for ln, t in src.items():
         if not disk.get(ln, "").replace('"', "").strip().startswith(t.replace('"', "").strip()):   # (ncu drops the quotes)
-            raise SystemExit(f"csrc/dies_fly.cuh differs from the profiled source at line {ln}: re-profile this commit")
+            raise SystemExit(f"csrc/{SRC} differs from the profiled source at line {ln}: re-profile this commit")
     lp = part_of_lines(disk)
     agg, cur = {}, "setup"
     rows = []
     for addr, f, ln, text, inst, thr, on, smp in sass:
-        if f == "dies_fly.cuh" and lp.get(ln):
+        if f == SRC and lp.get(ln):
             cur = lp[ln]
         a = agg.setdefault(cur, [0.0, 0.0, 0.0, 0.0, 0])
         a[0] += inst; a[1] += thr; a[2] += on; a[3] += smp; a[4] += 1
@@ -146,7 +156,11 @@ def main(argv=None):
     ap.add_argument("--counts", type=float, nargs=4, metavar=("CROSSINGS", "SCATTERINGS", "ABSORPTIONS", "PACKAGES"),
                     help="event counts of the profiled launch (dies_get_counters)")
     ap.add_argument("--sass", action="store_true", help="list the SASS of the crossing block with its executed counts")
+    ap.add_argument("--kernel", default="fly", choices=["fly", "tmc"],
+                    help="fly: dies_fly (default); tmc: dies_tmc, --counts CROSSINGS SCATTERINGS 0 PACKAGES")
     a = ap.parse_args(argv)
+    if a.kernel == "tmc":
+        return main_tmc(a)
     agg, rows = table(a.source_csv)
     tot = sum(v[0] for v in agg.values()); smp = sum(v[3] for v in agg.values())
     print(f"kernel sources sha256 {kernel_hash()}")
@@ -181,6 +195,32 @@ def main(argv=None):
         for addr, p, text, inst, thr, on in rows:
             if p == "cross_step":
                 print(f"{addr & 0xfffff:6x} {inst:12.0f}  {text}")
+
+
+def main_tmc(a):
+    """dies_tmc: one lane follows one package, so the parts are simply launch / crossing step / scattering / guard."""
+    import hashlib
+    global SRC, ANCHORS, SUB
+    SRC, ANCHORS, SUB = "dies_tmc.cuh", TMC_ANCHORS, []
+    agg, rows = table(a.source_csv)
+    tot = sum(v[0] for v in agg.values()); smp = sum(v[3] for v in agg.values())
+    print(f"csrc/dies_tmc.cuh sha256 {hashlib.sha256(open(os.path.join(HERE, SRC), 'rb').read()).hexdigest()}")
+    print(f"total warp-instructions {tot:.6g}, samples {smp:.0f}")
+    print("| part | SASS instr | warp-instr % | samples % | active lanes | predicated-on lanes | pred-on thread-instr |")
+    print("|---|---|---|---|---|---|---|")
+    for p in ["setup", "launch", "cross", "scatter", "guard", "flush"]:
+        if p in agg:
+            v = agg[p]
+            print(f"| {p} | {v[4]} | {100 * v[0] / tot:.1f} | {100 * v[3] / max(smp, 1):.1f} | {v[1] / max(v[0], 1):.1f} | "
+                  f"{v[2] / max(v[0], 1):.1f} | {v[2]:.4g} |")
+    if a.counts:
+        nc, ns, _, npk = a.counts
+        get = lambda k: agg.get(k, [0] * 5)[2]
+        print(f"I_crossing   = {(get('cross') + get('guard')) / max(nc, 1):.1f}  (step + continuous absorption + guard, per crossing)")
+        print(f"I_scattering = {get('scatter') / max(ns, 1):.1f}")
+        print(f"I_package    = {get('launch') / max(npk, 1):.1f}")
+        work = get('cross') + get('guard') + get('scatter') + get('launch')
+        print(f"work {work:.4g} pred-on thread-instr = {100 * work / (32 * tot):.1f} % of the issued lane slots")
 
 
 if __name__ == "__main__":

@@ -111,6 +111,9 @@ def test_bench_constants_belong_to_the_kernel_sources():
     import bench
     assert bench.KERNEL_SHA256 == build.kernel_hash()
     assert set(bench.INSTR) == {"crossing", "scattering", "absorption", "package"}
+    import hashlib
+    tmc = os.path.join(ROOT, "paper_2408_13807_b200", "csrc", "dies_tmc.cuh")
+    assert bench.TMC_SHA256 == hashlib.sha256(open(tmc, "rb").read()).hexdigest()
 
 
 def test_build_sees_every_kernel_source(lib):
