@@ -45,10 +45,13 @@ KERNEL_SHA256 = "a84e3db16bb33b0ed5791fb51d0a618d4104bd72c7814918120e8f7f5da46b4
 # The second workload, dies_tmc (python bench.py --mode tmc): predicated-on thread-instructions of the unit's own code per
 # unit, from profiles/r3_tmc_ncu_full.md (`python profile_parts.py source.csv --kernel tmc`); crossing = step +
 # continuous absorption (L37) + weight guard.  They belong to the csrc/dies_tmc.cuh that hashes to TMC_SHA256.
-INSTR_TMC = dict(crossing=115, scattering=380, package=575)
-TMC_SHA256 = "076ca0d2fcfb3783eb1dd2a3e72cde5f2223a480072ce0ccaad815180199bf27"
-TMC_TRAFFIC_BYTES_PER_LAUNCH = 263424
-TMC_NCU_PIPE_BUSY = dict(issue=0.876, smem_data=0.232)
+INSTR_TMC = dict(crossing=102, scattering=154, package=537)
+TMC_SHA256 = "0e8fa2c536f7b5514b0e3a29466b046f67b3ef332e364f808a2d51c4c8e9ac2b"
+TMC_TRAFFIC_BYTES_PER_LAUNCH = 264192
+TMC_NCU_PIPE_BUSY = dict(issue=0.904, smem_data=0.281)
+# frozen at their first derivation (the kernel with the scattering inside the step loop, 8.15 ms per iteration): the
+# fraction under these does not shrink when the code gets leaner
+INSTR_TMC_FROZEN = dict(crossing=115, scattering=380, package=575)
 # of the same ncu --set full capture (one dies_fly launch of config 2, 1e7 packages):
 # dram__bytes_read.sum + dram__bytes_write.sum; busy fractions of the XU pipe (MUFU.SQRT of the crossings, 8 cycles per
 # warp instruction) and of the shared-memory data pipe (l1tex__data_pipe_lsu_wavefronts, 1 wavefront per cycle and SM)
@@ -379,11 +382,14 @@ def run_ours(args, rank, world, local_rank):
         import hashlib
         tmc_src = os.path.join(ROOT, "paper_2408_13807_b200", "csrc", "dies_tmc.cuh")
         tmc_stale = hashlib.sha256(open(tmc_src, "rb").read()).hexdigest() != TMC_SHA256
-        w_tmc = (c1["crossings"] * INSTR_TMC["crossing"] + c1["scatterings"] * INSTR_TMC["scattering"] +
-                 c1["packages"] * INSTR_TMC["package"]) / (step_ms * 1e-3) / 1e12
+        def tmc_work(instr):
+            return (c1["crossings"] * instr["crossing"] + c1["scatterings"] * instr["scattering"] +
+                    c1["packages"] * instr["package"]) / (step_ms * 1e-3) / 1e12
+        w_tmc = tmc_work(INSTR_TMC)
         line["roofline"] = dict(bound="alu", achieved=None if tmc_stale else w_tmc, peak=peak, unit="Tinstr/s",
                                 frac=None if tmc_stale else w_tmc / peak,
                                 traffic=None if tmc_stale else TMC_TRAFFIC_BYTES_PER_LAUNCH,
+                                frac_frozen=tmc_work(INSTR_TMC_FROZEN) / peak, instr_per_unit_frozen=INSTR_TMC_FROZEN,
                                 ncu_pipe_busy=TMC_NCU_PIPE_BUSY, instr_per_unit=INSTR_TMC,
                                 peak_source=f"148 SMs x 4 schedulers x 32 lanes x {sm_max:.0f} MHz ({peak_src})",
                                 kernel="dies_tmc", kernel_ms=step_ms,

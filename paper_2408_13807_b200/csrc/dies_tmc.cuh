@@ -13,14 +13,20 @@
 // exact q f however small it is (thin cells, weak sources, attenuated packages: rounding each step to the nearest
 // integer would leave nothing there and bias T low).  The launch quantum of a package is cut the same way.  The tallies of a block are privatised in shared memory.
 // Lanes that finished their package wait until a quarter of the warp is idle, then the idle lanes launch new packages
-// together.
+// together; lanes whose step ended in a scattering wait for the end of the round of kTmcSteps steps and scatter together.
 #pragma once
 #include "dies_tracker.cuh"
 
 namespace dies {
 
-constexpr int kTmcSteps = 8;          // crossings between two looks at the idle lanes
-constexpr int kTmcRefill = 8;         // idle lanes that trigger a refill
+#ifndef DIES_TMC_STEPS
+#define DIES_TMC_STEPS 12
+#endif
+#ifndef DIES_TMC_REFILL
+#define DIES_TMC_REFILL 8
+#endif
+constexpr int kTmcSteps = DIES_TMC_STEPS;    // crossings between two looks at the idle lanes and the pending scatterings
+constexpr int kTmcRefill = DIES_TMC_REFILL;  // idle lanes that trigger a refill
 
 struct TmcModel {
     const float* G;                   // nT x K: row CDFs of the emission spectra themselves (thermal spectrum of T_t)
@@ -109,7 +115,7 @@ __global__ void __launch_bounds__(kBlock, kMinBlocks) dies_tmc(DeviceModel D, Ru
 
         // per-lane package: id, bin k, opacities of the bin, coordinate a along the entry ahead, impact parameter^2,
         // table position, remaining scattering depth, remaining quantum, relative weight, Philox block
-        bool active = false;
+        bool active = false, pend = false;
         unsigned long long id = 0;
         int k = 0;
         float kapA = 0.f, kapS = 0.f, g = 0.f, a = 0.f, b2 = 0.f, tauS = 0.f, w = 0.f, acc = 0.f;
@@ -209,10 +215,22 @@ __global__ void __launch_bounds__(kBlock, kMinBlocks) dies_tmc(DeviceModel D, Ru
             }
             if (!__any_sync(kFull, active)) break;
 
-            // ---- kTmcSteps crossings of every active lane
+            // L119: a package ends below 1e-10 of its launch weight
+            auto guard = [&]() {
+                if (w < 1e-10f) {
+                    if (mp.cav && pa == tab0) lc_cross++;        // (ended on the wall of the cavity: R10 counts its passage whole)
+                    lc_termraw += qrem;
+                    lc_term++;
+                    active = false;
+                }
+            };
+
+            // ---- kTmcSteps crossings of every active lane.  A lane whose step ends in a scattering waits (pend) for
+            //      the end of the round: the scattering code then runs once for all such lanes of the warp together
+            //      instead of inside the step loop at two or three active lanes.
 #pragma unroll 1
             for (int u = 0; u < kTmcSteps; u++) {
-                if (!active) continue;
+                if (!active || pend) continue;
                 const float2 T = lds_entry(pa);
                 const float d = T.x - b2;
                 if (d < 0.f) {
@@ -237,45 +255,48 @@ __global__ void __launch_bounds__(kBlock, kMinBlocks) dies_tmc(DeviceModel D, Ru
                 if (dq) smem_add64(&s_A[j], &s_A[ldS + j], (unsigned long long)dq);
                 qrem -= dq;
                 w *= expf(-dtA);                                 // (not 1 - frac: that cancels when little is left)
-                if (!event) {
-                    tauS -= dtauS;
-                    a = an;
-                    pa += 8u;
-                    lc_cross++;
-                    if (pa == pa_out) {
-                        // the outer surface: the package leaves the model (L87 last sentence)
-                        if (qrem) smem_add64(&s_esc[k], &s_esc[K + k], (unsigned long long)qrem);
-                        lc_esc++;
-                        active = false;
-                        continue;
-                    }
-                } else {
-                    // ---- scattering (L85): truncate the step, new direction from the HG function of the bin
-                    const float ae = fmaf(f, an - a, a);
-                    const float se = (pa <= tab0) ? -ae : ae;
-                    const float re2 = fmaf(se, se, b2);
-                    const float re = sqrtf(re2);
-                    float mu0 = re > 0.f ? se / re : 1.f;
-                    mu0 = fminf(1.f, fmaxf(-1.f, mu0));
-                    uint32_t xw[4];
-                    philox4x32_10_rk(R.rk, (uint32_t)id, (uint32_t)(id >> 32), blk++, (uint32_t)m + R.model0, xw);
-                    const float ct = hg_cos(g, uniform24(xw[0]));
-                    const float sm = sqrtf(fmaxf(1.f - mu0 * mu0, 0.f)), sth = sqrtf(fmaxf(1.f - ct * ct, 0.f));
-                    float mu = mu0 * ct + sm * sth * cospif(2.f * uniform24(xw[1]));
-                    mu = fminf(1.f, fmaxf(-1.f, mu));
-                    tauS = neg_log(uniform24(xw[2]));
-                    const float s = re * mu;
-                    b2 = fminf(re2 * (1.f - mu) * (1.f + mu), lds_entry(tab0 + 8u * (unsigned)(j + 1)).x);
-                    pa = tab0 + 8u * (unsigned)((s < 0.f) ? -j : j + 1);
-                    a = fabsf(s);
-                    lc_sca++;
+                if (event) {
+                    // scattering (L85): the step is truncated at the event; the new direction follows after the round
+                    a = fmaf(f, an - a, a);
+                    pend = true;
+                    continue;
                 }
-                if (w < 1e-10f) {                                // L119
-                    if (mp.cav && pa == tab0) lc_cross++;        // (ended on the wall of the cavity: R10 counts its passage whole)
-                    lc_termraw += qrem;
-                    lc_term++;
+                tauS -= dtauS;
+                a = an;
+                pa += 8u;
+                lc_cross++;
+                if (pa == pa_out) {
+                    // the outer surface: the package leaves the model (L87 last sentence)
+                    if (qrem) smem_add64(&s_esc[k], &s_esc[K + k], (unsigned long long)qrem);
+                    lc_esc++;
                     active = false;
+                    continue;
                 }
+                guard();
+            }
+            if (pend) {
+                // ---- scattering (L85): new direction from the HG function of the bin, at the truncated position
+                const int c = (int)(pa - tab0) / 8;
+                const int j = c <= 0 ? -c : c - 1;
+                const float se = (pa <= tab0) ? -a : a;
+                const float re2 = fmaf(se, se, b2);
+                const float re = sqrtf(re2);
+                float mu0 = re > 0.f ? se / re : 1.f;
+                mu0 = fminf(1.f, fmaxf(-1.f, mu0));
+                uint32_t xw[4];
+                philox4x32_10_rk(R.rk, (uint32_t)id, (uint32_t)(id >> 32), blk++, (uint32_t)m + R.model0, xw);
+                const float ct = hg_cos(g, uniform24(xw[0]));
+                const float sm = sqrtf(fmaxf(1.f - mu0 * mu0, 0.f)), sth = sqrtf(fmaxf(1.f - ct * ct, 0.f));
+                float mu = mu0 * ct + sm * sth * cospif(2.f * uniform24(xw[1]));
+                mu = fminf(1.f, fmaxf(-1.f, mu));
+                tauS = neg_log(uniform24(xw[2]));
+                const float s = re * mu;
+                b2 = fminf(re2 * (1.f - mu) * (1.f + mu), lds_entry(tab0 + 8u * (unsigned)(j + 1)).x);
+                pa = tab0 + 8u * (unsigned)((s < 0.f) ? -j : j + 1);
+                a = fabsf(s);
+                lc_sca++;
+                pend = false;
+                guard();
             }
         }
         // ---- flush the block's privatised tallies

@@ -43,9 +43,9 @@ ANCHORS = [
 # the second workload: dies_tmc (csrc/dies_tmc.cuh), chosen with --kernel tmc
 TMC_ANCHORS = [
     ("launch", "// ---- idle lanes launch new packages together"),
+    ("guard", "// L119: a package ends below 1e-10"),             # (a lambda, inlined after the step and the scattering)
     ("cross", "// ---- kTmcSteps crossings of every active lane"),
-    ("scatter", "// ---- scattering (L85): truncate the step"),
-    ("guard", "if (w < 1e-10f) {"),
+    ("scatter", "// ---- scattering (L85): new direction"),
     ("flush", "// ---- flush the block's privatised tallies"),
 ]
 SRC = "dies_fly.cuh"          # file the parts are cut in (main() switches it for --kernel tmc)
